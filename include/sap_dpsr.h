@@ -1,0 +1,117 @@
+/*
+ * sap_dpsr.h -- C ABI of the B200-native DPSR layer (Shape As Points, arXiv 2106.03452).
+ *
+ * DPSR = differentiable Poisson surface reconstruction: an oriented point cloud {(c_i, n_i)} is
+ * mapped to an indicator grid chi in R^{N x N x N} (Sec.3.1; Suppl. A, L337-L388)
+ * and the map is differentiable w.r.t. points and normals (L17; third factor of Eq.5).
+ * "PAPER.md:Lnnn" cites /root/reference/PAPER.md.  Readings R1..R14 of the paper: DESIGN.md.
+ *
+ * Every step runs in hand-written sm_100a CUDA kernels inside libsap_dpsr.so; there is no CPU or
+ * library (cuFFT) fallback.  All entry points return a status code and never throw or abort.
+ *
+ * Conventions
+ *   - Layout: C order, z fastest.  chi[b][jx][jy][jz] is the value at position (jx, jy, jz)/N of
+ *     the unit cube [0,1)^3 (R1: origin 0, voxel 1/N, periodic).
+ *   - Pointers marked "dev" are CUDA device pointers valid on the handle's device; "host" are
+ *     ordinary host pointers (pinned memory makes the *_host calls asynchronous copies).
+ *   - The caller owns every buffer it passes and the stream.  The handle owns its workspace,
+ *     allocated once in sap_dpsr_create; forward/backward never allocate.
+ *   - Work is enqueued on `stream` (a cudaStream_t cast to void*, NULL = default stream) and NOT
+ *     synchronised, except where stated.  Device-side faults surface at the caller's next sync.
+ *   - Preconditions not checked on the device: coordinates finite and in [0,1) (indices are wrapped
+ *     mod N, nothing is ever written out of bounds).  If the shifted corner value a = chi'[0,0,0]-mu
+ *     is 0 the scale is inf and chi is inf/NaN as IEEE dictates.
+ *   - A handle is not thread-safe; use one handle per stream.
+ */
+#ifndef SAP_DPSR_H
+#define SAP_DPSR_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sap_dpsr sap_dpsr_t; /* opaque */
+
+typedef enum {
+    SAP_OK = 0,
+    SAP_ERR_INVALID_ARG = 1, /* null pointer, non-positive size, sigma < 0 or non-finite, num_points out of range */
+    SAP_ERR_UNSUPPORTED = 2, /* N not in {32, 64, 128, 256, 512}; device is not sm_100 */
+    SAP_ERR_OOM = 3,         /* workspace allocation failed */
+    SAP_ERR_CUDA = 4         /* launch / runtime error; see sap_dpsr_last_error */
+} sap_status_t;
+
+/*
+ * Create a solver for grids of N^3 (N in {32,64,128,256,512}: the resolutions of the paper's
+ * coarse-to-fine schedule, plus 512), Gaussian bandwidth sigma >= 0 of Eq.3
+ * (sigma = 0 means no filter, L460), `batch` independent shapes per call (the
+ * learning setting uses 32, L419) and at most max_points points per shape.  The scale m of Eq.2 is
+ * fixed to 0.5 (L77).  Allocates the workspace (about 9 N^3 floats per batch item) on the current
+ * CUDA device.  *out is set only on SAP_OK.
+ */
+sap_status_t sap_dpsr_create(int N, float sigma, int batch, int max_points, sap_dpsr_t** out);
+
+/*
+ * Forward, Eq.2-4 = Eq.10-18 (L341-L388):
+ *   splat normals with trilinear weights (Eq.10-11) -> 3 real-to-complex 3-D FFTs (Eq.12) ->
+ *   chi~ = g_sigma(u) * i u.v~ / (-2 pi |u|^2), chi~(0) = 0 (Eq.3/16) -> inverse FFT (Eq.17) ->
+ *   chi = s (chi' - mu), mu = mean over the points of the trilinear sample of chi',
+ *   s = 0.5 / |chi'[0,0,0] - mu| (Eq.4/18, reading R5).
+ *   points   dev [batch][num_points][3] float, coordinates in [0,1)
+ *   normals  dev [batch][num_points][3] float, any magnitude (L494)
+ *   num_points 1 <= num_points <= max_points, the same for every item of the batch
+ *   chi      dev [batch][N][N][N] float, overwritten
+ * The handle remembers (mu, a, s) per item and the point density W for the backward.
+ */
+sap_status_t sap_dpsr_forward(sap_dpsr_t* h, const float* points, const float* normals,
+                              int num_points, float* chi, void* stream);
+
+/*
+ * Backward: the exact adjoint of sap_dpsr_forward (dL/dpoints, dL/dnormals from dL/dchi); must
+ * follow, on the same handle, the forward call it differentiates, with the same points/normals
+ * and that call's chi, unmodified.  Derivation: DESIGN.md "Backward".
+ *   chi          dev [batch][N][N][N]   forward output
+ *   grad_chi     dev [batch][N][N][N]   dL/dchi
+ *   grad_points  dev [batch][num_points][3], overwritten
+ *   grad_normals dev [batch][num_points][3], overwritten
+ */
+sap_status_t sap_dpsr_backward(sap_dpsr_t* h, const float* points, const float* normals,
+                               int num_points, const float* chi, const float* grad_chi,
+                               float* grad_points, float* grad_normals, void* stream);
+
+/*
+ * Host-buffer variants (the end-to-end path): the same computation with HOST pointers.  Inputs are
+ * copied to handle-owned device staging buffers with cudaMemcpyAsync on `stream`, the kernels run,
+ * and the outputs are copied back; the call returns after synchronising `stream`.
+ * sap_dpsr_forward_host keeps chi on the device inside the handle for the backward that follows;
+ * chi_host may be NULL to skip the device->host copy of chi.
+ */
+sap_status_t sap_dpsr_forward_host(sap_dpsr_t* h, const float* points_host,
+                                   const float* normals_host, int num_points, float* chi_host,
+                                   void* stream);
+sap_status_t sap_dpsr_backward_host(sap_dpsr_t* h, const float* grad_chi_host,
+                                    float* grad_points_host, float* grad_normals_host,
+                                    void* stream);
+
+/* Copies the per-item statistics of the last forward to host: stats_host[batch][3] = {mu, a, s}.
+ * Synchronises `stream`. */
+sap_status_t sap_dpsr_get_stats(sap_dpsr_t* h, float* stats_host, void* stream);
+
+/* Frees the workspace and the handle.  NULL is allowed. */
+void sap_dpsr_destroy(sap_dpsr_t* h);
+
+/* Message of the last error on this handle ("" if none); the string is owned by the handle.
+ * With h == NULL returns the message of the last failed sap_dpsr_create on this thread. */
+const char* sap_dpsr_last_error(const sap_dpsr_t* h);
+
+/* Bytes of device workspace owned by the handle. */
+size_t sap_dpsr_workspace_bytes(const sap_dpsr_t* h);
+
+/* Number of kernel launches the last forward / backward call enqueued (for bench.py's gpu_launches). */
+int sap_dpsr_last_launch_count(const sap_dpsr_t* h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SAP_DPSR_H */

@@ -1,0 +1,267 @@
+// fft_core.cuh -- in-shared-memory radix FFT building blocks for the DPSR kernels (sm_100a).
+//
+// All FFTs of the path (Eq.12/13/17) are power-of-two lengths 16..512 done on
+// lines that live in shared memory.  The forward transform is decimation-in-frequency, in place,
+// natural order in -> digit-reversed ("stored") order out; the inverse is the exact mirror
+// (decimation-in-time, stored order in -> natural order out).  Because every butterfly reads and
+// writes the same R slots, a stage has no intra-stage hazards: one block barrier between stages is
+// all the synchronisation there is.  Spectra are kept in stored order in HBM on all three axes; only
+// the spectral solve needs to know which frequency a slot holds (pos2freq).
+//
+// The functions are __host__ __device__ so that the same source can be exercised thread-by-thread
+// by a host harness; the product only ever runs them on the device.
+#pragma once
+#include <cuda_runtime.h>
+
+#define SAP_HD __host__ __device__ __forceinline__
+
+namespace sap {
+
+SAP_HD float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
+SAP_HD float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+SAP_HD float2 cmul(float2 a, float2 w) { return make_float2(a.x * w.x - a.y * w.y, a.x * w.y + a.y * w.x); }
+// a * conj(w)
+SAP_HD float2 cmulc(float2 a, float2 w) { return make_float2(a.x * w.x + a.y * w.y, a.y * w.x - a.x * w.y); }
+// a * (-i)
+SAP_HD float2 mul_mi(float2 a) { return make_float2(a.y, -a.x); }
+
+// ---- radix plans: N = R0 * R1 * R2 -------------------------------------------------------------
+template <int N> struct Plan;
+template <> struct Plan<16>  { static constexpr int NS = 1, R0 = 16, R1 = 1,  R2 = 1; };
+template <> struct Plan<32>  { static constexpr int NS = 2, R0 = 8,  R1 = 4,  R2 = 1; };
+template <> struct Plan<64>  { static constexpr int NS = 2, R0 = 8,  R1 = 8,  R2 = 1; };
+template <> struct Plan<128> { static constexpr int NS = 2, R0 = 8,  R1 = 16, R2 = 1; };
+template <> struct Plan<256> { static constexpr int NS = 2, R0 = 16, R1 = 16, R2 = 1; };
+template <> struct Plan<512> { static constexpr int NS = 3, R0 = 8,  R1 = 8,  R2 = 8; };
+
+template <int N, int S> struct StageInfo {
+    using P = Plan<N>;
+    static constexpr int R = (S == 0) ? P::R0 : (S == 1) ? P::R1 : P::R2;
+    // butterfly stride of stage S: N / (R0 * ... * RS)
+    static constexpr int ST = (S == 0) ? N / P::R0 : (S == 1) ? N / (P::R0 * P::R1) : N / (P::R0 * P::R1 * P::R2);
+};
+
+// slot p (stored order) of a forward-transformed line holds frequency pos2freq<N>(p)
+template <int N> SAP_HD int pos2freq(int p) {
+    using P = Plan<N>;
+    constexpr int st0 = N / P::R0;
+    constexpr int st1 = st0 / P::R1;
+    int k0 = p / st0;
+    int r = p - k0 * st0;
+    int k1 = r / st1;
+    int k2 = r - k1 * st1;
+    return k0 + P::R0 * (k1 + P::R1 * k2);
+}
+template <int N> SAP_HD int freq2pos(int k) {
+    using P = Plan<N>;
+    constexpr int st0 = N / P::R0;
+    constexpr int st1 = st0 / P::R1;
+    int k0 = k % P::R0;
+    int r = k / P::R0;
+    int k1 = r % P::R1;
+    int k2 = r / P::R1;
+    return k0 * st0 + k1 * st1 + k2;
+}
+
+// ---- register butterflies: forward DFT of R values, natural order in and out ------------------
+template <int R> SAP_HD float2 unit_root(int k);  // exp(-2 pi i k / R), k < R/2
+template <> SAP_HD float2 unit_root<8>(int k) {
+    switch (k) {
+        case 0: return make_float2(1.f, 0.f);
+        case 1: return make_float2(0.70710678118654752f, -0.70710678118654752f);
+        case 2: return make_float2(0.f, -1.f);
+        default: return make_float2(-0.70710678118654752f, -0.70710678118654752f);
+    }
+}
+template <> SAP_HD float2 unit_root<16>(int k) {
+    switch (k) {
+        case 0: return make_float2(1.f, 0.f);
+        case 1: return make_float2(0.92387953251128674f, -0.38268343236508977f);
+        case 2: return make_float2(0.70710678118654752f, -0.70710678118654752f);
+        case 3: return make_float2(0.38268343236508977f, -0.92387953251128674f);
+        case 4: return make_float2(0.f, -1.f);
+        case 5: return make_float2(-0.38268343236508977f, -0.92387953251128674f);
+        case 6: return make_float2(-0.70710678118654752f, -0.70710678118654752f);
+        default: return make_float2(-0.92387953251128674f, -0.38268343236508977f);
+    }
+}
+
+template <int R> SAP_HD void dft_fwd(float2 (&v)[R]) {
+    if constexpr (R == 1) {
+    } else if constexpr (R == 2) {
+        float2 a = v[0], b = v[1];
+        v[0] = cadd(a, b);
+        v[1] = csub(a, b);
+    } else if constexpr (R == 4) {
+        float2 t0 = cadd(v[0], v[2]), t1 = csub(v[0], v[2]);
+        float2 t2 = cadd(v[1], v[3]), t3 = mul_mi(csub(v[1], v[3]));
+        v[0] = cadd(t0, t2);
+        v[2] = csub(t0, t2);
+        v[1] = cadd(t1, t3);
+        v[3] = csub(t1, t3);
+    } else {
+        float2 e[R / 2], o[R / 2];
+#pragma unroll
+        for (int i = 0; i < R / 2; ++i) { e[i] = v[2 * i]; o[i] = v[2 * i + 1]; }
+        dft_fwd<R / 2>(e);
+        dft_fwd<R / 2>(o);
+#pragma unroll
+        for (int k = 0; k < R / 2; ++k) {
+            float2 t;
+            if (k == 0) t = o[k];
+            else if (k == R / 4) t = mul_mi(o[k]);
+            else t = cmul(o[k], unit_root<R>(k));
+            v[k] = cadd(e[k], t);
+            v[k + R / 2] = csub(e[k], t);
+        }
+    }
+}
+// inverse (unnormalised) DFT: swap re/im, forward, swap back
+template <int R> SAP_HD void dft_inv(float2 (&v)[R]) {
+#pragma unroll
+    for (int i = 0; i < R; ++i) { float t = v[i].x; v[i].x = v[i].y; v[i].y = t; }
+    dft_fwd<R>(v);
+#pragma unroll
+    for (int i = 0; i < R; ++i) { float t = v[i].x; v[i].x = v[i].y; v[i].y = t; }
+}
+
+// ---- one radix stage over a set of lines in shared memory --------------------------------------
+// Element n of line l lives at s[l * LS + n * ES].  tw is the table exp(-2 pi i t / TWN), t < TWN,
+// TWN a multiple of N.  LANES_LINES: consecutive threads take consecutive lines (same butterfly),
+// else consecutive threads take consecutive butterflies of one line.
+template <int N, int S, bool INV, int TWN, bool LANES_LINES>
+SAP_HD void fft_stage(float2* s, int ES, int LS, int nlines, const float2* tw, int tid, int nthr) {
+    constexpr int R = StageInfo<N, S>::R;
+    constexpr int ST = StageInfo<N, S>::ST;
+    constexpr int Q = N / R;               // butterflies per line
+    constexpr int TWMUL = TWN / (R * ST);  // w_{R*ST}^e = tw[e * TWMUL]
+    const int ntasks = nlines * Q;
+    for (int t = tid; t < ntasks; t += nthr) {
+        int line, q;
+        if (LANES_LINES) { q = t / nlines; line = t - q * nlines; }
+        else { line = t / Q; q = t - line * Q; }
+        const int blk = q / ST;
+        const int j = q - blk * ST;
+        float2* base = s + line * LS + (blk * (R * ST) + j) * ES;
+        float2 v[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) v[r] = base[r * ST * ES];
+        if (!INV) {
+            dft_fwd<R>(v);
+            if (ST > 1) {
+#pragma unroll
+                for (int r = 1; r < R; ++r) v[r] = cmul(v[r], tw[r * j * TWMUL]);
+            }
+        } else {
+            if (ST > 1) {
+#pragma unroll
+                for (int r = 1; r < R; ++r) v[r] = cmulc(v[r], tw[r * j * TWMUL]);
+            }
+            dft_inv<R>(v);
+        }
+#pragma unroll
+        for (int r = 0; r < R; ++r) base[r * ST * ES] = v[r];
+    }
+}
+
+// Whole transform of `nlines` lines: all stages with a barrier after each.
+// Forward: stages 0..NS-1 (DIF).  Inverse: stages NS-1..0 (DIT).
+template <int N, bool INV, int TWN, bool LANES_LINES, class Ctx>
+SAP_HD void fft_lines(Ctx& ctx, float2* s, int ES, int LS, int nlines, const float2* tw) {
+    constexpr int NS = Plan<N>::NS;
+    if (!INV) {
+        fft_stage<N, 0, false, TWN, LANES_LINES>(s, ES, LS, nlines, tw, ctx.tid, ctx.nthr);
+        ctx.sync();
+        if constexpr (NS > 1) {
+            fft_stage<N, 1, false, TWN, LANES_LINES>(s, ES, LS, nlines, tw, ctx.tid, ctx.nthr);
+            ctx.sync();
+        }
+        if constexpr (NS > 2) {
+            fft_stage<N, 2, false, TWN, LANES_LINES>(s, ES, LS, nlines, tw, ctx.tid, ctx.nthr);
+            ctx.sync();
+        }
+    } else {
+        if constexpr (NS > 2) {
+            fft_stage<N, 2, true, TWN, LANES_LINES>(s, ES, LS, nlines, tw, ctx.tid, ctx.nthr);
+            ctx.sync();
+        }
+        if constexpr (NS > 1) {
+            fft_stage<N, 1, true, TWN, LANES_LINES>(s, ES, LS, nlines, tw, ctx.tid, ctx.nthr);
+            ctx.sync();
+        }
+        fft_stage<N, 0, true, TWN, LANES_LINES>(s, ES, LS, nlines, tw, ctx.tid, ctx.nthr);
+        ctx.sync();
+    }
+}
+
+// ---- real <-> half-complex split for a length-N real line done as an H = N/2 point complex FFT --
+// After the forward H-point FFT, slot pos(k) holds Z[k] = E[k] + i O[k] (E, O = DFTs of the even and
+// odd samples).  X[k] = E[k] + w^k O[k], w = exp(-2 pi i / N), k = 0..H.  In place: X[k] goes to slot
+// pos(k) (k < H) and X[H] to the extra row H.  One task handles the pair (k, H-k).
+// Rows are at s[row * RS + line * LS].
+template <int N, int TWN, class Ctx>
+SAP_HD void r2c_split(Ctx& ctx, float2* s, int RS, int LS, int nlines, const float2* tw) {
+    constexpr int H = N / 2;
+    constexpr int TWMUL = TWN / N;
+    const int ntasks = nlines * (H / 2 + 1);
+    for (int t = ctx.tid; t < ntasks; t += ctx.nthr) {
+        const int k = t / nlines;
+        const int line = t - k * nlines;
+        float2* col = s + line * LS;
+        if (k == 0) {
+            float2 z = col[0];  // pos(0) = 0
+            col[0] = make_float2(z.x + z.y, 0.f);
+            col[H * RS] = make_float2(z.x - z.y, 0.f);
+        } else if (k == H / 2) {
+            float2* p = col + freq2pos<H>(k) * RS;
+            float2 z = *p;
+            *p = make_float2(z.x, -z.y);
+        } else {
+            float2* pa = col + freq2pos<H>(k) * RS;
+            float2* pb = col + freq2pos<H>(H - k) * RS;
+            float2 a = *pa, b = *pb;
+            float2 e = make_float2(0.5f * (a.x + b.x), 0.5f * (a.y - b.y));  // (A + conj B)/2
+            float2 d = make_float2(0.5f * (a.x - b.x), 0.5f * (a.y + b.y));  // (A - conj B)/2
+            float2 wd = cmul(d, tw[k * TWMUL]);
+            float2 f = make_float2(-wd.y, wd.x);  // i w^k D
+            *pa = csub(e, f);                     // X[k]   = E - F
+            float2 g = cadd(e, f);
+            *pb = make_float2(g.x, -g.y);         // X[H-k] = conj(E + F)
+        }
+    }
+}
+
+// Inverse of r2c_split: from X[k] (slot pos(k), k < H; X[H] in row H) rebuild Z[k] = E[k] + i O[k] in
+// place.  The unnormalised inverse H-point FFT of Z then gives (N/2) * (x[2m] + i x[2m+1]).
+template <int N, int TWN, class Ctx>
+SAP_HD void c2r_split(Ctx& ctx, float2* s, int RS, int LS, int nlines, const float2* tw) {
+    constexpr int H = N / 2;
+    constexpr int TWMUL = TWN / N;
+    const int ntasks = nlines * (H / 2 + 1);
+    for (int t = ctx.tid; t < ntasks; t += ctx.nthr) {
+        const int k = t / nlines;
+        const int line = t - k * nlines;
+        float2* col = s + line * LS;
+        if (k == 0) {
+            float x0 = col[0].x, xh = col[H * RS].x;
+            col[0] = make_float2(0.5f * (x0 + xh), 0.5f * (x0 - xh));
+        } else if (k == H / 2) {
+            float2* p = col + freq2pos<H>(k) * RS;
+            float2 x = *p;
+            *p = make_float2(x.x, -x.y);
+        } else {
+            float2* pa = col + freq2pos<H>(k) * RS;
+            float2* pb = col + freq2pos<H>(H - k) * RS;
+            float2 a = *pa, b = *pb;                                         // X[k], X[H-k]
+            float2 e = make_float2(0.5f * (a.x + b.x), 0.5f * (a.y - b.y));  // E = (X[k] + conj X[H-k])/2
+            float2 d = make_float2(0.5f * (a.x - b.x), 0.5f * (a.y + b.y));  // w^k O = (X[k] - conj X[H-k])/2
+            float2 o = cmulc(d, tw[k * TWMUL]);                              // O = conj(w^k) * d
+            float2 io = make_float2(-o.y, o.x);                              // i O
+            *pa = cadd(e, io);                                               // Z[k]   = E + i O
+            float2 g = csub(e, io);
+            *pb = make_float2(g.x, -g.y);                                    // Z[H-k] = conj(E - i O)
+        }
+    }
+}
+
+}  // namespace sap
