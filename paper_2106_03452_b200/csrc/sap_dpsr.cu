@@ -1,0 +1,635 @@
+// sap_dpsr.cu -- the C-ABI library of the B200-native DPSR layer (include/sap_dpsr.h).
+// Kernels: splat (F1), z/y/x FFT passes with the fused spectral solve (F2-F4, B3-B5), normalisation
+// (F5), grid reductions (B1), Gbar' assembly fused into the first backward pass (B2), gather (B6).
+// Step names F1..B6: SURVEY.md 8(a).  No cuFFT, no CPU fallback.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+#include <new>
+#include <string>
+
+#include "../../include/sap_dpsr.h"
+#include "dpsr_kernels.cuh"
+
+namespace sap {
+
+struct DevCtx {
+    int tid, nthr;
+    __device__ __forceinline__ void sync() const { __syncthreads(); }
+};
+
+// ------------------------------------------------------------------------------------------------
+// __global__ wrappers around the block bodies
+// ------------------------------------------------------------------------------------------------
+template <int N, int NL, bool DO_Y, bool GBAR, int NT>
+__global__ void __launch_bounds__(NT) k_zy_fwd(ZyFwdParams p) {
+    extern __shared__ float2 smem[];
+    DevCtx ctx{(int)threadIdx.x, NT};
+    zy_fwd_body<N, NL, DO_Y, GBAR>(ctx, p, smem, (int)blockIdx.x, (int)blockIdx.y);
+}
+template <int N, int NL, bool DO_Y, int NT>
+__global__ void __launch_bounds__(NT) k_zy_inv(ZyInvParams p) {
+    extern __shared__ float2 smem[];
+    DevCtx ctx{(int)threadIdx.x, NT};
+    zy_inv_body<N, NL, DO_Y>(ctx, p, smem, (int)blockIdx.x, (int)blockIdx.y);
+}
+template <int N, int MODE, int NT>
+__global__ void __launch_bounds__(NT) k_strided(StridedParams p) {
+    extern __shared__ float2 smem[];
+    DevCtx ctx{(int)threadIdx.x, NT};
+    strided_body<N, MODE>(ctx, p, smem, (int)blockIdx.x, (int)blockIdx.y);
+}
+
+// ------------------------------------------------------------------------------------------------
+// pointwise / point kernels
+// ------------------------------------------------------------------------------------------------
+__global__ void k_zero(float4* __restrict__ p, size_t n4) {
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += stride)
+        p[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+}
+
+struct Corner {
+    int j0[3];
+    float f[3];
+};
+// t = c N, j0 = floor(t), f = t - j0 (Eq.10-11; readings R1/R2).  N is a power
+// of two, so t, floor and f are exact in fp32.
+__device__ __forceinline__ Corner corner_of(const float* __restrict__ c, int N) {
+    Corner k;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const float t = c[a] * (float)N;
+        const float fl = floorf(t);
+        k.j0[a] = (int)fl;
+        k.f[a] = t - fl;
+    }
+    return k;
+}
+__device__ __forceinline__ size_t vox(int N, int jx, int jy, int jz) {
+    const int M = N - 1;  // periodic wrap (R1)
+    return ((size_t)(jx & M) * N + (jy & M)) * N + (jz & M);
+}
+
+// F1: v[ch][j] += w n[ch], W[j] += w over the 8 neighbours.  One thread per point; global RED.
+__global__ void k_splat(const float* __restrict__ pts, const float* __restrict__ nrm, int P, int N,
+                        float* __restrict__ v, float* __restrict__ W) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int b = blockIdx.y;
+    if (i >= P) return;
+    const size_t V = (size_t)N * N * N;
+    const float* c = pts + ((size_t)b * P + i) * 3;
+    const float* n = nrm + ((size_t)b * P + i) * 3;
+    const Corner k = corner_of(c, N);
+    const float n0 = n[0], n1 = n[1], n2 = n[2];
+    float* vb = v + (size_t)b * 3 * V;
+    float* Wb = W + (size_t)b * V;
+#pragma unroll
+    for (int d = 0; d < 8; ++d) {
+        const int dx = d >> 2, dy = (d >> 1) & 1, dz = d & 1;
+        const float w = (dx ? k.f[0] : 1.f - k.f[0]) * (dy ? k.f[1] : 1.f - k.f[1]) * (dz ? k.f[2] : 1.f - k.f[2]);
+        const size_t j = vox(N, k.j0[0] + dx, k.j0[1] + dy, k.j0[2] + dz);
+        atomicAdd(vb + j, w * n0);
+        atomicAdd(vb + V + j, w * n1);
+        atomicAdd(vb + 2 * V + j, w * n2);
+        atomicAdd(Wb + j, w);
+    }
+}
+
+__device__ __forceinline__ float warp_sum(float x) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+    return x;
+}
+// block sum of one float per thread; result valid in thread 0
+__device__ __forceinline__ float block_sum(float x, float* sh) {
+    x = warp_sum(x);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    __syncthreads();
+    if (lane == 0) sh[wid] = x;
+    __syncthreads();
+    float r = 0.f;
+    if (wid == 0) {
+        r = (lane < (int)(blockDim.x >> 5)) ? sh[lane] : 0.f;
+        r = warp_sum(r);
+    }
+    return r;
+}
+
+// F5a: mu = mean_i interp(chi', c_i); a = chi'[0,0,0] - mu; s = 0.5/|a| (Eq.4; R5, R11).
+// Partial sums go to a double accumulator; the last block of an item finalises stats = {mu, a, s, 0}.
+__global__ void k_sample_mean(const float* __restrict__ pts, int P, int N, const float* __restrict__ chi_p,
+                              double* __restrict__ acc, unsigned* __restrict__ ticket,
+                              float* __restrict__ stats) {
+    __shared__ float sh[32];
+    const int b = blockIdx.y;
+    const size_t V = (size_t)N * N * N;
+    const float* g = chi_p + (size_t)b * V;
+    float sum = 0.f;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < P; i += gridDim.x * blockDim.x) {
+        const Corner k = corner_of(pts + ((size_t)b * P + i) * 3, N);
+        float s = 0.f;
+#pragma unroll
+        for (int d = 0; d < 8; ++d) {
+            const int dx = d >> 2, dy = (d >> 1) & 1, dz = d & 1;
+            const float w = (dx ? k.f[0] : 1.f - k.f[0]) * (dy ? k.f[1] : 1.f - k.f[1]) * (dz ? k.f[2] : 1.f - k.f[2]);
+            s += w * __ldg(g + vox(N, k.j0[0] + dx, k.j0[1] + dy, k.j0[2] + dz));
+        }
+        sum += s;
+    }
+    const float bs = block_sum(sum, sh);
+    if (threadIdx.x == 0) {
+        atomicAdd(acc + b, (double)bs);
+        __threadfence();
+        const unsigned t = atomicAdd(ticket + b, 1u);
+        if (t == gridDim.x - 1) {
+            const double tot = atomicAdd(acc + b, 0.0);
+            const double mu = tot / (double)P;
+            const double a = (double)g[0] - mu;
+            const double s = 0.5 / fabs(a);  // m = 0.5
+            stats[b * 4 + 0] = (float)mu;
+            stats[b * 4 + 1] = (float)a;
+            stats[b * 4 + 2] = (float)s;
+            stats[b * 4 + 3] = 0.f;
+            acc[b] = 0.0;
+            ticket[b] = 0u;
+        }
+    }
+}
+
+// F5b: chi = s (chi' - mu), in place
+__global__ void k_scale_shift(float4* __restrict__ chi, size_t n4_per_item, const float* __restrict__ stats) {
+    const int b = blockIdx.y;
+    const float mu = stats[b * 4 + 0], s = stats[b * 4 + 2];
+    float4* p = chi + (size_t)b * n4_per_item;
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4_per_item; i += stride) {
+        float4 v = p[i];
+        v.x = s * (v.x - mu); v.y = s * (v.y - mu); v.z = s * (v.z - mu); v.w = s * (v.w - mu);
+        p[i] = v;
+    }
+}
+
+// B1: S0 = sum G, S1 = sum G chi; the last block writes bw = {s, beta/P, S1/a, beta/(P s)},
+// beta = S1/a - s S0.
+__global__ void k_reduce_g(const float4* __restrict__ G, const float4* __restrict__ chi, size_t n4_per_item,
+                           int P, const float* __restrict__ stats, double* __restrict__ acc,
+                           unsigned* __restrict__ ticket, float* __restrict__ bw) {
+    __shared__ float sh[32];
+    const int b = blockIdx.y;
+    const float4* g = G + (size_t)b * n4_per_item;
+    const float4* c = chi + (size_t)b * n4_per_item;
+    float s0 = 0.f, s1 = 0.f;
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4_per_item; i += stride) {
+        const float4 a = g[i], x = c[i];
+        s0 += (a.x + a.y) + (a.z + a.w);
+        s1 += (a.x * x.x + a.y * x.y) + (a.z * x.z + a.w * x.w);
+    }
+    const float b0 = block_sum(s0, sh);
+    const float b1 = block_sum(s1, sh);
+    if (threadIdx.x == 0) {
+        atomicAdd(acc + 2 * b, (double)b0);
+        atomicAdd(acc + 2 * b + 1, (double)b1);
+        __threadfence();
+        const unsigned t = atomicAdd(ticket + b, 1u);
+        if (t == gridDim.x - 1) {
+            const double S0 = atomicAdd(acc + 2 * b, 0.0), S1 = atomicAdd(acc + 2 * b + 1, 0.0);
+            const double a = stats[b * 4 + 1], s = stats[b * 4 + 2];
+            const double beta = S1 / a - s * S0;
+            bw[b * 4 + 0] = (float)s;
+            bw[b * 4 + 1] = (float)(beta / (double)P);
+            bw[b * 4 + 2] = (float)(S1 / a);
+            bw[b * 4 + 3] = (float)(beta / ((double)P * s));
+            acc[2 * b] = 0.0;
+            acc[2 * b + 1] = 0.0;
+            ticket[b] = 0u;
+        }
+    }
+}
+
+// B6: dL/dn_i = sum_corners w vbar[corner];
+//     dL/dc_i[a] = sum_corners (dw/dc_a) (n_i . vbar[corner] + (beta/(P s)) chi[corner]),
+//     dw/dc_a = N (d_a ? +1 : -1) prod_{b != a} w_b   (adjoint of F1 and F5; the mu part of chi' = chi/s + mu
+//     cancels because sum_corners dw/dc_a = 0).
+__global__ void k_gather_grads(const float* __restrict__ pts, const float* __restrict__ nrm, int P, int N,
+                               const float* __restrict__ vbar, const float* __restrict__ chi,
+                               const float* __restrict__ bw, float* __restrict__ gp, float* __restrict__ gn) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int b = blockIdx.y;
+    if (i >= P) return;
+    const size_t V = (size_t)N * N * N;
+    const size_t o = ((size_t)b * P + i) * 3;
+    const Corner k = corner_of(pts + o, N);
+    const float n0 = nrm[o], n1 = nrm[o + 1], n2 = nrm[o + 2];
+    const float cchi = bw[b * 4 + 3];
+    const float* vb = vbar + (size_t)b * 3 * V;
+    const float* cb = chi + (size_t)b * V;
+    float g0 = 0.f, g1 = 0.f, g2 = 0.f, c0 = 0.f, c1 = 0.f, c2 = 0.f;
+#pragma unroll
+    for (int d = 0; d < 8; ++d) {
+        const int dx = d >> 2, dy = (d >> 1) & 1, dz = d & 1;
+        const float wx = dx ? k.f[0] : 1.f - k.f[0];
+        const float wy = dy ? k.f[1] : 1.f - k.f[1];
+        const float wz = dz ? k.f[2] : 1.f - k.f[2];
+        const size_t j = vox(N, k.j0[0] + dx, k.j0[1] + dy, k.j0[2] + dz);
+        const float a0 = __ldg(vb + j), a1 = __ldg(vb + V + j), a2 = __ldg(vb + 2 * V + j);
+        const float x = __ldg(cb + j);
+        const float w = wx * wy * wz;
+        g0 += w * a0; g1 += w * a1; g2 += w * a2;
+        const float val = n0 * a0 + n1 * a1 + n2 * a2 + cchi * x;
+        c0 += (dx ? val : -val) * (wy * wz);
+        c1 += (dy ? val : -val) * (wx * wz);
+        c2 += (dz ? val : -val) * (wx * wy);
+    }
+    const float fN = (float)N;
+    gn[o] = g0; gn[o + 1] = g1; gn[o + 2] = g2;
+    gp[o] = fN * c0; gp[o + 1] = fN * c1; gp[o + 2] = fN * c2;
+}
+
+}  // namespace sap
+
+// ================================================================================================
+// handle, launch plumbing
+// ================================================================================================
+struct sap_dpsr {
+    int N = 0, batch = 0, max_points = 0, device = 0;
+    float sigma = 0.f;
+    // workspace (device)
+    float* v = nullptr;        // [B][3][N^3]  splatted field / vbar
+    float* W = nullptr;        // [B][N^3]     point density
+    float2* S3 = nullptr;      // [B*3][N*N*H] 3-channel spectra
+    float2* Q3 = nullptr;      // [B*3][N*N]
+    float2* S1 = nullptr;      // [B][N*N*H]   1-channel spectrum
+    float2* Q1 = nullptr;      // [B][N*N]
+    float2* tw = nullptr;      // [N]
+    double* acc = nullptr;     // [B][3] reduction accumulators (mean | S0,S1)
+    unsigned* ticket = nullptr;  // [B][2]
+    float* stats = nullptr;    // [B][4] {mu, a, s, -}
+    float* bw = nullptr;       // [B][4] {s, beta/P, S1/a, beta/(P s)}
+    // staging for the *_host entry points (allocated on first use)
+    float *h_pts = nullptr, *h_nrm = nullptr, *h_chi = nullptr, *h_gchi = nullptr, *h_gp = nullptr, *h_gn = nullptr;
+    int host_P = 0;
+    size_t ws_bytes = 0;
+    int launches = 0;
+    std::string err;
+};
+
+namespace sap {
+
+static thread_local std::string g_create_err;
+
+static bool cuda_ok(sap_dpsr* h, cudaError_t e, const char* what) {
+    if (e == cudaSuccess) return true;
+    char buf[512];
+    snprintf(buf, sizeof buf, "%s: %s", what, cudaGetErrorString(e));
+    if (h) h->err = buf; else g_create_err = buf;
+    return false;
+}
+
+template <class T> static cudaError_t dev_alloc(sap_dpsr* h, T** p, size_t count) {
+    cudaError_t e = cudaMalloc((void**)p, count * sizeof(T));
+    if (e == cudaSuccess) h->ws_bytes += count * sizeof(T);
+    return e;
+}
+
+#define SAP_LAUNCH_CHECK(h, name)                                          \
+    do {                                                                   \
+        ++(h)->launches;                                                   \
+        if (!cuda_ok((h), cudaGetLastError(), name)) return SAP_ERR_CUDA;  \
+    } while (0)
+
+template <class K> static cudaError_t set_smem(K kernel, size_t bytes) {
+    return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
+
+// threads per block of the FFT kernels
+template <int N> struct Cfg {
+    static constexpr bool FUSED_ZY = (N <= 128);  // a whole (y,z) plane fits one CTA's shared memory
+    static constexpr int NL = FUSED_ZY ? N : 16;
+    static constexpr int NT_ZY = 256;
+    static constexpr int NT_ST = 256;
+};
+
+template <int N> struct Runner {
+    static constexpr int H = N / 2;
+    using C = Cfg<N>;
+
+    static sap_status_t prepare(sap_dpsr* h) {
+        cudaError_t e = cudaSuccess;
+        auto upd = [&](cudaError_t x) { if (e == cudaSuccess) e = x; };
+        upd(set_smem(k_zy_fwd<N, C::NL, C::FUSED_ZY, false, C::NT_ZY>, zy_smem_bytes<N, C::NL, C::FUSED_ZY, false>()));
+        upd(set_smem(k_zy_fwd<N, C::NL, C::FUSED_ZY, true, C::NT_ZY>, zy_smem_bytes<N, C::NL, C::FUSED_ZY, true>()));
+        upd(set_smem(k_zy_inv<N, C::NL, C::FUSED_ZY, C::NT_ZY>, zy_smem_bytes<N, C::NL, C::FUSED_ZY, false>()));
+        upd(set_smem(k_strided<N, MODE_SOLVE, C::NT_ST>, strided_smem_bytes<N, MODE_SOLVE>()));
+        upd(set_smem(k_strided<N, MODE_ADJ, C::NT_ST>, strided_smem_bytes<N, MODE_ADJ>()));
+        upd(set_smem(k_strided<N, MODE_FWD, C::NT_ST>, strided_smem_bytes<N, MODE_FWD>()));
+        upd(set_smem(k_strided<N, MODE_INV, C::NT_ST>, strided_smem_bytes<N, MODE_INV>()));
+        return cuda_ok(h, e, "cudaFuncSetAttribute") ? SAP_OK : SAP_ERR_CUDA;
+    }
+
+    static StridedParams sp(sap_dpsr* h, const float2* inS, const float2* inQ, float2* outS, float2* outQ, int axis) {
+        StridedParams p;
+        p.inS = inS; p.inQ = inQ; p.outS = outS; p.outQ = outQ; p.tw = h->tw; p.axis = axis;
+        p.cg = 2.f * h->sigma * h->sigma / ((float)N * (float)N);
+        p.cs = (float)((2.0 / ((double)N * N * N)) / (-2.0 * 3.14159265358979323846));
+        return p;
+    }
+
+    static sap_status_t forward(sap_dpsr* h, const float* pts, const float* nrm, int P, float* chi, cudaStream_t st) {
+        const int B = h->batch;
+        const size_t V = (size_t)N * N * N;
+        // F1 splat (v and W are contiguous: one zero fill)
+        {
+            const size_t n4 = (size_t)B * 4 * V / 4;
+            k_zero<<<148 * 8, 256, 0, st>>>(reinterpret_cast<float4*>(h->v), n4);
+            SAP_LAUNCH_CHECK(h, "k_zero");
+            k_splat<<<dim3((P + 127) / 128, B), 128, 0, st>>>(pts, nrm, P, N, h->v, h->W);
+            SAP_LAUNCH_CHECK(h, "k_splat");
+        }
+        // F2 z (+y) forward, 3 channels
+        {
+            ZyFwdParams p{h->v, nullptr, nullptr, h->S3, h->Q3, h->tw, 3};
+            k_zy_fwd<N, C::NL, C::FUSED_ZY, false, C::NT_ZY>
+                <<<dim3(N * N / C::NL, B * 3), C::NT_ZY, zy_smem_bytes<N, C::NL, C::FUSED_ZY, false>(), st>>>(p);
+            SAP_LAUNCH_CHECK(h, "k_zy_fwd");
+        }
+        if (!C::FUSED_ZY) {
+            k_strided<N, MODE_FWD, C::NT_ST><<<dim3(strided_tiles<N>(), B * 3), C::NT_ST, strided_smem_bytes<N, MODE_FWD>(), st>>>(
+                sp(h, h->S3, h->Q3, h->S3, h->Q3, 1));
+            SAP_LAUNCH_CHECK(h, "k_strided<FWD,y>");
+        }
+        // F2x + F3 + F4x: x forward, spectral solve, x inverse (3 -> 1)
+        k_strided<N, MODE_SOLVE, C::NT_ST><<<dim3(strided_tiles<N>(), B), C::NT_ST, strided_smem_bytes<N, MODE_SOLVE>(), st>>>(
+            sp(h, h->S3, h->Q3, h->S1, h->Q1, 0));
+        SAP_LAUNCH_CHECK(h, "k_strided<SOLVE>");
+        if (!C::FUSED_ZY) {
+            k_strided<N, MODE_INV, C::NT_ST><<<dim3(strided_tiles<N>(), B), C::NT_ST, strided_smem_bytes<N, MODE_INV>(), st>>>(
+                sp(h, h->S1, h->Q1, h->S1, h->Q1, 1));
+            SAP_LAUNCH_CHECK(h, "k_strided<INV,y>");
+        }
+        // F4 (y +) z inverse -> chi'
+        {
+            ZyInvParams p{h->S1, h->Q1, chi, h->tw};
+            k_zy_inv<N, C::NL, C::FUSED_ZY, C::NT_ZY>
+                <<<dim3(N * N / C::NL, B), C::NT_ZY, zy_smem_bytes<N, C::NL, C::FUSED_ZY, false>(), st>>>(p);
+            SAP_LAUNCH_CHECK(h, "k_zy_inv");
+        }
+        // F5 normalise
+        {
+            int nb = (P + 255) / 256; if (nb > 296) nb = 296;
+            k_sample_mean<<<dim3(nb, B), 256, 0, st>>>(pts, P, N, chi, h->acc, h->ticket, h->stats);
+            SAP_LAUNCH_CHECK(h, "k_sample_mean");
+            const size_t n4 = V / 4;
+            int gb = (int)((n4 + 255) / 256); const int cap = (148 * 8 + B - 1) / B; if (gb > cap) gb = cap; if (gb < 1) gb = 1;
+            k_scale_shift<<<dim3(gb, B), 256, 0, st>>>(reinterpret_cast<float4*>(chi), n4, h->stats);
+            SAP_LAUNCH_CHECK(h, "k_scale_shift");
+        }
+        return SAP_OK;
+    }
+
+    static sap_status_t backward(sap_dpsr* h, const float* pts, const float* nrm, int P, const float* chi,
+                                 const float* gchi, float* gp, float* gn, cudaStream_t st) {
+        const int B = h->batch;
+        const size_t V = (size_t)N * N * N;
+        // B1 reductions
+        {
+            const size_t n4 = V / 4;
+            int gb = (int)((n4 + 255) / 256); const int cap = (148 * 4 + B - 1) / B; if (gb > cap) gb = cap; if (gb < 1) gb = 1;
+            k_reduce_g<<<dim3(gb, B), 256, 0, st>>>(reinterpret_cast<const float4*>(gchi), reinterpret_cast<const float4*>(chi),
+                                                   n4, P, h->stats, h->acc + B, h->ticket + B, h->bw);
+            SAP_LAUNCH_CHECK(h, "k_reduce_g");
+        }
+        // B2 + B3: Gbar' assembled on load, z (+y) forward
+        {
+            ZyFwdParams p{gchi, h->W, h->bw, h->S1, h->Q1, h->tw, 1};
+            k_zy_fwd<N, C::NL, C::FUSED_ZY, true, C::NT_ZY>
+                <<<dim3(N * N / C::NL, B), C::NT_ZY, zy_smem_bytes<N, C::NL, C::FUSED_ZY, true>(), st>>>(p);
+            SAP_LAUNCH_CHECK(h, "k_zy_fwd<GBAR>");
+        }
+        if (!C::FUSED_ZY) {
+            k_strided<N, MODE_FWD, C::NT_ST><<<dim3(strided_tiles<N>(), B), C::NT_ST, strided_smem_bytes<N, MODE_FWD>(), st>>>(
+                sp(h, h->S1, h->Q1, h->S1, h->Q1, 1));
+            SAP_LAUNCH_CHECK(h, "k_strided<FWD,y>");
+        }
+        // B3x + B4 + B5x: x forward, transposed multiplier, 3 x inverse
+        k_strided<N, MODE_ADJ, C::NT_ST><<<dim3(strided_tiles<N>(), B), C::NT_ST, strided_smem_bytes<N, MODE_ADJ>(), st>>>(
+            sp(h, h->S1, h->Q1, h->S3, h->Q3, 0));
+        SAP_LAUNCH_CHECK(h, "k_strided<ADJ>");
+        if (!C::FUSED_ZY) {
+            k_strided<N, MODE_INV, C::NT_ST><<<dim3(strided_tiles<N>(), B * 3), C::NT_ST, strided_smem_bytes<N, MODE_INV>(), st>>>(
+                sp(h, h->S3, h->Q3, h->S3, h->Q3, 1));
+            SAP_LAUNCH_CHECK(h, "k_strided<INV,y>");
+        }
+        // B5 (y +) z inverse -> vbar (into the v workspace)
+        {
+            ZyInvParams p{h->S3, h->Q3, h->v, h->tw};
+            k_zy_inv<N, C::NL, C::FUSED_ZY, C::NT_ZY>
+                <<<dim3(N * N / C::NL, B * 3), C::NT_ZY, zy_smem_bytes<N, C::NL, C::FUSED_ZY, false>(), st>>>(p);
+            SAP_LAUNCH_CHECK(h, "k_zy_inv");
+        }
+        // B6 gather
+        k_gather_grads<<<dim3((P + 127) / 128, B), 128, 0, st>>>(pts, nrm, P, N, h->v, chi, h->bw, gp, gn);
+        SAP_LAUNCH_CHECK(h, "k_gather_grads");
+        return SAP_OK;
+    }
+};
+
+template <class F> static sap_status_t dispatch(int N, F&& f) {
+    switch (N) {
+        case 32: return f(Runner<32>{});
+        case 64: return f(Runner<64>{});
+        case 128: return f(Runner<128>{});
+        case 256: return f(Runner<256>{});
+        case 512: return f(Runner<512>{});
+        default: return SAP_ERR_UNSUPPORTED;
+    }
+}
+
+}  // namespace sap
+
+// ================================================================================================
+// C ABI (include/sap_dpsr.h)
+// ================================================================================================
+using namespace sap;
+
+static bool supported_N(int N) { return N == 32 || N == 64 || N == 128 || N == 256 || N == 512; }
+
+static void free_all(sap_dpsr* h) {
+    cudaFree(h->v); cudaFree(h->S3); cudaFree(h->Q3); cudaFree(h->S1); cudaFree(h->Q1); cudaFree(h->tw);
+    cudaFree(h->acc); cudaFree(h->ticket); cudaFree(h->stats); cudaFree(h->bw);
+    cudaFree(h->h_pts); cudaFree(h->h_nrm); cudaFree(h->h_chi); cudaFree(h->h_gchi); cudaFree(h->h_gp); cudaFree(h->h_gn);
+}
+
+extern "C" sap_status_t sap_dpsr_create(int N, float sigma, int batch, int max_points, sap_dpsr_t** out) {
+    g_create_err.clear();
+    if (!out) { g_create_err = "out is NULL"; return SAP_ERR_INVALID_ARG; }
+    if (N <= 0 || batch <= 0 || max_points <= 0) { g_create_err = "N, batch and max_points must be positive"; return SAP_ERR_INVALID_ARG; }
+    if (!(sigma >= 0.f) || !isfinite(sigma)) { g_create_err = "sigma must be finite and >= 0"; return SAP_ERR_INVALID_ARG; }
+    if (!supported_N(N)) { g_create_err = "N must be one of 32, 64, 128, 256, 512"; return SAP_ERR_UNSUPPORTED; }
+    if ((long long)batch * 3 > 65535) { g_create_err = "batch too large (batch*3 must fit gridDim.y)"; return SAP_ERR_UNSUPPORTED; }
+    int dev = 0;
+    if (!cuda_ok(nullptr, cudaGetDevice(&dev), "cudaGetDevice")) return SAP_ERR_CUDA;
+    cudaDeviceProp prop;
+    if (!cuda_ok(nullptr, cudaGetDeviceProperties(&prop, dev), "cudaGetDeviceProperties")) return SAP_ERR_CUDA;
+    if (prop.major != 10) { g_create_err = "device is not sm_100 (Blackwell B200); this library has no other code path"; return SAP_ERR_UNSUPPORTED; }
+
+    sap_dpsr* h = new (std::nothrow) sap_dpsr;
+    if (!h) { g_create_err = "host allocation failed"; return SAP_ERR_OOM; }
+    h->N = N; h->sigma = sigma; h->batch = batch; h->max_points = max_points; h->device = dev;
+    const size_t V = (size_t)N * N * N, SP = (size_t)N * N * (N / 2), QP = (size_t)N * N, B = (size_t)batch;
+    cudaError_t e = cudaSuccess;
+    auto upd = [&](cudaError_t x) { if (e == cudaSuccess) e = x; };
+    upd(dev_alloc(h, &h->v, B * 4 * V));
+    upd(dev_alloc(h, &h->S3, B * 3 * SP));
+    upd(dev_alloc(h, &h->Q3, B * 3 * QP));
+    upd(dev_alloc(h, &h->S1, B * SP));
+    upd(dev_alloc(h, &h->Q1, B * QP));
+    upd(dev_alloc(h, &h->tw, (size_t)N));
+    upd(dev_alloc(h, &h->acc, B * 3));
+    upd(dev_alloc(h, &h->ticket, B * 2));
+    upd(dev_alloc(h, &h->stats, B * 4));
+    upd(dev_alloc(h, &h->bw, B * 4));
+    if (e != cudaSuccess) {
+        cuda_ok(nullptr, e, "cudaMalloc(workspace)");
+        const bool oom = (e == cudaErrorMemoryAllocation);
+        free_all(h); delete h; cudaGetLastError();
+        return oom ? SAP_ERR_OOM : SAP_ERR_CUDA;
+    }
+    h->W = h->v + B * 3 * V;
+    // twiddle table exp(-2 pi i t / N) computed in double
+    float2* tw = new (std::nothrow) float2[N];
+    if (!tw) { free_all(h); delete h; g_create_err = "host allocation failed"; return SAP_ERR_OOM; }
+    for (int t = 0; t < N; ++t) {
+        const double a = -2.0 * 3.14159265358979323846 * (double)t / (double)N;
+        tw[t] = make_float2((float)cos(a), (float)sin(a));
+    }
+    upd(cudaMemcpy(h->tw, tw, sizeof(float2) * N, cudaMemcpyHostToDevice));
+    delete[] tw;
+    upd(cudaMemset(h->acc, 0, sizeof(double) * B * 3));
+    upd(cudaMemset(h->ticket, 0, sizeof(unsigned) * B * 2));
+    upd(cudaMemset(h->stats, 0, sizeof(float) * B * 4));
+    upd(cudaMemset(h->bw, 0, sizeof(float) * B * 4));
+    sap_status_t st = SAP_OK;
+    if (e != cudaSuccess) { cuda_ok(nullptr, e, "workspace init"); st = SAP_ERR_CUDA; }
+    if (st == SAP_OK) {
+        st = dispatch(N, [&](auto r) { return decltype(r)::prepare(h); });
+        if (st != SAP_OK) g_create_err = h->err;
+    }
+    if (st != SAP_OK) { free_all(h); delete h; return st; }
+    *out = h;
+    return SAP_OK;
+}
+
+static sap_status_t check_common(sap_dpsr* h, int num_points) {
+    if (!h) return SAP_ERR_INVALID_ARG;
+    h->err.clear();
+    h->launches = 0;
+    if (num_points < 1 || num_points > h->max_points) { h->err = "num_points out of range [1, max_points]"; return SAP_ERR_INVALID_ARG; }
+    return SAP_OK;
+}
+
+extern "C" sap_status_t sap_dpsr_forward(sap_dpsr_t* h, const float* points, const float* normals, int num_points,
+                                         float* chi, void* stream) {
+    sap_status_t st = check_common(h, num_points);
+    if (st != SAP_OK) return st;
+    if (!points || !normals || !chi) { h->err = "null pointer argument"; return SAP_ERR_INVALID_ARG; }
+    return dispatch(h->N, [&](auto r) { return decltype(r)::forward(h, points, normals, num_points, chi, (cudaStream_t)stream); });
+}
+
+extern "C" sap_status_t sap_dpsr_backward(sap_dpsr_t* h, const float* points, const float* normals, int num_points,
+                                          const float* chi, const float* grad_chi, float* grad_points,
+                                          float* grad_normals, void* stream) {
+    sap_status_t st = check_common(h, num_points);
+    if (st != SAP_OK) return st;
+    if (!points || !normals || !chi || !grad_chi || !grad_points || !grad_normals) { h->err = "null pointer argument"; return SAP_ERR_INVALID_ARG; }
+    return dispatch(h->N, [&](auto r) {
+        return decltype(r)::backward(h, points, normals, num_points, chi, grad_chi, grad_points, grad_normals, (cudaStream_t)stream);
+    });
+}
+
+static sap_status_t ensure_staging(sap_dpsr* h) {
+    if (h->h_pts) return SAP_OK;
+    const size_t V = (size_t)h->N * h->N * h->N, B = (size_t)h->batch, PP = B * (size_t)h->max_points * 3;
+    cudaError_t e = cudaSuccess;
+    auto upd = [&](cudaError_t x) { if (e == cudaSuccess) e = x; };
+    upd(dev_alloc(h, &h->h_pts, PP)); upd(dev_alloc(h, &h->h_nrm, PP));
+    upd(dev_alloc(h, &h->h_gp, PP)); upd(dev_alloc(h, &h->h_gn, PP));
+    upd(dev_alloc(h, &h->h_chi, B * V)); upd(dev_alloc(h, &h->h_gchi, B * V));
+    if (e != cudaSuccess) {
+        cuda_ok(h, e, "cudaMalloc(staging)");
+        cudaFree(h->h_pts); cudaFree(h->h_nrm); cudaFree(h->h_gp); cudaFree(h->h_gn); cudaFree(h->h_chi); cudaFree(h->h_gchi);
+        h->h_pts = h->h_nrm = h->h_gp = h->h_gn = h->h_chi = h->h_gchi = nullptr;
+        cudaGetLastError();
+        return e == cudaErrorMemoryAllocation ? SAP_ERR_OOM : SAP_ERR_CUDA;
+    }
+    return SAP_OK;
+}
+
+extern "C" sap_status_t sap_dpsr_forward_host(sap_dpsr_t* h, const float* points_host, const float* normals_host,
+                                              int num_points, float* chi_host, void* stream) {
+    sap_status_t st = check_common(h, num_points);
+    if (st != SAP_OK) return st;
+    if (!points_host || !normals_host) { h->err = "null pointer argument"; return SAP_ERR_INVALID_ARG; }
+    if ((st = ensure_staging(h)) != SAP_OK) return st;
+    cudaStream_t s = (cudaStream_t)stream;
+    const size_t pb = (size_t)h->batch * num_points * 3 * sizeof(float);
+    const size_t vb = (size_t)h->batch * h->N * h->N * h->N * sizeof(float);
+    if (!cuda_ok(h, cudaMemcpyAsync(h->h_pts, points_host, pb, cudaMemcpyHostToDevice, s), "H2D points")) return SAP_ERR_CUDA;
+    if (!cuda_ok(h, cudaMemcpyAsync(h->h_nrm, normals_host, pb, cudaMemcpyHostToDevice, s), "H2D normals")) return SAP_ERR_CUDA;
+    st = dispatch(h->N, [&](auto r) { return decltype(r)::forward(h, h->h_pts, h->h_nrm, num_points, h->h_chi, s); });
+    if (st != SAP_OK) return st;
+    h->host_P = num_points;
+    if (chi_host && !cuda_ok(h, cudaMemcpyAsync(chi_host, h->h_chi, vb, cudaMemcpyDeviceToHost, s), "D2H chi")) return SAP_ERR_CUDA;
+    if (!cuda_ok(h, cudaStreamSynchronize(s), "cudaStreamSynchronize")) return SAP_ERR_CUDA;
+    return SAP_OK;
+}
+
+extern "C" sap_status_t sap_dpsr_backward_host(sap_dpsr_t* h, const float* grad_chi_host, float* grad_points_host,
+                                               float* grad_normals_host, void* stream) {
+    if (!h) return SAP_ERR_INVALID_ARG;
+    h->err.clear();
+    const int keep = h->launches;
+    if (!h->h_pts || h->host_P < 1) { h->err = "sap_dpsr_backward_host must follow sap_dpsr_forward_host"; return SAP_ERR_INVALID_ARG; }
+    if (!grad_chi_host || !grad_points_host || !grad_normals_host) { h->err = "null pointer argument"; return SAP_ERR_INVALID_ARG; }
+    (void)keep;
+    h->launches = 0;
+    cudaStream_t s = (cudaStream_t)stream;
+    const int P = h->host_P;
+    const size_t pb = (size_t)h->batch * P * 3 * sizeof(float);
+    const size_t vb = (size_t)h->batch * h->N * h->N * h->N * sizeof(float);
+    if (!cuda_ok(h, cudaMemcpyAsync(h->h_gchi, grad_chi_host, vb, cudaMemcpyHostToDevice, s), "H2D grad_chi")) return SAP_ERR_CUDA;
+    sap_status_t st = dispatch(h->N, [&](auto r) {
+        return decltype(r)::backward(h, h->h_pts, h->h_nrm, P, h->h_chi, h->h_gchi, h->h_gp, h->h_gn, s);
+    });
+    if (st != SAP_OK) return st;
+    if (!cuda_ok(h, cudaMemcpyAsync(grad_points_host, h->h_gp, pb, cudaMemcpyDeviceToHost, s), "D2H grad_points")) return SAP_ERR_CUDA;
+    if (!cuda_ok(h, cudaMemcpyAsync(grad_normals_host, h->h_gn, pb, cudaMemcpyDeviceToHost, s), "D2H grad_normals")) return SAP_ERR_CUDA;
+    if (!cuda_ok(h, cudaStreamSynchronize(s), "cudaStreamSynchronize")) return SAP_ERR_CUDA;
+    return SAP_OK;
+}
+
+extern "C" sap_status_t sap_dpsr_get_stats(sap_dpsr_t* h, float* stats_host, void* stream) {
+    if (!h) return SAP_ERR_INVALID_ARG;
+    h->err.clear();
+    if (!stats_host) { h->err = "null pointer argument"; return SAP_ERR_INVALID_ARG; }
+    cudaStream_t s = (cudaStream_t)stream;
+    float* tmp = new (std::nothrow) float[(size_t)h->batch * 4];
+    if (!tmp) { h->err = "host allocation failed"; return SAP_ERR_OOM; }
+    bool ok = cuda_ok(h, cudaMemcpyAsync(tmp, h->stats, sizeof(float) * 4 * h->batch, cudaMemcpyDeviceToHost, s), "D2H stats") &&
+              cuda_ok(h, cudaStreamSynchronize(s), "cudaStreamSynchronize");
+    if (ok) for (int b = 0; b < h->batch; ++b) for (int k = 0; k < 3; ++k) stats_host[b * 3 + k] = tmp[b * 4 + k];
+    delete[] tmp;
+    return ok ? SAP_OK : SAP_ERR_CUDA;
+}
+
+extern "C" void sap_dpsr_destroy(sap_dpsr_t* h) {
+    if (!h) return;
+    free_all(h);
+    delete h;
+}
+
+extern "C" const char* sap_dpsr_last_error(const sap_dpsr_t* h) { return h ? h->err.c_str() : g_create_err.c_str(); }
+extern "C" size_t sap_dpsr_workspace_bytes(const sap_dpsr_t* h) { return h ? h->ws_bytes : 0; }
+extern "C" int sap_dpsr_last_launch_count(const sap_dpsr_t* h) { return h ? h->launches : 0; }
