@@ -1,0 +1,143 @@
+"""GPU parity: the CUDA path (through the C ABI, via the thin binding) against the float64 oracle,
+element by element, on the same seeded inputs.  Bars (BASELINE.json north_star):
+max|d chi| <= 1e-4 max|chi|; gradients <= 1e-3 relative L2."""
+import numpy as np
+import pytest
+
+from oracle import dpsr_oracle as orc
+from paper_2106_03452_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+CHI_TOL = 1e-4
+GRAD_TOL = 1e-3
+
+
+def _gpu_run(N, sigma, pts, nrm, G):
+    import torch
+    from paper_2106_03452_b200.binding import Dpsr
+    B, P = pts.shape[0], pts.shape[1]
+    h = Dpsr(N, sigma, B, P)
+    tp, tn = torch.from_numpy(pts).cuda(), torch.from_numpy(nrm).cuda()
+    chi = h.forward(tp, tn)
+    stats = h.stats()
+    out = dict(chi=chi.cpu().numpy(), stats=stats, fwd_launches=h.last_launch_count)
+    if G is not None:
+        gp, gn = h.backward(tp, tn, chi, torch.from_numpy(G).cuda())
+        out.update(gp=gp.cpu().numpy(), gn=gn.cpu().numpy(), bwd_launches=h.last_launch_count)
+    torch.cuda.synchronize()
+    h.close()
+    return out
+
+
+def _check_item(N, sigma, pts, nrm, G, got_chi, got_stats, got_gp, got_gn):
+    f = orc.forward(N, sigma, pts, nrm)
+    err = np.abs(got_chi - f["chi"]).max() / np.abs(f["chi"]).max()
+    assert err <= CHI_TOL, f"chi rel-max err {err:.3e}"
+    assert abs(got_stats[0] - f["mu"]) <= 1e-4 * abs(f["a"])
+    assert abs(got_stats[2] - f["s"]) <= 1e-4 * f["s"]
+    if G is not None:
+        b = orc.backward(N, sigma, pts, nrm, f, G)
+        ep = np.linalg.norm(got_gp - b["grad_points"]) / np.linalg.norm(b["grad_points"])
+        en = np.linalg.norm(got_gn - b["grad_normals"]) / np.linalg.norm(b["grad_normals"])
+        assert ep <= GRAD_TOL and en <= GRAD_TOL, f"grad rel-L2 err points {ep:.3e} normals {en:.3e}"
+    return err
+
+
+@pytest.mark.parametrize("cfg_id", [1, 2])
+def test_config_parity(cfg_id):
+    cfg, pts, nrm = inputs.make_config(cfg_id)
+    G = inputs.upstream_grad(cfg.N, 1)
+    r = _gpu_run(cfg.N, cfg.sigma, pts, nrm, G)
+    _check_item(cfg.N, cfg.sigma, pts[0], nrm[0], G[0], r["chi"][0], r["stats"][0], r["gp"][0], r["gn"][0])
+    assert r["fwd_launches"] > 0 and r["bwd_launches"] > 0
+
+
+@pytest.mark.parametrize("N,P,sigma,shape", [(64, 5000, 2.0, "torus"), (32, 777, 3.0, "ellipsoids3"),
+                                             (64, 1, 0.0, "sphere"), (128, 4099, 5.0, "bumpy")])
+def test_other_sizes_and_ragged_point_counts(N, P, sigma, shape):
+    pts, nrm = inputs.make_cloud(shape, P, seed=7)
+    G = inputs.upstream_grad(N, 1, seed=3)
+    r = _gpu_run(N, sigma, pts[None], nrm[None], G)
+    _check_item(N, sigma, pts, nrm, G[0], r["chi"][0], r["stats"][0], r["gp"][0], r["gn"][0])
+
+
+def test_batch_items_are_independent():
+    # config 3 shape, small batch: item b of a batched call == the oracle on item b alone
+    cfg, pts, nrm = inputs.make_config(3, batch=3, P=4000)
+    G = inputs.upstream_grad(cfg.N, 3, seed=1)
+    r = _gpu_run(cfg.N, cfg.sigma, pts, nrm, G)
+    for b in range(3):
+        _check_item(cfg.N, cfg.sigma, pts[b], nrm[b], G[b], r["chi"][b], r["stats"][b], r["gp"][b], r["gn"][b])
+
+
+def test_points_on_lattice_planes_and_wrap():
+    # degenerate positions: exactly on vertices, in the last cell (periodic wrap), coincident pairs
+    N, sigma = 32, 2.0
+    pts, nrm = inputs.make_cloud("sphere", 500, seed=11)
+    pts[:50] = np.round(pts[:50] * N) / N
+    pts[50:60, 0] = (N - 0.25) / N
+    pts[60:70, 2] = 0.0
+    pts[70:80] = pts[80:90]
+    nrm[70:80] = -nrm[80:90]
+    r = _gpu_run(N, sigma, pts[None], nrm[None], None)
+    _check_item(N, sigma, pts, nrm, None, r["chi"][0], r["stats"][0], None, None)
+
+
+@pytest.mark.slow
+def test_config4_256_parity_one_iteration():
+    cfg, pts, nrm = inputs.make_config(4)
+    G = inputs.upstream_grad(cfg.N, 1)
+    r = _gpu_run(cfg.N, cfg.sigma, pts, nrm, G)
+    _check_item(cfg.N, cfg.sigma, pts[0], nrm[0], G[0], r["chi"][0], r["stats"][0], r["gp"][0], r["gn"][0])
+
+
+def test_repeatable_and_handle_reuse():
+    import torch
+    from paper_2106_03452_b200.binding import Dpsr
+    cfg, pts, nrm = inputs.make_config(1)
+    h = Dpsr(cfg.N, cfg.sigma, 1, cfg.P)
+    tp, tn = torch.from_numpy(pts).cuda(), torch.from_numpy(nrm).cuda()
+    a = h.forward(tp, tn).clone()
+    b = h.forward(tp, tn)
+    # only the atomics' summation order may differ between two runs
+    assert (a - b).abs().max().item() <= 1e-5 * a.abs().max().item()
+    # fewer points than max_points on the same handle
+    c = h.forward(tp[:, :1000].contiguous(), tn[:, :1000].contiguous())
+    f = orc.forward(cfg.N, cfg.sigma, pts[0, :1000], nrm[0, :1000])
+    assert np.abs(c.cpu().numpy()[0] - f["chi"]).max() <= CHI_TOL * np.abs(f["chi"]).max()
+    h.close()
+
+
+def test_host_buffer_entry_points_match_device_ones():
+    import torch
+    from paper_2106_03452_b200.binding import Dpsr
+    cfg, pts, nrm = inputs.make_config(1)
+    G = inputs.upstream_grad(cfg.N, 1)
+    r = _gpu_run(cfg.N, cfg.sigma, pts, nrm, G)
+    h = Dpsr(cfg.N, cfg.sigma, 1, cfg.P)
+    chi = torch.empty((1, cfg.N, cfg.N, cfg.N)).pin_memory()
+    gp, gn = torch.empty((1, cfg.P, 3)).pin_memory(), torch.empty((1, cfg.P, 3)).pin_memory()
+    h.forward_host(torch.from_numpy(pts), torch.from_numpy(nrm), chi)
+    h.backward_host(torch.from_numpy(G), gp, gn)
+    assert np.abs(chi.numpy() - r["chi"]).max() <= 1e-5 * np.abs(r["chi"]).max()
+    assert np.linalg.norm(gp.numpy() - r["gp"]) <= 1e-4 * np.linalg.norm(r["gp"])
+    assert np.linalg.norm(gn.numpy() - r["gn"]) <= 1e-4 * np.linalg.norm(r["gn"])
+    h.close()
+
+
+def test_autograd_function():
+    import torch
+    from paper_2106_03452_b200.binding import Dpsr, dpsr
+    cfg, pts, nrm = inputs.make_config(1)
+    G = inputs.upstream_grad(cfg.N, 1)
+    h = Dpsr(cfg.N, cfg.sigma, 1, cfg.P)
+    tp = torch.from_numpy(pts).cuda().requires_grad_(True)
+    tn = torch.from_numpy(nrm).cuda().requires_grad_(True)
+    chi = dpsr(h)(tp, tn)
+    (chi * torch.from_numpy(G).cuda()).sum().backward()
+    f = orc.forward(cfg.N, cfg.sigma, pts[0], nrm[0])
+    b = orc.backward(cfg.N, cfg.sigma, pts[0], nrm[0], f, G[0])
+    assert np.linalg.norm(tp.grad.cpu().numpy()[0] - b["grad_points"]) <= GRAD_TOL * np.linalg.norm(b["grad_points"])
+    assert np.linalg.norm(tn.grad.cpu().numpy()[0] - b["grad_normals"]) <= GRAD_TOL * np.linalg.norm(b["grad_normals"])
+    h.close()
