@@ -111,6 +111,17 @@ size_t sap_dpsr_workspace_bytes(const sap_dpsr_t* h);
 /* Number of kernel launches the last forward / backward call enqueued (for bench.py's gpu_launches). */
 int sap_dpsr_last_launch_count(const sap_dpsr_t* h);
 
+/*
+ * Per-kernel timing for the bench (off by default).  When on, forward/backward record a CUDA event on
+ * the caller's stream before their first launch and after every launch.  sap_dpsr_get_profile waits
+ * for the last event of the most recent forward or backward call and writes, for each of its
+ * launches in order, the device time in milliseconds between the surrounding events (ms[i]) and a
+ * static kernel label (names[i]; either array may be NULL).  Returns the number of entries written
+ * (at most cap), 0 if profiling is off or nothing was recorded.
+ */
+sap_status_t sap_dpsr_set_profiling(sap_dpsr_t* h, int on);
+int sap_dpsr_get_profile(sap_dpsr_t* h, float* ms, const char** names, int cap);
+
 #ifdef __cplusplus
 }
 #endif

@@ -15,7 +15,7 @@ STATUS_NAMES = {0: "SAP_OK", 1: "SAP_ERR_INVALID_ARG", 2: "SAP_ERR_UNSUPPORTED",
 EXPORTS = [
     "sap_dpsr_create", "sap_dpsr_forward", "sap_dpsr_backward", "sap_dpsr_forward_host",
     "sap_dpsr_backward_host", "sap_dpsr_get_stats", "sap_dpsr_destroy", "sap_dpsr_last_error",
-    "sap_dpsr_workspace_bytes", "sap_dpsr_last_launch_count",
+    "sap_dpsr_workspace_bytes", "sap_dpsr_last_launch_count", "sap_dpsr_set_profiling", "sap_dpsr_get_profile",
 ]
 
 _lib = None
@@ -58,6 +58,10 @@ def lib():
     L.sap_dpsr_workspace_bytes.restype = ctypes.c_size_t
     L.sap_dpsr_last_launch_count.argtypes = [vp]
     L.sap_dpsr_last_launch_count.restype = ci
+    L.sap_dpsr_set_profiling.argtypes = [vp, ci]
+    L.sap_dpsr_set_profiling.restype = ci
+    L.sap_dpsr_get_profile.argtypes = [vp, ctypes.POINTER(cf), ctypes.POINTER(ctypes.c_char_p), ci]
+    L.sap_dpsr_get_profile.restype = ci
     _lib = L
     return L
 
@@ -150,6 +154,17 @@ class Dpsr:
         out = np.empty((self.batch, 3), np.float32)
         self._check(lib().sap_dpsr_get_stats(self._h, out.ctypes.data_as(ctypes.c_void_p), _stream_ptr(stream)))
         return out
+
+    def set_profiling(self, on=True):
+        self._check(lib().sap_dpsr_set_profiling(self._h, int(bool(on))))
+
+    def profile(self):
+        """[(kernel label, ms)] of the launches of the last forward or backward call (profiling on)."""
+        cap = 24
+        ms = (ctypes.c_float * cap)()
+        names = (ctypes.c_char_p * cap)()
+        n = lib().sap_dpsr_get_profile(self._h, ms, names, cap)
+        return [(names[i].decode(), float(ms[i])) for i in range(n)]
 
     @property
     def workspace_bytes(self):

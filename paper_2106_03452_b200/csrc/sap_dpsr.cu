@@ -273,6 +273,12 @@ struct sap_dpsr {
     int host_P = 0;
     size_t ws_bytes = 0;
     int launches = 0;
+    // optional per-kernel timing (sap_dpsr_set_profiling): one event before the first launch, one after each
+    bool prof = false;
+    static constexpr int MAX_EV = 24;
+    cudaEvent_t ev[MAX_EV] = {};
+    const char* ev_name[MAX_EV] = {};
+    int nev = 0;
     std::string err;
 };
 
@@ -298,7 +304,19 @@ template <class T> static cudaError_t dev_alloc(sap_dpsr* h, T** p, size_t count
     do {                                                                   \
         ++(h)->launches;                                                   \
         if (!cuda_ok((h), cudaGetLastError(), name)) return SAP_ERR_CUDA;  \
+        prof_mark((h), name, st);                                          \
     } while (0)
+
+static void prof_mark(sap_dpsr* h, const char* name, cudaStream_t st) {
+    if (!h->prof || h->nev >= sap_dpsr::MAX_EV) return;
+    h->ev_name[h->nev] = name;
+    cudaEventRecord(h->ev[h->nev], st);
+    ++h->nev;
+}
+static void prof_begin(sap_dpsr* h, cudaStream_t st) {
+    h->nev = 0;
+    prof_mark(h, "begin", st);
+}
 
 template <class K> static cudaError_t set_smem(K kernel, size_t bytes) {
     return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
@@ -340,6 +358,7 @@ template <int N> struct Runner {
     static sap_status_t forward(sap_dpsr* h, const float* pts, const float* nrm, int P, float* chi, cudaStream_t st) {
         const int B = h->batch;
         const size_t V = (size_t)N * N * N;
+        prof_begin(h, st);
         // F1 splat (v and W are contiguous: one zero fill)
         {
             const size_t n4 = (size_t)B * 4 * V / 4;
@@ -393,6 +412,7 @@ template <int N> struct Runner {
                                  const float* gchi, float* gp, float* gn, cudaStream_t st) {
         const int B = h->batch;
         const size_t V = (size_t)N * N * N;
+        prof_begin(h, st);
         // B1 reductions
         {
             const size_t n4 = V / 4;
@@ -457,6 +477,7 @@ using namespace sap;
 static bool supported_N(int N) { return N == 32 || N == 64 || N == 128 || N == 256 || N == 512; }
 
 static void free_all(sap_dpsr* h) {
+    for (int i = 0; i < sap_dpsr::MAX_EV; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
     cudaFree(h->v); cudaFree(h->S3); cudaFree(h->Q3); cudaFree(h->S1); cudaFree(h->Q1); cudaFree(h->tw);
     cudaFree(h->acc); cudaFree(h->ticket); cudaFree(h->stats); cudaFree(h->bw);
     cudaFree(h->h_pts); cudaFree(h->h_nrm); cudaFree(h->h_chi); cudaFree(h->h_gchi); cudaFree(h->h_gp); cudaFree(h->h_gn);
@@ -633,3 +654,28 @@ extern "C" void sap_dpsr_destroy(sap_dpsr_t* h) {
 extern "C" const char* sap_dpsr_last_error(const sap_dpsr_t* h) { return h ? h->err.c_str() : g_create_err.c_str(); }
 extern "C" size_t sap_dpsr_workspace_bytes(const sap_dpsr_t* h) { return h ? h->ws_bytes : 0; }
 extern "C" int sap_dpsr_last_launch_count(const sap_dpsr_t* h) { return h ? h->launches : 0; }
+
+extern "C" sap_status_t sap_dpsr_set_profiling(sap_dpsr_t* h, int on) {
+    if (!h) return SAP_ERR_INVALID_ARG;
+    h->err.clear();
+    if (on && !h->ev[0]) {
+        for (int i = 0; i < sap_dpsr::MAX_EV; ++i)
+            if (!cuda_ok(h, cudaEventCreate(&h->ev[i]), "cudaEventCreate")) return SAP_ERR_CUDA;
+    }
+    h->prof = on != 0;
+    h->nev = 0;
+    return SAP_OK;
+}
+
+extern "C" int sap_dpsr_get_profile(sap_dpsr_t* h, float* ms, const char** names, int cap) {
+    if (!h || h->nev < 2) return 0;
+    if (cudaEventSynchronize(h->ev[h->nev - 1]) != cudaSuccess) return 0;
+    int n = 0;
+    for (int i = 1; i < h->nev && n < cap; ++i, ++n) {
+        float t = 0.f;
+        cudaEventElapsedTime(&t, h->ev[i - 1], h->ev[i]);
+        if (ms) ms[n] = t;
+        if (names) names[n] = h->ev_name[i];
+    }
+    return n;
+}
