@@ -125,6 +125,55 @@ template <int R> SAP_HD void dft_inv(float2 (&v)[R]) {
     for (int i = 0; i < R; ++i) { float t = v[i].x; v[i].x = v[i].y; v[i].y = t; }
 }
 
+// ---- register-level stage butterflies --------------------------------------------------------------
+// Stage S of the length-N plan on R values held in registers.  j is the butterfly's index inside its
+// sub-transform (0 <= j < ST).  Forward (DIF): DFT_R then twiddle w_{R*ST}^{r j}; inverse (DIT): conjugate
+// twiddle then inverse DFT_R.  tw = exp(-2 pi i t / TWN).
+template <int N, int S, int TWN>
+SAP_HD void bfly_fwd(float2 (&v)[StageInfo<N, S>::R], int j, const float2* tw) {
+    constexpr int R = StageInfo<N, S>::R;
+    constexpr int ST = StageInfo<N, S>::ST;
+    constexpr int TWMUL = TWN / (R * ST);
+    dft_fwd<R>(v);
+    if (ST > 1) {
+#pragma unroll
+        for (int r = 1; r < R; ++r) v[r] = cmul(v[r], tw[r * j * TWMUL]);
+    }
+}
+template <int N, int S, int TWN>
+SAP_HD void bfly_inv(float2 (&v)[StageInfo<N, S>::R], int j, const float2* tw) {
+    constexpr int R = StageInfo<N, S>::R;
+    constexpr int ST = StageInfo<N, S>::ST;
+    constexpr int TWMUL = TWN / (R * ST);
+    if (ST > 1) {
+#pragma unroll
+        for (int r = 1; r < R; ++r) v[r] = cmulc(v[r], tw[r * j * TWMUL]);
+    }
+    dft_inv<R>(v);
+}
+
+// r2c / c2r pair formulas on single values (see r2c_split / c2r_split below for the derivation).
+// w = exp(-2 pi i k / N).  In: a = Z[k], b = Z[H-k].  Out: a = X[k], b = X[H-k].
+SAP_HD void r2c_pair(float2& a, float2& b, float2 w) {
+    float2 e = make_float2(0.5f * (a.x + b.x), 0.5f * (a.y - b.y));
+    float2 d = make_float2(0.5f * (a.x - b.x), 0.5f * (a.y + b.y));
+    float2 wd = cmul(d, w);
+    float2 f = make_float2(-wd.y, wd.x);
+    a = csub(e, f);
+    float2 g = cadd(e, f);
+    b = make_float2(g.x, -g.y);
+}
+// In: a = X[k], b = X[H-k].  Out: a = Z[k], b = Z[H-k].
+SAP_HD void c2r_pair(float2& a, float2& b, float2 w) {
+    float2 e = make_float2(0.5f * (a.x + b.x), 0.5f * (a.y - b.y));
+    float2 d = make_float2(0.5f * (a.x - b.x), 0.5f * (a.y + b.y));
+    float2 o = cmulc(d, w);
+    float2 io = make_float2(-o.y, o.x);
+    a = cadd(e, io);
+    float2 g = csub(e, io);
+    b = make_float2(g.x, -g.y);
+}
+
 // ---- one radix stage over a set of lines in shared memory --------------------------------------
 // Element n of line l lives at s[l * LS + n * ES].  tw is the table exp(-2 pi i t / TWN), t < TWN,
 // TWN a multiple of N.  LANES_LINES: consecutive threads take consecutive lines (same butterfly),

@@ -34,11 +34,11 @@ __global__ void __launch_bounds__(NT) k_zy_inv(ZyInvParams p) {
     DevCtx ctx{(int)threadIdx.x, NT};
     zy_inv_body<N, NL, DO_Y>(ctx, p, smem, (int)blockIdx.x, (int)blockIdx.y);
 }
-template <int N, int MODE, int NT>
+template <int N, int MODE, int NT, int W>
 __global__ void __launch_bounds__(NT) k_strided(StridedParams p) {
     extern __shared__ float2 smem[];
     DevCtx ctx{(int)threadIdx.x, NT};
-    strided_body<N, MODE>(ctx, p, smem, (int)blockIdx.x, (int)blockIdx.y);
+    strided_body<N, MODE, NT, W>(ctx, p, smem, (int)blockIdx.x, (int)blockIdx.y);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -325,9 +325,11 @@ template <class K> static cudaError_t set_smem(K kernel, size_t bytes) {
 // threads per block of the FFT kernels
 template <int N> struct Cfg {
     static constexpr bool FUSED_ZY = (N <= 128);  // a whole (y,z) plane fits one CTA's shared memory
-    static constexpr int NL = FUSED_ZY ? N : 16;
+    static constexpr int NL = FUSED_ZY ? N : 32;
     static constexpr int NT_ZY = 256;
-    static constexpr int NT_ST = 256;
+    // strided tiles: columns per tile (W) and threads, for the plain y pass (Y) and the fused x pass (X)
+    static constexpr int WY = 16, NTY = 256;
+    static constexpr int WX = (N >= 64) ? 32 : 16, NTX = (N >= 256) ? 512 : 256;
 };
 
 template <int N> struct Runner {
@@ -337,13 +339,13 @@ template <int N> struct Runner {
     static sap_status_t prepare(sap_dpsr* h) {
         cudaError_t e = cudaSuccess;
         auto upd = [&](cudaError_t x) { if (e == cudaSuccess) e = x; };
-        upd(set_smem(k_zy_fwd<N, C::NL, C::FUSED_ZY, false, C::NT_ZY>, zy_smem_bytes<N, C::NL, C::FUSED_ZY, false>()));
-        upd(set_smem(k_zy_fwd<N, C::NL, C::FUSED_ZY, true, C::NT_ZY>, zy_smem_bytes<N, C::NL, C::FUSED_ZY, true>()));
-        upd(set_smem(k_zy_inv<N, C::NL, C::FUSED_ZY, C::NT_ZY>, zy_smem_bytes<N, C::NL, C::FUSED_ZY, false>()));
-        upd(set_smem(k_strided<N, MODE_SOLVE, C::NT_ST>, strided_smem_bytes<N, MODE_SOLVE>()));
-        upd(set_smem(k_strided<N, MODE_ADJ, C::NT_ST>, strided_smem_bytes<N, MODE_ADJ>()));
-        upd(set_smem(k_strided<N, MODE_FWD, C::NT_ST>, strided_smem_bytes<N, MODE_FWD>()));
-        upd(set_smem(k_strided<N, MODE_INV, C::NT_ST>, strided_smem_bytes<N, MODE_INV>()));
+        upd(set_smem(k_zy_fwd<N, C::NL, C::FUSED_ZY, false, C::NT_ZY>, zy_smem_bytes<N, C::NL>()));
+        upd(set_smem(k_zy_fwd<N, C::NL, C::FUSED_ZY, true, C::NT_ZY>, zy_smem_bytes<N, C::NL>()));
+        upd(set_smem(k_zy_inv<N, C::NL, C::FUSED_ZY, C::NT_ZY>, zy_smem_bytes<N, C::NL>()));
+        upd(set_smem(k_strided<N, MODE_SOLVE, C::NTX, C::WX>, strided_smem_bytes<N, C::WX>()));
+        upd(set_smem(k_strided<N, MODE_ADJ, C::NTX, C::WX>, strided_smem_bytes<N, C::WX>()));
+        upd(set_smem(k_strided<N, MODE_FWD, C::NTY, C::WY>, strided_smem_bytes<N, C::WY>()));
+        upd(set_smem(k_strided<N, MODE_INV, C::NTY, C::WY>, strided_smem_bytes<N, C::WY>()));
         return cuda_ok(h, e, "cudaFuncSetAttribute") ? SAP_OK : SAP_ERR_CUDA;
     }
 
@@ -371,20 +373,20 @@ template <int N> struct Runner {
         {
             ZyFwdParams p{h->v, nullptr, nullptr, h->S3, h->Q3, h->tw, 3};
             k_zy_fwd<N, C::NL, C::FUSED_ZY, false, C::NT_ZY>
-                <<<dim3(N * N / C::NL, B * 3), C::NT_ZY, zy_smem_bytes<N, C::NL, C::FUSED_ZY, false>(), st>>>(p);
+                <<<dim3(N * N / C::NL, B * 3), C::NT_ZY, zy_smem_bytes<N, C::NL>(), st>>>(p);
             SAP_LAUNCH_CHECK(h, "k_zy_fwd");
         }
         if (!C::FUSED_ZY) {
-            k_strided<N, MODE_FWD, C::NT_ST><<<dim3(strided_tiles<N>(), B * 3), C::NT_ST, strided_smem_bytes<N, MODE_FWD>(), st>>>(
+            k_strided<N, MODE_FWD, C::NTY, C::WY><<<dim3(strided_tiles<N, C::WY>(), B * 3), C::NTY, strided_smem_bytes<N, C::WY>(), st>>>(
                 sp(h, h->S3, h->Q3, h->S3, h->Q3, 1));
             SAP_LAUNCH_CHECK(h, "k_strided<FWD,y>");
         }
         // F2x + F3 + F4x: x forward, spectral solve, x inverse (3 -> 1)
-        k_strided<N, MODE_SOLVE, C::NT_ST><<<dim3(strided_tiles<N>(), B), C::NT_ST, strided_smem_bytes<N, MODE_SOLVE>(), st>>>(
+        k_strided<N, MODE_SOLVE, C::NTX, C::WX><<<dim3(strided_tiles<N, C::WX>(), B), C::NTX, strided_smem_bytes<N, C::WX>(), st>>>(
             sp(h, h->S3, h->Q3, h->S1, h->Q1, 0));
         SAP_LAUNCH_CHECK(h, "k_strided<SOLVE>");
         if (!C::FUSED_ZY) {
-            k_strided<N, MODE_INV, C::NT_ST><<<dim3(strided_tiles<N>(), B), C::NT_ST, strided_smem_bytes<N, MODE_INV>(), st>>>(
+            k_strided<N, MODE_INV, C::NTY, C::WY><<<dim3(strided_tiles<N, C::WY>(), B), C::NTY, strided_smem_bytes<N, C::WY>(), st>>>(
                 sp(h, h->S1, h->Q1, h->S1, h->Q1, 1));
             SAP_LAUNCH_CHECK(h, "k_strided<INV,y>");
         }
@@ -392,7 +394,7 @@ template <int N> struct Runner {
         {
             ZyInvParams p{h->S1, h->Q1, chi, h->tw};
             k_zy_inv<N, C::NL, C::FUSED_ZY, C::NT_ZY>
-                <<<dim3(N * N / C::NL, B), C::NT_ZY, zy_smem_bytes<N, C::NL, C::FUSED_ZY, false>(), st>>>(p);
+                <<<dim3(N * N / C::NL, B), C::NT_ZY, zy_smem_bytes<N, C::NL>(), st>>>(p);
             SAP_LAUNCH_CHECK(h, "k_zy_inv");
         }
         // F5 normalise
@@ -425,20 +427,20 @@ template <int N> struct Runner {
         {
             ZyFwdParams p{gchi, h->W, h->bw, h->S1, h->Q1, h->tw, 1};
             k_zy_fwd<N, C::NL, C::FUSED_ZY, true, C::NT_ZY>
-                <<<dim3(N * N / C::NL, B), C::NT_ZY, zy_smem_bytes<N, C::NL, C::FUSED_ZY, true>(), st>>>(p);
+                <<<dim3(N * N / C::NL, B), C::NT_ZY, zy_smem_bytes<N, C::NL>(), st>>>(p);
             SAP_LAUNCH_CHECK(h, "k_zy_fwd<GBAR>");
         }
         if (!C::FUSED_ZY) {
-            k_strided<N, MODE_FWD, C::NT_ST><<<dim3(strided_tiles<N>(), B), C::NT_ST, strided_smem_bytes<N, MODE_FWD>(), st>>>(
+            k_strided<N, MODE_FWD, C::NTY, C::WY><<<dim3(strided_tiles<N, C::WY>(), B), C::NTY, strided_smem_bytes<N, C::WY>(), st>>>(
                 sp(h, h->S1, h->Q1, h->S1, h->Q1, 1));
             SAP_LAUNCH_CHECK(h, "k_strided<FWD,y>");
         }
         // B3x + B4 + B5x: x forward, transposed multiplier, 3 x inverse
-        k_strided<N, MODE_ADJ, C::NT_ST><<<dim3(strided_tiles<N>(), B), C::NT_ST, strided_smem_bytes<N, MODE_ADJ>(), st>>>(
+        k_strided<N, MODE_ADJ, C::NTX, C::WX><<<dim3(strided_tiles<N, C::WX>(), B), C::NTX, strided_smem_bytes<N, C::WX>(), st>>>(
             sp(h, h->S1, h->Q1, h->S3, h->Q3, 0));
         SAP_LAUNCH_CHECK(h, "k_strided<ADJ>");
         if (!C::FUSED_ZY) {
-            k_strided<N, MODE_INV, C::NT_ST><<<dim3(strided_tiles<N>(), B * 3), C::NT_ST, strided_smem_bytes<N, MODE_INV>(), st>>>(
+            k_strided<N, MODE_INV, C::NTY, C::WY><<<dim3(strided_tiles<N, C::WY>(), B * 3), C::NTY, strided_smem_bytes<N, C::WY>(), st>>>(
                 sp(h, h->S3, h->Q3, h->S3, h->Q3, 1));
             SAP_LAUNCH_CHECK(h, "k_strided<INV,y>");
         }
@@ -446,7 +448,7 @@ template <int N> struct Runner {
         {
             ZyInvParams p{h->S3, h->Q3, h->v, h->tw};
             k_zy_inv<N, C::NL, C::FUSED_ZY, C::NT_ZY>
-                <<<dim3(N * N / C::NL, B * 3), C::NT_ZY, zy_smem_bytes<N, C::NL, C::FUSED_ZY, false>(), st>>>(p);
+                <<<dim3(N * N / C::NL, B * 3), C::NT_ZY, zy_smem_bytes<N, C::NL>(), st>>>(p);
             SAP_LAUNCH_CHECK(h, "k_zy_inv");
         }
         // B6 gather

@@ -1,0 +1,278 @@
+// zy_pass.cuh -- z (+ y) passes: real lines <-> half spectrum (F2/F4 and B3/B5 of SURVEY 8(a)).
+//
+// One block owns NL z-lines (consecutive in memory, NL % 32 == 0).  With DO_Y (N <= 128) NL == N: the
+// block owns a whole x-plane and transforms along z and y in ONE trip through shared memory.
+// Shared-memory traffic is kept to ~6 passes per plane: the first z stage runs global -> registers ->
+// smem, the r2c split is fused into the first y stage, and the last y stage runs smem -> registers ->
+// global (and the mirror image for the inverse).
+// smem: (H+1) rows (kz slots + Nyquist) x PITCH = NL+1 columns (lines); PITCH == 1 (mod 16).
+#pragma once
+#include "fft_core.cuh"
+
+namespace sap {
+
+struct ZyFwdParams {
+    const float* in;    // [planes][N^3] real input (v, or G in GBAR mode)
+    const float* W;     // GBAR: [batch][N^3] point density
+    const float* bw;    // GBAR: [batch][4] = {s, beta/P, S1/a, -}
+    float2* S;          // [planes][N*N*H]
+    float2* Q;          // [planes][N*N]
+    const float2* tw;   // exp(-2 pi i t / N), t < N
+    int nch;            // planes per batch item
+};
+struct ZyInvParams {
+    const float2* S;
+    const float2* Q;
+    float* out;         // [planes][N^3]
+    const float2* tw;
+};
+
+template <int N, int NL> constexpr size_t zy_smem_bytes() { return ((size_t)(N / 2 + 1) * (NL + 1) + N) * sizeof(float2); }
+
+// task t -> (line, q) for the global<->smem z stage: q (ST0 consecutive complex of one line) fastest,
+// the 32/ST0 lines of a warp spaced ST0 apart so that (q + line) is distinct mod 16 per half-warp.
+template <int ST0> SAP_HD void zline_task(int t, int& line, int& q) {
+    constexpr int s = (ST0 > 16) ? 16 : ST0;  // ST0 <= 16 for every supported plan
+    const int g = t >> 5, w = t & 31;
+    q = w % s;
+    const int i = w / s;
+    line = i * s + (g % s) + 32 * (g / s);
+}
+
+// ---- forward ---------------------------------------------------------------------------------------
+template <int N, int NL, bool DO_Y, bool GBAR, class Ctx>
+SAP_HD void zy_fwd_body(Ctx& ctx, const ZyFwdParams& p, float2* smem, int bx, int by) {
+    constexpr int H = N / 2;
+    constexpr int PITCH = NL + 1;
+    constexpr int R0 = StageInfo<H, 0>::R, ST0 = StageInfo<H, 0>::ST;
+    static_assert(NL % 32 == 0 && ST0 <= 16, "line-group mapping");
+    static_assert(!DO_Y || NL == N, "plane mode owns N lines");
+    float2* s = smem;
+    float2* tw = smem + (H + 1) * PITCH;
+    const size_t V = (size_t)N * N * N;
+    const size_t line0 = (size_t)bx * NL;  // global line index = x*N + y
+    for (int i = ctx.tid; i < N; i += ctx.nthr) tw[i] = p.tw[i];
+    ctx.sync();
+
+    // A: global -> z stage 0 (registers) -> smem
+    {
+        const float2* in2 = reinterpret_cast<const float2*>(p.in + (size_t)by * V) + line0 * H;
+        const float2* w2 = nullptr;
+        float cs_ = 0.f, cw = 0.f, c0 = 0.f;
+        if (GBAR) {
+            const int item = by / p.nch;
+            w2 = reinterpret_cast<const float2*>(p.W + (size_t)item * V) + line0 * H;
+            cs_ = p.bw[item * 4 + 0]; cw = p.bw[item * 4 + 1]; c0 = p.bw[item * 4 + 2];
+        }
+        for (int t = ctx.tid; t < NL * ST0; t += ctx.nthr) {
+            int l, q;
+            zline_task<ST0>(t, l, q);
+            float2 v[R0];
+#pragma unroll
+            for (int r = 0; r < R0; ++r) {
+                const int e = l * H + q + ST0 * r;
+                float2 x = in2[e];
+                if (GBAR) {
+                    const float2 w = w2[e];
+                    x = make_float2(cs_ * x.x + cw * w.x, cs_ * x.y + cw * w.y);
+                    if (line0 == 0 && e == 0) x.x -= c0;
+                }
+                v[r] = x;
+            }
+            bfly_fwd<H, 0, N>(v, q, tw);
+#pragma unroll
+            for (int r = 0; r < R0; ++r) s[(q + ST0 * r) * PITCH + l] = v[r];
+        }
+        ctx.sync();
+    }
+    // B: remaining z stages in shared memory, one line per lane
+    if constexpr (Plan<H>::NS > 1) {
+        fft_stage<H, 1, false, N, true>(s, PITCH, 1, NL, tw, ctx.tid, ctx.nthr);
+        ctx.sync();
+    }
+    if constexpr (Plan<H>::NS > 2) {
+        fft_stage<H, 2, false, N, true>(s, PITCH, 1, NL, tw, ctx.tid, ctx.nthr);
+        ctx.sync();
+    }
+    float2* So = p.S + (size_t)by * ((size_t)N * N * H) + line0 * H;
+    float2* Qo = p.Q + (size_t)by * ((size_t)N * N) + line0;
+    if constexpr (!DO_Y) {
+        // C: in-place Hermitian split, then copy out (slot-major rows are contiguous in HBM)
+        r2c_split<N, N>(ctx, s, PITCH, 1, NL, tw);
+        ctx.sync();
+        for (int i = ctx.tid; i < NL * H; i += ctx.nthr) {
+            const int l = i / H, pz = i - l * H;
+            So[i] = s[pz * PITCH + l];
+        }
+        for (int l = ctx.tid; l < NL; l += ctx.nthr) Qo[l] = s[H * PITCH + l];
+    } else {
+        static_assert(!DO_Y || Plan<N>::NS == 2, "fused planes use two-stage y plans");
+        // C: r2c split fused into y stage 0.  One task owns the row pair (k, H-k) for R y-values.
+        constexpr int RY = StageInfo<N, 0>::R, STY = StageInfo<N, 0>::ST;
+        constexpr int TWMUL = 1;  // tw has length N: w_N^k = tw[k]
+        for (int t = ctx.tid; t < (H / 2 + 1) * STY; t += ctx.nthr) {
+            const int k = t / STY, q = t - k * STY;
+            float2 a[RY], b[RY];
+            int ra, rb;
+            if (k == 0) {
+                ra = 0; rb = H;
+#pragma unroll
+                for (int r = 0; r < RY; ++r) {
+                    const float2 z = s[q + STY * r];
+                    a[r] = make_float2(z.x + z.y, 0.f);
+                    b[r] = make_float2(z.x - z.y, 0.f);
+                }
+            } else if (k == H / 2) {
+                ra = rb = freq2pos<H>(k);
+#pragma unroll
+                for (int r = 0; r < RY; ++r) {
+                    const float2 z = s[ra * PITCH + q + STY * r];
+                    a[r] = make_float2(z.x, -z.y);
+                    b[r] = a[r];
+                }
+            } else {
+                ra = freq2pos<H>(k); rb = freq2pos<H>(H - k);
+                const float2 w = tw[k * TWMUL];
+#pragma unroll
+                for (int r = 0; r < RY; ++r) {
+                    a[r] = s[ra * PITCH + q + STY * r];
+                    b[r] = s[rb * PITCH + q + STY * r];
+                    r2c_pair(a[r], b[r], w);
+                }
+            }
+            bfly_fwd<N, 0, N>(a, q, tw);
+#pragma unroll
+            for (int r = 0; r < RY; ++r) s[ra * PITCH + q + STY * r] = a[r];
+            if (rb != ra) {
+                bfly_fwd<N, 0, N>(b, q, tw);
+#pragma unroll
+                for (int r = 0; r < RY; ++r) s[rb * PITCH + q + STY * r] = b[r];
+            }
+        }
+        ctx.sync();
+        // D: last y stage smem -> registers -> global; lanes over kz slots (contiguous in HBM)
+        constexpr int R1 = StageInfo<N, 1>::R;
+        static_assert(StageInfo<N, 1>::ST == 1, "last stage");
+        for (int t = ctx.tid; t < H * (N / R1); t += ctx.nthr) {
+            const int blk = t / H, pz = t - blk * H;
+            float2 v[R1];
+#pragma unroll
+            for (int r = 0; r < R1; ++r) v[r] = s[pz * PITCH + blk * R1 + r];
+            dft_fwd<R1>(v);
+#pragma unroll
+            for (int r = 0; r < R1; ++r) So[(size_t)(blk * R1 + r) * H + pz] = v[r];
+        }
+        for (int blk = ctx.tid; blk < N / R1; blk += ctx.nthr) {  // Nyquist row
+            float2 v[R1];
+#pragma unroll
+            for (int r = 0; r < R1; ++r) v[r] = s[H * PITCH + blk * R1 + r];
+            dft_fwd<R1>(v);
+#pragma unroll
+            for (int r = 0; r < R1; ++r) Qo[blk * R1 + r] = v[r];
+        }
+    }
+}
+
+// ---- inverse: mirror image -------------------------------------------------------------------------
+template <int N, int NL, bool DO_Y, class Ctx>
+SAP_HD void zy_inv_body(Ctx& ctx, const ZyInvParams& p, float2* smem, int bx, int by) {
+    constexpr int H = N / 2;
+    constexpr int PITCH = NL + 1;
+    constexpr int R0 = StageInfo<H, 0>::R, ST0 = StageInfo<H, 0>::ST;
+    static_assert(NL % 32 == 0 && ST0 <= 16, "line-group mapping");
+    float2* s = smem;
+    float2* tw = smem + (H + 1) * PITCH;
+    const size_t V = (size_t)N * N * N;
+    const size_t line0 = (size_t)bx * NL;
+    for (int i = ctx.tid; i < N; i += ctx.nthr) tw[i] = p.tw[i];
+    const float2* Si = p.S + (size_t)by * ((size_t)N * N * H) + line0 * H;
+    const float2* Qi = p.Q + (size_t)by * ((size_t)N * N) + line0;
+    if constexpr (!DO_Y) {
+        for (int i = ctx.tid; i < NL * H; i += ctx.nthr) {
+            const int l = i / H, pz = i - l * H;
+            s[pz * PITCH + l] = Si[i];
+        }
+        for (int l = ctx.tid; l < NL; l += ctx.nthr) s[H * PITCH + l] = Qi[l];
+        ctx.sync();
+        c2r_split<N, N>(ctx, s, PITCH, 1, NL, tw);
+        ctx.sync();
+    } else {
+        static_assert(!DO_Y || Plan<N>::NS == 2, "fused planes use two-stage y plans");
+        // D': global -> registers -> inverse of the last y stage -> smem; lanes over kz slots
+        constexpr int R1 = StageInfo<N, 1>::R;
+        for (int t = ctx.tid; t < H * (N / R1); t += ctx.nthr) {
+            const int blk = t / H, pz = t - blk * H;
+            float2 v[R1];
+#pragma unroll
+            for (int r = 0; r < R1; ++r) v[r] = Si[(size_t)(blk * R1 + r) * H + pz];
+            dft_inv<R1>(v);
+#pragma unroll
+            for (int r = 0; r < R1; ++r) s[pz * PITCH + blk * R1 + r] = v[r];
+        }
+        for (int blk = ctx.tid; blk < N / R1; blk += ctx.nthr) {
+            float2 v[R1];
+#pragma unroll
+            for (int r = 0; r < R1; ++r) v[r] = Qi[blk * R1 + r];
+            dft_inv<R1>(v);
+#pragma unroll
+            for (int r = 0; r < R1; ++r) s[H * PITCH + blk * R1 + r] = v[r];
+        }
+        ctx.sync();
+        // C': inverse y stage 0 on the row pair (k, H-k), then the c2r split, in registers
+        constexpr int RY = StageInfo<N, 0>::R, STY = StageInfo<N, 0>::ST;
+        for (int t = ctx.tid; t < (H / 2 + 1) * STY; t += ctx.nthr) {
+            const int k = t / STY, q = t - k * STY;
+            float2 a[RY], b[RY];
+            const int ra = (k == 0) ? 0 : freq2pos<H>(k);
+            const int rb = (k == 0) ? H : freq2pos<H>(H - k);
+#pragma unroll
+            for (int r = 0; r < RY; ++r) a[r] = s[ra * PITCH + q + STY * r];
+            bfly_inv<N, 0, N>(a, q, tw);
+            if (rb != ra) {
+#pragma unroll
+                for (int r = 0; r < RY; ++r) b[r] = s[rb * PITCH + q + STY * r];
+                bfly_inv<N, 0, N>(b, q, tw);
+            }
+            if (k == 0) {
+#pragma unroll
+                for (int r = 0; r < RY; ++r)
+                    s[q + STY * r] = make_float2(0.5f * (a[r].x + b[r].x), 0.5f * (a[r].x - b[r].x));
+            } else if (k == H / 2) {
+#pragma unroll
+                for (int r = 0; r < RY; ++r) s[ra * PITCH + q + STY * r] = make_float2(a[r].x, -a[r].y);
+            } else {
+                const float2 w = tw[k];
+#pragma unroll
+                for (int r = 0; r < RY; ++r) {
+                    c2r_pair(a[r], b[r], w);
+                    s[ra * PITCH + q + STY * r] = a[r];
+                    s[rb * PITCH + q + STY * r] = b[r];
+                }
+            }
+        }
+        ctx.sync();
+    }
+    // B': inverse z stages that stay in shared memory (last plan stage first)
+    if constexpr (Plan<H>::NS > 2) {
+        fft_stage<H, 2, true, N, true>(s, PITCH, 1, NL, tw, ctx.tid, ctx.nthr);
+        ctx.sync();
+    }
+    if constexpr (Plan<H>::NS > 1) {
+        fft_stage<H, 1, true, N, true>(s, PITCH, 1, NL, tw, ctx.tid, ctx.nthr);
+        ctx.sync();
+    }
+    // A': smem -> inverse z stage 0 (registers) -> global
+    float2* out2 = reinterpret_cast<float2*>(p.out + (size_t)by * V) + line0 * H;
+    for (int t = ctx.tid; t < NL * ST0; t += ctx.nthr) {
+        int l, q;
+        zline_task<ST0>(t, l, q);
+        float2 v[R0];
+#pragma unroll
+        for (int r = 0; r < R0; ++r) v[r] = s[(q + ST0 * r) * PITCH + l];
+        bfly_inv<H, 0, N>(v, q, tw);
+#pragma unroll
+        for (int r = 0; r < R0; ++r) out2[l * H + q + ST0 * r] = v[r];
+    }
+}
+
+}  // namespace sap
