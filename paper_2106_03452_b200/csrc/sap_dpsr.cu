@@ -11,12 +11,45 @@
 
 #include "../../include/sap_dpsr.h"
 #include "dpsr_kernels.cuh"
+#include "strided_async.cuh"
 
 namespace sap {
+
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 
 struct DevCtx {
     int tid, nthr;
     __device__ __forceinline__ void sync() const { __syncthreads(); }
+    // ---- asynchronous-copy pipeline primitives (mbarrier + cp.async.bulk, sm_90+/sm_100a)
+    __device__ __forceinline__ void bar_init(unsigned long long* bar) const {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(bar)) : "memory");
+    }
+    __device__ __forceinline__ void fence_init() const {
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __device__ __forceinline__ void fence_async() const { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+    __device__ __forceinline__ void bar_expect(unsigned long long* bar, unsigned bytes) const {
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+    }
+    __device__ __forceinline__ void bulk_row(float2* dst, const float2* src, unsigned bytes, unsigned long long* bar) const {
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+                     "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                     : "memory");
+    }
+    __device__ __forceinline__ void bar_wait(unsigned long long* bar, unsigned parity) const {
+        const unsigned a = smem_u32(bar);
+        for (unsigned it = 0; it < (1u << 24); ++it) {
+            unsigned ok;
+            asm volatile(
+                "{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
+                : "=r"(ok)
+                : "r"(a), "r"(parity)
+                : "memory");
+            if (ok) return;
+        }
+        __trap();  // a copy never landed: fail loudly instead of hanging the GPU
+    }
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -39,6 +72,13 @@ __global__ void __launch_bounds__(NT) k_strided(StridedParams p) {
     extern __shared__ float2 smem[];
     DevCtx ctx{(int)threadIdx.x, NT};
     strided_body<N, MODE, NT, W>(ctx, p, smem, (int)blockIdx.x, (int)blockIdx.y);
+}
+
+template <int N, int MODE, int NT, int W, int NB>
+__global__ void __launch_bounds__(NT) k_strided_async(StridedParams p, int nby) {
+    extern __shared__ __align__(128) float2 smem[];
+    DevCtx ctx{(int)threadIdx.x, NT};
+    strided_async_body<N, MODE, NT, W, NB>(ctx, p, smem, (int)blockIdx.x, (int)gridDim.x, nby);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -254,7 +294,7 @@ __global__ void k_gather_grads(const float* __restrict__ pts, const float* __res
 // handle, launch plumbing
 // ================================================================================================
 struct sap_dpsr {
-    int N = 0, batch = 0, max_points = 0, device = 0;
+    int N = 0, batch = 0, max_points = 0, device = 0, num_sms = 148;
     float sigma = 0.f;
     // workspace (device)
     float* v = nullptr;        // [B][3][N^3]  splatted field / vbar
@@ -328,8 +368,9 @@ template <int N> struct Cfg {
     static constexpr int NL = FUSED_ZY ? N : 32;
     static constexpr int NT_ZY = 256;
     // strided tiles: columns per tile (W) and threads, for the plain y pass (Y) and the fused x pass (X)
-    static constexpr int WY = 16, NTY = 256;
-    static constexpr int WX = (N >= 64) ? 32 : 16, NTX = (N >= 256) ? 512 : 256;
+    static constexpr bool ASYNC_X = false, ASYNC_Y = false;
+    static constexpr int WY = 16, NTY = 256, NBY = 3;
+    static constexpr int WX = (N >= 64) ? 32 : 16, NTX = (N >= 256) ? 512 : 256, NBX = (N >= 256) ? 2 : 4;
 };
 
 template <int N> struct Runner {
@@ -346,6 +387,10 @@ template <int N> struct Runner {
         upd(set_smem(k_strided<N, MODE_ADJ, C::NTX, C::WX>, strided_smem_bytes<N, C::WX>()));
         upd(set_smem(k_strided<N, MODE_FWD, C::NTY, C::WY>, strided_smem_bytes<N, C::WY>()));
         upd(set_smem(k_strided<N, MODE_INV, C::NTY, C::WY>, strided_smem_bytes<N, C::WY>()));
+        upd(set_smem(k_strided_async<N, MODE_SOLVE, C::NTX, C::WX, C::NBX>, strided_async_smem_bytes<N, MODE_SOLVE, C::WX, C::NBX>()));
+        upd(set_smem(k_strided_async<N, MODE_ADJ, C::NTX, C::WX, C::NBX>, strided_async_smem_bytes<N, MODE_ADJ, C::WX, C::NBX>()));
+        upd(set_smem(k_strided_async<N, MODE_FWD, C::NTY, C::WY, C::NBY>, strided_async_smem_bytes<N, MODE_FWD, C::WY, C::NBY>()));
+        upd(set_smem(k_strided_async<N, MODE_INV, C::NTY, C::WY, C::NBY>, strided_async_smem_bytes<N, MODE_INV, C::WY, C::NBY>()));
         return cuda_ok(h, e, "cudaFuncSetAttribute") ? SAP_OK : SAP_ERR_CUDA;
     }
 
@@ -355,6 +400,24 @@ template <int N> struct Runner {
         p.cg = 2.f * h->sigma * h->sigma / ((float)N * (float)N);
         p.cs = (float)((2.0 / ((double)N * N * N)) / (-2.0 * 3.14159265358979323846));
         return p;
+    }
+
+    // persistent launch: as many CTAs as fit the chip at once (or fewer if there is less work)
+    template <int MODE, int NT, int W, int NB>
+    static void launch_strided(sap_dpsr* h, cudaStream_t st, int planes, const StridedParams& p) {
+        constexpr bool ASYNC = (MODE == MODE_SOLVE || MODE == MODE_ADJ) ? C::ASYNC_X : C::ASYNC_Y;
+        if (!ASYNC) {
+            k_strided<N, MODE, NT, W><<<dim3(strided_tiles<N, W>(), planes), NT, strided_smem_bytes<N, W>(), st>>>(p);
+            return;
+        }
+        constexpr size_t smem = strided_async_smem_bytes<N, MODE, W, NB>();
+        int per_sm = (int)((227 * 1024) / (smem + 1024));
+        if (per_sm > 2048 / NT) per_sm = 2048 / NT;
+        if (per_sm < 1) per_sm = 1;
+        long long work = (long long)strided_tiles<N, W>() * planes;
+        long long grid = (long long)h->num_sms * per_sm;
+        if (grid > work) grid = work;
+        k_strided_async<N, MODE, NT, W, NB><<<(unsigned)grid, NT, smem, st>>>(p, planes);
     }
 
     static sap_status_t forward(sap_dpsr* h, const float* pts, const float* nrm, int P, float* chi, cudaStream_t st) {
@@ -377,16 +440,16 @@ template <int N> struct Runner {
             SAP_LAUNCH_CHECK(h, "k_zy_fwd");
         }
         if (!C::FUSED_ZY) {
-            k_strided<N, MODE_FWD, C::NTY, C::WY><<<dim3(strided_tiles<N, C::WY>(), B * 3), C::NTY, strided_smem_bytes<N, C::WY>(), st>>>(
+            launch_strided<MODE_FWD, C::NTY, C::WY, C::NBY>(h, st, B * 3,
                 sp(h, h->S3, h->Q3, h->S3, h->Q3, 1));
             SAP_LAUNCH_CHECK(h, "k_strided<FWD,y>");
         }
         // F2x + F3 + F4x: x forward, spectral solve, x inverse (3 -> 1)
-        k_strided<N, MODE_SOLVE, C::NTX, C::WX><<<dim3(strided_tiles<N, C::WX>(), B), C::NTX, strided_smem_bytes<N, C::WX>(), st>>>(
-            sp(h, h->S3, h->Q3, h->S1, h->Q1, 0));
+        launch_strided<MODE_SOLVE, C::NTX, C::WX, C::NBX>(h, st, B,
+                sp(h, h->S3, h->Q3, h->S1, h->Q1, 0));
         SAP_LAUNCH_CHECK(h, "k_strided<SOLVE>");
         if (!C::FUSED_ZY) {
-            k_strided<N, MODE_INV, C::NTY, C::WY><<<dim3(strided_tiles<N, C::WY>(), B), C::NTY, strided_smem_bytes<N, C::WY>(), st>>>(
+            launch_strided<MODE_INV, C::NTY, C::WY, C::NBY>(h, st, B,
                 sp(h, h->S1, h->Q1, h->S1, h->Q1, 1));
             SAP_LAUNCH_CHECK(h, "k_strided<INV,y>");
         }
@@ -431,16 +494,16 @@ template <int N> struct Runner {
             SAP_LAUNCH_CHECK(h, "k_zy_fwd<GBAR>");
         }
         if (!C::FUSED_ZY) {
-            k_strided<N, MODE_FWD, C::NTY, C::WY><<<dim3(strided_tiles<N, C::WY>(), B), C::NTY, strided_smem_bytes<N, C::WY>(), st>>>(
+            launch_strided<MODE_FWD, C::NTY, C::WY, C::NBY>(h, st, B,
                 sp(h, h->S1, h->Q1, h->S1, h->Q1, 1));
             SAP_LAUNCH_CHECK(h, "k_strided<FWD,y>");
         }
         // B3x + B4 + B5x: x forward, transposed multiplier, 3 x inverse
-        k_strided<N, MODE_ADJ, C::NTX, C::WX><<<dim3(strided_tiles<N, C::WX>(), B), C::NTX, strided_smem_bytes<N, C::WX>(), st>>>(
-            sp(h, h->S1, h->Q1, h->S3, h->Q3, 0));
+        launch_strided<MODE_ADJ, C::NTX, C::WX, C::NBX>(h, st, B,
+                sp(h, h->S1, h->Q1, h->S3, h->Q3, 0));
         SAP_LAUNCH_CHECK(h, "k_strided<ADJ>");
         if (!C::FUSED_ZY) {
-            k_strided<N, MODE_INV, C::NTY, C::WY><<<dim3(strided_tiles<N, C::WY>(), B * 3), C::NTY, strided_smem_bytes<N, C::WY>(), st>>>(
+            launch_strided<MODE_INV, C::NTY, C::WY, C::NBY>(h, st, B * 3,
                 sp(h, h->S3, h->Q3, h->S3, h->Q3, 1));
             SAP_LAUNCH_CHECK(h, "k_strided<INV,y>");
         }
@@ -500,7 +563,7 @@ extern "C" sap_status_t sap_dpsr_create(int N, float sigma, int batch, int max_p
 
     sap_dpsr* h = new (std::nothrow) sap_dpsr;
     if (!h) { g_create_err = "host allocation failed"; return SAP_ERR_OOM; }
-    h->N = N; h->sigma = sigma; h->batch = batch; h->max_points = max_points; h->device = dev;
+    h->num_sms = prop.multiProcessorCount; h->N = N; h->sigma = sigma; h->batch = batch; h->max_points = max_points; h->device = dev;
     const size_t V = (size_t)N * N * N, SP = (size_t)N * N * (N / 2), QP = (size_t)N * N, B = (size_t)batch;
     cudaError_t e = cudaSuccess;
     auto upd = [&](cudaError_t x) { if (e == cudaSuccess) e = x; };
