@@ -20,6 +20,7 @@ __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)_
 struct DevCtx {
     int tid, nthr;
     __device__ __forceinline__ void sync() const { __syncthreads(); }
+    __device__ __forceinline__ void atomic_add(float* p, float v) const { atomicAdd(p, v); }
     // ---- asynchronous-copy pipeline primitives (mbarrier + cp.async.bulk, sm_90+/sm_100a)
     __device__ __forceinline__ void bar_init(unsigned long long* bar) const {
         asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(bar)) : "memory");
@@ -55,11 +56,11 @@ struct DevCtx {
 // ------------------------------------------------------------------------------------------------
 // __global__ wrappers around the block bodies
 // ------------------------------------------------------------------------------------------------
-template <int N, int NL, bool DO_Y, bool GBAR, int NT>
+template <int N, int NL, bool DO_Y, int SRC, int NT>
 __global__ void __launch_bounds__(NT) k_zy_fwd(ZyFwdParams p) {
     extern __shared__ float2 smem[];
     DevCtx ctx{(int)threadIdx.x, NT};
-    zy_fwd_body<N, NL, DO_Y, GBAR>(ctx, p, smem, (int)blockIdx.x, (int)blockIdx.y);
+    zy_fwd_body<N, NL, DO_Y, SRC>(ctx, p, smem, (int)blockIdx.x, (int)blockIdx.y);
 }
 template <int N, int NL, bool DO_Y, int NT>
 __global__ void __launch_bounds__(NT) k_zy_inv(ZyInvParams p) {
@@ -84,12 +85,6 @@ __global__ void __launch_bounds__(NT) k_strided_async(StridedParams p, int nby) 
 // ------------------------------------------------------------------------------------------------
 // pointwise / point kernels
 // ------------------------------------------------------------------------------------------------
-__global__ void k_zero(float4* __restrict__ p, size_t n4) {
-    const size_t stride = (size_t)gridDim.x * blockDim.x;
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += stride)
-        p[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-}
-
 struct Corner {
     int j0[3];
     float f[3];
@@ -112,29 +107,68 @@ __device__ __forceinline__ size_t vox(int N, int jx, int jy, int jz) {
     return ((size_t)(jx & M) * N + (jy & M)) * N + (jz & M);
 }
 
-// F1: v[ch][j] += w n[ch], W[j] += w over the 8 neighbours.  One thread per point; global RED.
-__global__ void k_splat(const float* __restrict__ pts, const float* __restrict__ nrm, int P, int N,
-                        float* __restrict__ v, float* __restrict__ W) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    const int b = blockIdx.y;
+// ---- F1a: counting sort of the points by bin key j0x * NTY + j0y / NL (NTY = N / NL) -----------------
+// The z/y forward kernel rasterises each block's lines from the bins that can touch them, so the
+// splatted field never exists in HBM (no zero fill, no global atomics on the grid).
+__device__ __forceinline__ int bin_key(const float* __restrict__ c, int N, int NL) {
+    const int M = N - 1;
+    const int jx = (int)floorf(c[0] * (float)N) & M, jy = (int)floorf(c[1] * (float)N) & M;
+    return jx * (N / NL) + jy / NL;
+}
+__global__ void k_bin_count(const float* __restrict__ pts, int P, int N, int NL, int nbins, int* __restrict__ cnt) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y;
     if (i >= P) return;
-    const size_t V = (size_t)N * N * N;
+    atomicAdd(cnt + (size_t)b * nbins + bin_key(pts + ((size_t)b * P + i) * 3, N, NL), 1);
+}
+// one block per item: exclusive scan of the counts -> start[nbins+1]; cursor = start; counts reset to 0
+__global__ void k_bin_scan(int* __restrict__ cnt, int nbins, int P, int* __restrict__ start, int* __restrict__ cursor) {
+    __shared__ int wsum[32];
+    const int b = blockIdx.x, tid = threadIdx.x, nt = blockDim.x;
+    int* c = cnt + (size_t)b * nbins;
+    int* st = start + (size_t)b * (nbins + 1);
+    int* cu = cursor + (size_t)b * nbins;
+    const int per = (nbins + nt - 1) / nt;
+    const int lo = tid * per, hi = min(lo + per, nbins);
+    int local = 0;
+    for (int i = lo; i < hi; ++i) local += c[i];
+    int incl = local;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(0xffffffffu, incl, o);
+        if ((tid & 31) >= o) incl += t;
+    }
+    if ((tid & 31) == 31) wsum[tid >> 5] = incl;
+    __syncthreads();
+    if (tid < 32) {
+        int w = (tid < (nt >> 5)) ? wsum[tid] : 0;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, w, o);
+            if (tid >= o) w += t;
+        }
+        wsum[tid] = w;  // inclusive over warps
+    }
+    __syncthreads();
+    int run = incl - local + ((tid >> 5) ? wsum[(tid >> 5) - 1] : 0);
+    for (int i = lo; i < hi; ++i) {
+        const int n = c[i];
+        st[i] = run;
+        cu[i] = run;
+        c[i] = 0;
+        run += n;
+    }
+    if (tid == 0) st[nbins] = P;
+}
+__global__ void k_bin_scatter(const float* __restrict__ pts, const float* __restrict__ nrm, int P, int N, int NL,
+                              int nbins, int* __restrict__ cursor, float4* __restrict__ spts,
+                              float4* __restrict__ snrm) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y;
+    if (i >= P) return;
     const float* c = pts + ((size_t)b * P + i) * 3;
     const float* n = nrm + ((size_t)b * P + i) * 3;
-    const Corner k = corner_of(c, N);
-    const float n0 = n[0], n1 = n[1], n2 = n[2];
-    float* vb = v + (size_t)b * 3 * V;
-    float* Wb = W + (size_t)b * V;
-#pragma unroll
-    for (int d = 0; d < 8; ++d) {
-        const int dx = d >> 2, dy = (d >> 1) & 1, dz = d & 1;
-        const float w = (dx ? k.f[0] : 1.f - k.f[0]) * (dy ? k.f[1] : 1.f - k.f[1]) * (dz ? k.f[2] : 1.f - k.f[2]);
-        const size_t j = vox(N, k.j0[0] + dx, k.j0[1] + dy, k.j0[2] + dz);
-        atomicAdd(vb + j, w * n0);
-        atomicAdd(vb + V + j, w * n1);
-        atomicAdd(vb + 2 * V + j, w * n2);
-        atomicAdd(Wb + j, w);
-    }
+    const int pos = atomicAdd(cursor + (size_t)b * nbins + bin_key(c, N, NL), 1);
+    spts[(size_t)b * P + pos] = make_float4(c[0], c[1], c[2], 0.f);
+    snrm[(size_t)b * P + pos] = make_float4(n[0], n[1], n[2], 0.f);
 }
 
 __device__ __forceinline__ float warp_sum(float x) {
@@ -298,7 +332,12 @@ struct sap_dpsr {
     float sigma = 0.f;
     // workspace (device)
     float* v = nullptr;        // [B][3][N^3]  splatted field / vbar
-    float* W = nullptr;        // [B][N^3]     point density
+    float4* spts = nullptr;    // [B][max_points] points sorted by bin
+    float4* snrm = nullptr;    // [B][max_points] normals, same order
+    int* bin_cnt = nullptr;    // [B][nbins]   (zero between calls)
+    int* bin_cursor = nullptr; // [B][nbins]
+    int* bin_start = nullptr;  // [B][nbins+1]
+    int nbins = 0;
     float2* S3 = nullptr;      // [B*3][N*N*H] 3-channel spectra
     float2* Q3 = nullptr;      // [B*3][N*N]
     float2* S1 = nullptr;      // [B][N*N*H]   1-channel spectrum
@@ -311,6 +350,7 @@ struct sap_dpsr {
     // staging for the *_host entry points (allocated on first use)
     float *h_pts = nullptr, *h_nrm = nullptr, *h_chi = nullptr, *h_gchi = nullptr, *h_gp = nullptr, *h_gn = nullptr;
     int host_P = 0;
+    int binned_P = 0;          // num_points of the forward whose bins are in the workspace
     size_t ws_bytes = 0;
     int launches = 0;
     // optional per-kernel timing (sap_dpsr_set_profiling): one event before the first launch, one after each
@@ -380,17 +420,21 @@ template <int N> struct Runner {
     static sap_status_t prepare(sap_dpsr* h) {
         cudaError_t e = cudaSuccess;
         auto upd = [&](cudaError_t x) { if (e == cudaSuccess) e = x; };
-        upd(set_smem(k_zy_fwd<N, C::NL, C::FUSED_ZY, false, C::NT_ZY>, zy_smem_bytes<N, C::NL>()));
-        upd(set_smem(k_zy_fwd<N, C::NL, C::FUSED_ZY, true, C::NT_ZY>, zy_smem_bytes<N, C::NL>()));
+        upd(set_smem(k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_SPLAT, C::NT_ZY>, zy_smem_bytes<N, C::NL>()));
+        upd(set_smem(k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_GBAR, C::NT_ZY>, zy_smem_bytes<N, C::NL>()));
         upd(set_smem(k_zy_inv<N, C::NL, C::FUSED_ZY, C::NT_ZY>, zy_smem_bytes<N, C::NL>()));
         upd(set_smem(k_strided<N, MODE_SOLVE, C::NTX, C::WX>, strided_smem_bytes<N, C::WX>()));
         upd(set_smem(k_strided<N, MODE_ADJ, C::NTX, C::WX>, strided_smem_bytes<N, C::WX>()));
         upd(set_smem(k_strided<N, MODE_FWD, C::NTY, C::WY>, strided_smem_bytes<N, C::WY>()));
         upd(set_smem(k_strided<N, MODE_INV, C::NTY, C::WY>, strided_smem_bytes<N, C::WY>()));
+        if constexpr (C::ASYNC_X) {
         upd(set_smem(k_strided_async<N, MODE_SOLVE, C::NTX, C::WX, C::NBX>, strided_async_smem_bytes<N, MODE_SOLVE, C::WX, C::NBX>()));
         upd(set_smem(k_strided_async<N, MODE_ADJ, C::NTX, C::WX, C::NBX>, strided_async_smem_bytes<N, MODE_ADJ, C::WX, C::NBX>()));
+        }
+        if constexpr (C::ASYNC_Y) {
         upd(set_smem(k_strided_async<N, MODE_FWD, C::NTY, C::WY, C::NBY>, strided_async_smem_bytes<N, MODE_FWD, C::WY, C::NBY>()));
         upd(set_smem(k_strided_async<N, MODE_INV, C::NTY, C::WY, C::NBY>, strided_async_smem_bytes<N, MODE_INV, C::WY, C::NBY>()));
+        }
         return cuda_ok(h, e, "cudaFuncSetAttribute") ? SAP_OK : SAP_ERR_CUDA;
     }
 
@@ -406,36 +450,39 @@ template <int N> struct Runner {
     template <int MODE, int NT, int W, int NB>
     static void launch_strided(sap_dpsr* h, cudaStream_t st, int planes, const StridedParams& p) {
         constexpr bool ASYNC = (MODE == MODE_SOLVE || MODE == MODE_ADJ) ? C::ASYNC_X : C::ASYNC_Y;
-        if (!ASYNC) {
+        if constexpr (!ASYNC) {
             k_strided<N, MODE, NT, W><<<dim3(strided_tiles<N, W>(), planes), NT, strided_smem_bytes<N, W>(), st>>>(p);
-            return;
+        } else {
+            constexpr size_t smem = strided_async_smem_bytes<N, MODE, W, NB>();
+            int per_sm = (int)((227 * 1024) / (smem + 1024));
+            if (per_sm > 2048 / NT) per_sm = 2048 / NT;
+            if (per_sm < 1) per_sm = 1;
+            long long work = (long long)strided_tiles<N, W>() * planes;
+            long long grid = (long long)h->num_sms * per_sm;
+            if (grid > work) grid = work;
+    k_strided_async<N, MODE, NT, W, NB><<<(unsigned)grid, NT, smem, st>>>(p, planes);
         }
-        constexpr size_t smem = strided_async_smem_bytes<N, MODE, W, NB>();
-        int per_sm = (int)((227 * 1024) / (smem + 1024));
-        if (per_sm > 2048 / NT) per_sm = 2048 / NT;
-        if (per_sm < 1) per_sm = 1;
-        long long work = (long long)strided_tiles<N, W>() * planes;
-        long long grid = (long long)h->num_sms * per_sm;
-        if (grid > work) grid = work;
-        k_strided_async<N, MODE, NT, W, NB><<<(unsigned)grid, NT, smem, st>>>(p, planes);
     }
 
     static sap_status_t forward(sap_dpsr* h, const float* pts, const float* nrm, int P, float* chi, cudaStream_t st) {
         const int B = h->batch;
         const size_t V = (size_t)N * N * N;
         prof_begin(h, st);
-        // F1 splat (v and W are contiguous: one zero fill)
+        // F1a: bin the points (counting sort); the rasterisation itself happens inside k_zy_fwd
         {
-            const size_t n4 = (size_t)B * 4 * V / 4;
-            k_zero<<<148 * 8, 256, 0, st>>>(reinterpret_cast<float4*>(h->v), n4);
-            SAP_LAUNCH_CHECK(h, "k_zero");
-            k_splat<<<dim3((P + 127) / 128, B), 128, 0, st>>>(pts, nrm, P, N, h->v, h->W);
-            SAP_LAUNCH_CHECK(h, "k_splat");
+            const dim3 gp((P + 255) / 256, B);
+            k_bin_count<<<gp, 256, 0, st>>>(pts, P, N, C::NL, h->nbins, h->bin_cnt);
+            SAP_LAUNCH_CHECK(h, "k_bin_count");
+            k_bin_scan<<<B, 1024, 0, st>>>(h->bin_cnt, h->nbins, P, h->bin_start, h->bin_cursor);
+            SAP_LAUNCH_CHECK(h, "k_bin_scan");
+            k_bin_scatter<<<gp, 256, 0, st>>>(pts, nrm, P, N, C::NL, h->nbins, h->bin_cursor, h->spts, h->snrm);
+            SAP_LAUNCH_CHECK(h, "k_bin_scatter");
+            h->binned_P = P;
         }
         // F2 z (+y) forward, 3 channels
         {
-            ZyFwdParams p{h->v, nullptr, nullptr, h->S3, h->Q3, h->tw, 3};
-            k_zy_fwd<N, C::NL, C::FUSED_ZY, false, C::NT_ZY>
+            ZyFwdParams p{h->spts, h->snrm, h->bin_start, P, nullptr, nullptr, h->S3, h->Q3, h->tw, 3};
+            k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_SPLAT, C::NT_ZY>
                 <<<dim3(N * N / C::NL, B * 3), C::NT_ZY, zy_smem_bytes<N, C::NL>(), st>>>(p);
             SAP_LAUNCH_CHECK(h, "k_zy_fwd");
         }
@@ -488,8 +535,8 @@ template <int N> struct Runner {
         }
         // B2 + B3: Gbar' assembled on load, z (+y) forward
         {
-            ZyFwdParams p{gchi, h->W, h->bw, h->S1, h->Q1, h->tw, 1};
-            k_zy_fwd<N, C::NL, C::FUSED_ZY, true, C::NT_ZY>
+            ZyFwdParams p{h->spts, h->snrm, h->bin_start, P, gchi, h->bw, h->S1, h->Q1, h->tw, 1};
+            k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_GBAR, C::NT_ZY>
                 <<<dim3(N * N / C::NL, B), C::NT_ZY, zy_smem_bytes<N, C::NL>(), st>>>(p);
             SAP_LAUNCH_CHECK(h, "k_zy_fwd<GBAR>");
         }
@@ -543,7 +590,7 @@ static bool supported_N(int N) { return N == 32 || N == 64 || N == 128 || N == 2
 
 static void free_all(sap_dpsr* h) {
     for (int i = 0; i < sap_dpsr::MAX_EV; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
-    cudaFree(h->v); cudaFree(h->S3); cudaFree(h->Q3); cudaFree(h->S1); cudaFree(h->Q1); cudaFree(h->tw);
+    cudaFree(h->v); cudaFree(h->spts); cudaFree(h->snrm); cudaFree(h->bin_cnt); cudaFree(h->bin_cursor); cudaFree(h->bin_start); cudaFree(h->S3); cudaFree(h->Q3); cudaFree(h->S1); cudaFree(h->Q1); cudaFree(h->tw);
     cudaFree(h->acc); cudaFree(h->ticket); cudaFree(h->stats); cudaFree(h->bw);
     cudaFree(h->h_pts); cudaFree(h->h_nrm); cudaFree(h->h_chi); cudaFree(h->h_gchi); cudaFree(h->h_gp); cudaFree(h->h_gn);
 }
@@ -567,7 +614,13 @@ extern "C" sap_status_t sap_dpsr_create(int N, float sigma, int batch, int max_p
     const size_t V = (size_t)N * N * N, SP = (size_t)N * N * (N / 2), QP = (size_t)N * N, B = (size_t)batch;
     cudaError_t e = cudaSuccess;
     auto upd = [&](cudaError_t x) { if (e == cudaSuccess) e = x; };
-    upd(dev_alloc(h, &h->v, B * 4 * V));
+    h->nbins = N * (N <= 128 ? 1 : N / 32);
+    upd(dev_alloc(h, &h->v, B * 3 * V));
+    upd(dev_alloc(h, &h->spts, B * (size_t)max_points));
+    upd(dev_alloc(h, &h->snrm, B * (size_t)max_points));
+    upd(dev_alloc(h, &h->bin_cnt, B * (size_t)h->nbins));
+    upd(dev_alloc(h, &h->bin_cursor, B * (size_t)h->nbins));
+    upd(dev_alloc(h, &h->bin_start, B * (size_t)(h->nbins + 1)));
     upd(dev_alloc(h, &h->S3, B * 3 * SP));
     upd(dev_alloc(h, &h->Q3, B * 3 * QP));
     upd(dev_alloc(h, &h->S1, B * SP));
@@ -583,7 +636,6 @@ extern "C" sap_status_t sap_dpsr_create(int N, float sigma, int batch, int max_p
         free_all(h); delete h; cudaGetLastError();
         return oom ? SAP_ERR_OOM : SAP_ERR_CUDA;
     }
-    h->W = h->v + B * 3 * V;
     // twiddle table exp(-2 pi i t / N) computed in double
     float2* tw = new (std::nothrow) float2[N];
     if (!tw) { free_all(h); delete h; g_create_err = "host allocation failed"; return SAP_ERR_OOM; }
@@ -593,6 +645,7 @@ extern "C" sap_status_t sap_dpsr_create(int N, float sigma, int batch, int max_p
     }
     upd(cudaMemcpy(h->tw, tw, sizeof(float2) * N, cudaMemcpyHostToDevice));
     delete[] tw;
+    upd(cudaMemset(h->bin_cnt, 0, sizeof(int) * B * h->nbins));
     upd(cudaMemset(h->acc, 0, sizeof(double) * B * 3));
     upd(cudaMemset(h->ticket, 0, sizeof(unsigned) * B * 2));
     upd(cudaMemset(h->stats, 0, sizeof(float) * B * 4));
@@ -630,6 +683,7 @@ extern "C" sap_status_t sap_dpsr_backward(sap_dpsr_t* h, const float* points, co
     sap_status_t st = check_common(h, num_points);
     if (st != SAP_OK) return st;
     if (!points || !normals || !chi || !grad_chi || !grad_points || !grad_normals) { h->err = "null pointer argument"; return SAP_ERR_INVALID_ARG; }
+    if (num_points != h->binned_P) { h->err = "backward must follow a forward call on this handle with the same num_points"; return SAP_ERR_INVALID_ARG; }
     return dispatch(h->N, [&](auto r) {
         return decltype(r)::backward(h, points, normals, num_points, chi, grad_chi, grad_points, grad_normals, (cudaStream_t)stream);
     });

@@ -11,14 +11,23 @@
 
 namespace sap {
 
+// Input of the forward pass.  The real plane is never read from HBM: it is rasterised on the fly
+// ("owner computes") from the points of the bins that can touch this block's lines.
+//   SRC_SPLAT (F1+F2): v_ch = sum_i w n_i[ch]                      (Eq.10-11)
+//   SRC_GBAR  (B2+B3): Gbar' = s G + (beta/P) W - (S1/a) delta_0,  W = sum_i w rasterised the same way
+// Points are pre-sorted by bin key j0x * (N/NL) + j0y / NL (k_bin_* kernels); bin_start has NBINS+1 entries.
+enum { SRC_SPLAT = 0, SRC_GBAR = 1 };
 struct ZyFwdParams {
-    const float* in;    // [planes][N^3] real input (v, or G in GBAR mode)
-    const float* W;     // GBAR: [batch][N^3] point density
-    const float* bw;    // GBAR: [batch][4] = {s, beta/P, S1/a, -}
-    float2* S;          // [planes][N*N*H]
-    float2* Q;          // [planes][N*N]
-    const float2* tw;   // exp(-2 pi i t / N), t < N
-    int nch;            // planes per batch item
+    const float4* spts;    // [batch][P] sorted points  {cx, cy, cz, -}
+    const float4* snrm;    // [batch][P] sorted normals {nx, ny, nz, -}
+    const int* bin_start;  // [batch][NBINS + 1]
+    int P;
+    const float* G;        // GBAR: [batch][N^3] upstream gradient
+    const float* bw;       // GBAR: [batch][4] = {s, beta/P, S1/a, -}
+    float2* S;             // [planes][N*N*H]
+    float2* Q;             // [planes][N*N]
+    const float2* tw;      // exp(-2 pi i t / N), t < N
+    int nch;               // planes per batch item (3 for SPLAT, 1 for GBAR)
 };
 struct ZyInvParams {
     const float2* S;
@@ -40,7 +49,7 @@ template <int ST0> SAP_HD void zline_task(int t, int& line, int& q) {
 }
 
 // ---- forward ---------------------------------------------------------------------------------------
-template <int N, int NL, bool DO_Y, bool GBAR, class Ctx>
+template <int N, int NL, bool DO_Y, int SRC, class Ctx>
 SAP_HD void zy_fwd_body(Ctx& ctx, const ZyFwdParams& p, float2* smem, int bx, int by) {
     constexpr int H = N / 2;
     constexpr int PITCH = NL + 1;
@@ -54,14 +63,75 @@ SAP_HD void zy_fwd_body(Ctx& ctx, const ZyFwdParams& p, float2* smem, int bx, in
     for (int i = ctx.tid; i < N; i += ctx.nthr) tw[i] = p.tw[i];
     ctx.sync();
 
-    // A: global -> z stage 0 (registers) -> smem
+    float2* So = p.S + (size_t)by * ((size_t)N * N * H) + line0 * H;
+    float2* Qo = p.Q + (size_t)by * ((size_t)N * N) + line0;
+    // A0: which bins can touch lines [line0, line0 + NL): x-slabs {x, x-1} x y-tiles {ty, ty-1}
+    constexpr int NTY = N / NL, NBINS = N * NTY, M = N - 1;
+    const int item = by / p.nch, ch = by - item * p.nch;
+    const int x = (int)(line0 / N), y0 = (int)(line0 % N), ty = y0 / NL;
+    const int* bs = p.bin_start + (size_t)item * (NBINS + 1);
+    int b_lo[4], b_n[4], total = 0;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const int xb = (k & 1) ? ((x - 1) & M) : x;
+        const int tb = (k & 2) ? ((ty + NTY - 1) % NTY) : ty;
+        const bool use = (NTY > 1) || !(k & 2);
+        const int bin = xb * NTY + tb;
+        b_lo[k] = use ? bs[bin] : 0;
+        b_n[k] = use ? bs[bin + 1] - b_lo[k] : 0;
+        total += b_n[k];
+    }
+    if (SRC == SRC_SPLAT && total == 0) {  // nothing lands here: the spectrum of zeros is zeros
+        for (int i = ctx.tid; i < NL * H; i += ctx.nthr) So[i] = make_float2(0.f, 0.f);
+        for (int l = ctx.tid; l < NL; l += ctx.nthr) Qo[l] = make_float2(0.f, 0.f);
+        return;
+    }
+    // A1: zero the plane, rasterise the points into it (shared-memory atomics), z = 2m + parity
+    for (int i = ctx.tid; i < H * PITCH; i += ctx.nthr) s[i] = make_float2(0.f, 0.f);
+    ctx.sync();
     {
-        const float2* in2 = reinterpret_cast<const float2*>(p.in + (size_t)by * V) + line0 * H;
-        const float2* w2 = nullptr;
+        float* sf = reinterpret_cast<float*>(s);
+        const float4* sp = p.spts + (size_t)item * p.P;
+        const float4* sn = p.snrm + (size_t)item * p.P;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            for (int i = b_lo[k] + ctx.tid; i < b_lo[k] + b_n[k]; i += ctx.nthr) {
+                const float4 c = sp[i];
+                float val = 1.f;
+                if (SRC == SRC_SPLAT) {
+                    const float4 n = sn[i];
+                    val = (ch == 0) ? n.x : (ch == 1) ? n.y : n.z;
+                }
+                const float tx = c.x * (float)N, tyf = c.y * (float)N, tz = c.z * (float)N;
+                const float fx0 = floorf(tx), fy0 = floorf(tyf), fz0 = floorf(tz);
+                const int jx = (int)fx0, jy = (int)fy0, jz = (int)fz0;
+                const float fx = tx - fx0, fy = tyf - fy0, fz = tz - fz0;
+#pragma unroll
+                for (int dx = 0; dx < 2; ++dx) {
+                    if (((jx + dx) & M) != x) continue;
+                    const float wx = (dx ? fx : 1.f - fx) * val;
+#pragma unroll
+                    for (int dy = 0; dy < 2; ++dy) {
+                        const int ly = ((jy + dy) & M) - y0;
+                        if ((unsigned)ly >= (unsigned)NL) continue;
+                        const float wxy = wx * (dy ? fy : 1.f - fy);
+#pragma unroll
+                        for (int dz = 0; dz < 2; ++dz) {
+                            const int z = (jz + dz) & M;
+                            ctx.atomic_add(sf + ((z >> 1) * PITCH + ly) * 2 + (z & 1), wxy * (dz ? fz : 1.f - fz));
+                        }
+                    }
+                }
+            }
+        }
+    }
+    ctx.sync();
+    // A2: z stage 0 in place (GBAR: combined with G from HBM on the way)
+    {
+        const float2* g2 = nullptr;
         float cs_ = 0.f, cw = 0.f, c0 = 0.f;
-        if (GBAR) {
-            const int item = by / p.nch;
-            w2 = reinterpret_cast<const float2*>(p.W + (size_t)item * V) + line0 * H;
+        if (SRC == SRC_GBAR) {
+            g2 = reinterpret_cast<const float2*>(p.G + (size_t)item * V) + line0 * H;
             cs_ = p.bw[item * 4 + 0]; cw = p.bw[item * 4 + 1]; c0 = p.bw[item * 4 + 2];
         }
         for (int t = ctx.tid; t < NL * ST0; t += ctx.nthr) {
@@ -70,14 +140,14 @@ SAP_HD void zy_fwd_body(Ctx& ctx, const ZyFwdParams& p, float2* smem, int bx, in
             float2 v[R0];
 #pragma unroll
             for (int r = 0; r < R0; ++r) {
-                const int e = l * H + q + ST0 * r;
-                float2 x = in2[e];
-                if (GBAR) {
-                    const float2 w = w2[e];
-                    x = make_float2(cs_ * x.x + cw * w.x, cs_ * x.y + cw * w.y);
-                    if (line0 == 0 && e == 0) x.x -= c0;
+                float2 xv = s[(q + ST0 * r) * PITCH + l];
+                if (SRC == SRC_GBAR) {
+                    const int e = l * H + q + ST0 * r;
+                    const float2 g = g2[e];
+                    xv = make_float2(cs_ * g.x + cw * xv.x, cs_ * g.y + cw * xv.y);
+                    if (line0 == 0 && e == 0) xv.x -= c0;
                 }
-                v[r] = x;
+                v[r] = xv;
             }
             bfly_fwd<H, 0, N>(v, q, tw);
 #pragma unroll
@@ -94,8 +164,6 @@ SAP_HD void zy_fwd_body(Ctx& ctx, const ZyFwdParams& p, float2* smem, int bx, in
         fft_stage<H, 2, false, N, true>(s, PITCH, 1, NL, tw, ctx.tid, ctx.nthr);
         ctx.sync();
     }
-    float2* So = p.S + (size_t)by * ((size_t)N * N * H) + line0 * H;
-    float2* Qo = p.Q + (size_t)by * ((size_t)N * N) + line0;
     if constexpr (!DO_Y) {
         // C: in-place Hermitian split, then copy out (slot-major rows are contiguous in HBM)
         r2c_split<N, N>(ctx, s, PITCH, 1, NL, tw);
