@@ -35,9 +35,11 @@ UNIT = "ms/grid"
 YARD_FWD_BWD_V = 52.0
 KERNEL_BYTES_V = {
     # forward
-    "F:k_zero": (0.0, 0.0, 4.0),                    # zero fill of v (3V) + W (1V): part of "splat 3V"
-    "F:k_splat": (3.0, 3.0, 0.0),                   # row "splat (write every cell once)"
-    "F:k_zy_fwd": (12.0, 6.0, 6.0),                 # rows z r2c x3 (6V) [+ y x3 (6V) when fused]
+    "F:k_bin_count": (0.0, 0.0, 0.0),               # counting sort of the points (bytes ~ 72 B/point, ignored)
+    "F:k_bin_scan": (0.0, 0.0, 0.0),
+    "F:k_bin_scatter": (0.0, 0.0, 0.0),
+    # splat fused in: rows "splat" (3V) + z r2c x3 (6V) [+ y x3 (6V) when fused]; it only WRITES 3V itself
+    "F:k_zy_fwd": (15.0, 9.0, 3.0),
     "F:k_strided<FWD,y>": (0.0, 6.0, 6.0),          # row y sweep x3
     "F:k_strided<SOLVE>": (4.0, 4.0, 4.0),          # row x sweep + solve + x inverse (3V in, 1V out)
     "F:k_strided<INV,y>": (0.0, 2.0, 2.0),          # row inverse y
@@ -46,7 +48,7 @@ KERNEL_BYTES_V = {
     "F:k_scale_shift": (2.0, 2.0, 2.0),             # row normalise
     # backward
     "B:k_reduce_g": (2.0, 2.0, 2.0),                # row reductions
-    "B:k_zy_fwd<GBAR>": (5.0, 3.0, 3.0),            # rows z r2c (G+W in, 1 out = 3V) [+ y (2V)]
+    "B:k_zy_fwd<GBAR>": (5.0, 3.0, 2.0),            # rows z r2c (G+W in, 1 out = 3V) [+ y (2V)]; W is re-rasterised, not read
     "B:k_strided<FWD,y>": (0.0, 2.0, 2.0),
     "B:k_strided<ADJ>": (4.0, 4.0, 4.0),            # row x sweep + conj(M) fan-out + 3 x inverse
     "B:k_strided<INV,y>": (0.0, 6.0, 6.0),

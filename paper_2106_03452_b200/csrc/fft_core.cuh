@@ -30,8 +30,8 @@ template <int N> struct Plan;
 template <> struct Plan<16>  { static constexpr int NS = 1, R0 = 16, R1 = 1,  R2 = 1; };
 template <> struct Plan<32>  { static constexpr int NS = 2, R0 = 8,  R1 = 4,  R2 = 1; };
 template <> struct Plan<64>  { static constexpr int NS = 2, R0 = 8,  R1 = 8,  R2 = 1; };
-template <> struct Plan<128> { static constexpr int NS = 2, R0 = 8,  R1 = 16, R2 = 1; };
-template <> struct Plan<256> { static constexpr int NS = 2, R0 = 16, R1 = 16, R2 = 1; };
+template <> struct Plan<128> { static constexpr int NS = 2, R0 = 16, R1 = 8,  R2 = 1; };
+template <> struct Plan<256> { static constexpr int NS = 2, R0 = 32, R1 = 8,  R2 = 1; };
 template <> struct Plan<512> { static constexpr int NS = 3, R0 = 8,  R1 = 8,  R2 = 8; };
 
 template <int N, int S> struct StageInfo {
@@ -84,6 +84,19 @@ template <> SAP_HD float2 unit_root<16>(int k) {
         case 6: return make_float2(-0.70710678118654752f, -0.70710678118654752f);
         default: return make_float2(-0.92387953251128674f, -0.38268343236508977f);
     }
+}
+
+template <> SAP_HD float2 unit_root<32>(int k) {
+    // exp(-2 pi i k / 32), k = 0..15
+    const float c[16] = {1.f, 0.98078528040323043f, 0.92387953251128674f, 0.83146961230254524f, 0.70710678118654752f,
+                         0.55557023301960218f, 0.38268343236508977f, 0.19509032201612825f, 0.f, -0.19509032201612825f,
+                         -0.38268343236508977f, -0.55557023301960218f, -0.70710678118654752f, -0.83146961230254524f,
+                         -0.92387953251128674f, -0.98078528040323043f};
+    const float sn[16] = {0.f, 0.19509032201612825f, 0.38268343236508977f, 0.55557023301960218f, 0.70710678118654752f,
+                          0.83146961230254524f, 0.92387953251128674f, 0.98078528040323043f, 1.f, 0.98078528040323043f,
+                          0.92387953251128674f, 0.83146961230254524f, 0.70710678118654752f, 0.55557023301960218f,
+                          0.38268343236508977f, 0.19509032201612825f};
+    return make_float2(c[k], -sn[k]);
 }
 
 template <int R> SAP_HD void dft_fwd(float2 (&v)[R]) {

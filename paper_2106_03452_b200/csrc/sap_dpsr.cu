@@ -11,46 +11,13 @@
 
 #include "../../include/sap_dpsr.h"
 #include "dpsr_kernels.cuh"
-#include "strided_async.cuh"
 
 namespace sap {
-
-__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 
 struct DevCtx {
     int tid, nthr;
     __device__ __forceinline__ void sync() const { __syncthreads(); }
     __device__ __forceinline__ void atomic_add(float* p, float v) const { atomicAdd(p, v); }
-    // ---- asynchronous-copy pipeline primitives (mbarrier + cp.async.bulk, sm_90+/sm_100a)
-    __device__ __forceinline__ void bar_init(unsigned long long* bar) const {
-        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(bar)) : "memory");
-    }
-    __device__ __forceinline__ void fence_init() const {
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    }
-    __device__ __forceinline__ void fence_async() const { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-    __device__ __forceinline__ void bar_expect(unsigned long long* bar, unsigned bytes) const {
-        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-    }
-    __device__ __forceinline__ void bulk_row(float2* dst, const float2* src, unsigned bytes, unsigned long long* bar) const {
-        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
-                     "l"(src), "r"(bytes), "r"(smem_u32(bar))
-                     : "memory");
-    }
-    __device__ __forceinline__ void bar_wait(unsigned long long* bar, unsigned parity) const {
-        const unsigned a = smem_u32(bar);
-        for (unsigned it = 0; it < (1u << 24); ++it) {
-            unsigned ok;
-            asm volatile(
-                "{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
-                : "=r"(ok)
-                : "r"(a), "r"(parity)
-                : "memory");
-            if (ok) return;
-        }
-        __trap();  // a copy never landed: fail loudly instead of hanging the GPU
-    }
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -73,13 +40,6 @@ __global__ void __launch_bounds__(NT) k_strided(StridedParams p) {
     extern __shared__ float2 smem[];
     DevCtx ctx{(int)threadIdx.x, NT};
     strided_body<N, MODE, NT, W>(ctx, p, smem, (int)blockIdx.x, (int)blockIdx.y);
-}
-
-template <int N, int MODE, int NT, int W, int NB>
-__global__ void __launch_bounds__(NT) k_strided_async(StridedParams p, int nby) {
-    extern __shared__ __align__(128) float2 smem[];
-    DevCtx ctx{(int)threadIdx.x, NT};
-    strided_async_body<N, MODE, NT, W, NB>(ctx, p, smem, (int)blockIdx.x, (int)gridDim.x, nby);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -343,6 +303,7 @@ struct sap_dpsr {
     float2* S1 = nullptr;      // [B][N*N*H]   1-channel spectrum
     float2* Q1 = nullptr;      // [B][N*N]
     float2* tw = nullptr;      // [N]
+    float4* ftab = nullptr;    // [N + N/2 + 1] per-slot frequency table of the spectral multiplier
     double* acc = nullptr;     // [B][3] reduction accumulators (mean | S0,S1)
     unsigned* ticket = nullptr;  // [B][2]
     float* stats = nullptr;    // [B][4] {mu, a, s, -}
@@ -408,9 +369,8 @@ template <int N> struct Cfg {
     static constexpr int NL = FUSED_ZY ? N : 32;
     static constexpr int NT_ZY = 256;
     // strided tiles: columns per tile (W) and threads, for the plain y pass (Y) and the fused x pass (X)
-    static constexpr bool ASYNC_X = false, ASYNC_Y = false;
-    static constexpr int WY = 16, NTY = 256, NBY = 3;
-    static constexpr int WX = (N >= 64) ? 32 : 16, NTX = (N >= 256) ? 512 : 256, NBX = (N >= 256) ? 2 : 4;
+    static constexpr int WY = 16, NTY = 256;
+    static constexpr int WX = (N >= 64) ? 32 : 16, NTX = (N >= 256) ? 512 : 256;
 };
 
 template <int N> struct Runner {
@@ -419,6 +379,13 @@ template <int N> struct Runner {
 
     static sap_status_t prepare(sap_dpsr* h) {
         cudaError_t e = cudaSuccess;
+        {   // frequency table of the multiplier, in stored-slot order
+            float4 tab[N + H + 1];
+            const float cg = 2.f * h->sigma * h->sigma / ((float)N * (float)N);
+            for (int i = 0; i < N; ++i) tab[i] = freq_entry_n<N>(i, cg);
+            for (int i = 0; i <= H; ++i) tab[N + i] = freq_entry_z<N>(i, cg);
+            e = cudaMemcpy(h->ftab, tab, sizeof(tab), cudaMemcpyHostToDevice);
+        }
         auto upd = [&](cudaError_t x) { if (e == cudaSuccess) e = x; };
         upd(set_smem(k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_SPLAT, C::NT_ZY>, zy_smem_bytes<N, C::NL>()));
         upd(set_smem(k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_GBAR, C::NT_ZY>, zy_smem_bytes<N, C::NL>()));
@@ -427,41 +394,21 @@ template <int N> struct Runner {
         upd(set_smem(k_strided<N, MODE_ADJ, C::NTX, C::WX>, strided_smem_bytes<N, C::WX>()));
         upd(set_smem(k_strided<N, MODE_FWD, C::NTY, C::WY>, strided_smem_bytes<N, C::WY>()));
         upd(set_smem(k_strided<N, MODE_INV, C::NTY, C::WY>, strided_smem_bytes<N, C::WY>()));
-        if constexpr (C::ASYNC_X) {
-        upd(set_smem(k_strided_async<N, MODE_SOLVE, C::NTX, C::WX, C::NBX>, strided_async_smem_bytes<N, MODE_SOLVE, C::WX, C::NBX>()));
-        upd(set_smem(k_strided_async<N, MODE_ADJ, C::NTX, C::WX, C::NBX>, strided_async_smem_bytes<N, MODE_ADJ, C::WX, C::NBX>()));
-        }
-        if constexpr (C::ASYNC_Y) {
-        upd(set_smem(k_strided_async<N, MODE_FWD, C::NTY, C::WY, C::NBY>, strided_async_smem_bytes<N, MODE_FWD, C::WY, C::NBY>()));
-        upd(set_smem(k_strided_async<N, MODE_INV, C::NTY, C::WY, C::NBY>, strided_async_smem_bytes<N, MODE_INV, C::WY, C::NBY>()));
-        }
         return cuda_ok(h, e, "cudaFuncSetAttribute") ? SAP_OK : SAP_ERR_CUDA;
     }
 
     static StridedParams sp(sap_dpsr* h, const float2* inS, const float2* inQ, float2* outS, float2* outQ, int axis) {
         StridedParams p;
-        p.inS = inS; p.inQ = inQ; p.outS = outS; p.outQ = outQ; p.tw = h->tw; p.axis = axis;
+        p.inS = inS; p.inQ = inQ; p.outS = outS; p.outQ = outQ; p.tw = h->tw; p.ftab = h->ftab; p.axis = axis;
         p.cg = 2.f * h->sigma * h->sigma / ((float)N * (float)N);
         p.cs = (float)((2.0 / ((double)N * N * N)) / (-2.0 * 3.14159265358979323846));
         return p;
     }
 
-    // persistent launch: as many CTAs as fit the chip at once (or fewer if there is less work)
-    template <int MODE, int NT, int W, int NB>
+    template <int MODE, int NT, int W>
     static void launch_strided(sap_dpsr* h, cudaStream_t st, int planes, const StridedParams& p) {
-        constexpr bool ASYNC = (MODE == MODE_SOLVE || MODE == MODE_ADJ) ? C::ASYNC_X : C::ASYNC_Y;
-        if constexpr (!ASYNC) {
-            k_strided<N, MODE, NT, W><<<dim3(strided_tiles<N, W>(), planes), NT, strided_smem_bytes<N, W>(), st>>>(p);
-        } else {
-            constexpr size_t smem = strided_async_smem_bytes<N, MODE, W, NB>();
-            int per_sm = (int)((227 * 1024) / (smem + 1024));
-            if (per_sm > 2048 / NT) per_sm = 2048 / NT;
-            if (per_sm < 1) per_sm = 1;
-            long long work = (long long)strided_tiles<N, W>() * planes;
-            long long grid = (long long)h->num_sms * per_sm;
-            if (grid > work) grid = work;
-    k_strided_async<N, MODE, NT, W, NB><<<(unsigned)grid, NT, smem, st>>>(p, planes);
-        }
+        (void)h;
+        k_strided<N, MODE, NT, W><<<dim3(strided_tiles<N, W>(), planes), NT, strided_smem_bytes<N, W>(), st>>>(p);
     }
 
     static sap_status_t forward(sap_dpsr* h, const float* pts, const float* nrm, int P, float* chi, cudaStream_t st) {
@@ -487,16 +434,16 @@ template <int N> struct Runner {
             SAP_LAUNCH_CHECK(h, "k_zy_fwd");
         }
         if (!C::FUSED_ZY) {
-            launch_strided<MODE_FWD, C::NTY, C::WY, C::NBY>(h, st, B * 3,
+            launch_strided<MODE_FWD, C::NTY, C::WY>(h, st, B * 3,
                 sp(h, h->S3, h->Q3, h->S3, h->Q3, 1));
             SAP_LAUNCH_CHECK(h, "k_strided<FWD,y>");
         }
         // F2x + F3 + F4x: x forward, spectral solve, x inverse (3 -> 1)
-        launch_strided<MODE_SOLVE, C::NTX, C::WX, C::NBX>(h, st, B,
+        launch_strided<MODE_SOLVE, C::NTX, C::WX>(h, st, B,
                 sp(h, h->S3, h->Q3, h->S1, h->Q1, 0));
         SAP_LAUNCH_CHECK(h, "k_strided<SOLVE>");
         if (!C::FUSED_ZY) {
-            launch_strided<MODE_INV, C::NTY, C::WY, C::NBY>(h, st, B,
+            launch_strided<MODE_INV, C::NTY, C::WY>(h, st, B,
                 sp(h, h->S1, h->Q1, h->S1, h->Q1, 1));
             SAP_LAUNCH_CHECK(h, "k_strided<INV,y>");
         }
@@ -541,16 +488,16 @@ template <int N> struct Runner {
             SAP_LAUNCH_CHECK(h, "k_zy_fwd<GBAR>");
         }
         if (!C::FUSED_ZY) {
-            launch_strided<MODE_FWD, C::NTY, C::WY, C::NBY>(h, st, B,
+            launch_strided<MODE_FWD, C::NTY, C::WY>(h, st, B,
                 sp(h, h->S1, h->Q1, h->S1, h->Q1, 1));
             SAP_LAUNCH_CHECK(h, "k_strided<FWD,y>");
         }
         // B3x + B4 + B5x: x forward, transposed multiplier, 3 x inverse
-        launch_strided<MODE_ADJ, C::NTX, C::WX, C::NBX>(h, st, B,
+        launch_strided<MODE_ADJ, C::NTX, C::WX>(h, st, B,
                 sp(h, h->S1, h->Q1, h->S3, h->Q3, 0));
         SAP_LAUNCH_CHECK(h, "k_strided<ADJ>");
         if (!C::FUSED_ZY) {
-            launch_strided<MODE_INV, C::NTY, C::WY, C::NBY>(h, st, B * 3,
+            launch_strided<MODE_INV, C::NTY, C::WY>(h, st, B * 3,
                 sp(h, h->S3, h->Q3, h->S3, h->Q3, 1));
             SAP_LAUNCH_CHECK(h, "k_strided<INV,y>");
         }
@@ -590,7 +537,7 @@ static bool supported_N(int N) { return N == 32 || N == 64 || N == 128 || N == 2
 
 static void free_all(sap_dpsr* h) {
     for (int i = 0; i < sap_dpsr::MAX_EV; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
-    cudaFree(h->v); cudaFree(h->spts); cudaFree(h->snrm); cudaFree(h->bin_cnt); cudaFree(h->bin_cursor); cudaFree(h->bin_start); cudaFree(h->S3); cudaFree(h->Q3); cudaFree(h->S1); cudaFree(h->Q1); cudaFree(h->tw);
+    cudaFree(h->v); cudaFree(h->spts); cudaFree(h->snrm); cudaFree(h->bin_cnt); cudaFree(h->bin_cursor); cudaFree(h->bin_start); cudaFree(h->S3); cudaFree(h->Q3); cudaFree(h->S1); cudaFree(h->Q1); cudaFree(h->tw); cudaFree(h->ftab);
     cudaFree(h->acc); cudaFree(h->ticket); cudaFree(h->stats); cudaFree(h->bw);
     cudaFree(h->h_pts); cudaFree(h->h_nrm); cudaFree(h->h_chi); cudaFree(h->h_gchi); cudaFree(h->h_gp); cudaFree(h->h_gn);
 }
@@ -626,6 +573,7 @@ extern "C" sap_status_t sap_dpsr_create(int N, float sigma, int batch, int max_p
     upd(dev_alloc(h, &h->S1, B * SP));
     upd(dev_alloc(h, &h->Q1, B * QP));
     upd(dev_alloc(h, &h->tw, (size_t)N));
+    upd(dev_alloc(h, &h->ftab, (size_t)(N + N / 2 + 1)));
     upd(dev_alloc(h, &h->acc, B * 3));
     upd(dev_alloc(h, &h->ticket, B * 2));
     upd(dev_alloc(h, &h->stats, B * 4));

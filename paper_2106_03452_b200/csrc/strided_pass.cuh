@@ -20,12 +20,29 @@ namespace sap {
 //   M_c(k) = i m_c,  m_c = f uh_c,  f = cs exp(-cg q) / q,  q = |u|^2,  cg = 2 sigma^2 / N^2,
 //   cs = (2 / N^3) / (-2 pi): folds the inverse-transform scale (R8) and the factor 2 of the half-length
 //   c2r trick into the multiplier.
+// Per-slot table (built once in sap_dpsr_create, float4 {uh, u^2, exp(-cg u^2), 0}): entries [0, N) for the
+// slots of a length-N axis (x, y), entries [N, N + H] for the z slots (slot H = the Nyquist plane).
 template <int N> SAP_HD int signed_freq(int k) { return (k < N / 2) ? k : k - N; }
-template <int N> SAP_HD float mult_f(int ux, int uy, int uz, float cg, float cs) {
-    const int qi = ux * ux + uy * uy + uz * uz;
-    if (qi == 0) return 0.f;
-    const float q = (float)qi;
-    return cs * expf(-cg * q) / q;
+template <int N> SAP_HD float4 freq_entry_n(int slot, float cg) {
+    const int k = pos2freq<N>(slot), u = signed_freq<N>(k);
+    return make_float4((k == N / 2) ? 0.f : (float)u, (float)(u * u), expf(-cg * (float)(u * u)), 0.f);
+}
+template <int N> SAP_HD float4 freq_entry_z(int slot, float cg) {
+    constexpr int H = N / 2;
+    const int k = (slot == H) ? H : pos2freq<H>(slot);
+    return make_float4((k == H) ? 0.f : (float)k, (float)(k * k), expf(-cg * (float)(k * k)), 0.f);
+}
+SAP_HD float fast_rcp(float x) {
+#ifdef __CUDA_ARCH__
+    return __frcp_rn(x);
+#else
+    return 1.f / x;
+#endif
+}
+// f = cs g / q from three table entries (0 at DC)
+SAP_HD float mult_f(const float4& ex, const float4& ey, const float4& ez, float cs) {
+    const float q = ex.y + ey.y + ez.y;
+    return (q == 0.f) ? 0.f : cs * (ex.z * ey.z) * ez.z * fast_rcp(q);
 }
 
 enum { MODE_FWD = 0, MODE_INV = 1, MODE_SOLVE = 2, MODE_ADJ = 3 };
@@ -36,6 +53,7 @@ struct StridedParams {
     float2* outS;
     float2* outQ;
     const float2* tw;
+    const float4* ftab;  // [N + H + 1] frequency table (see freq_entry_*)
     int axis;     // 0: along x (stride N*H / N), 1: along y (stride H / 1)
     float cg;     // 2 sigma^2 / N^2
     float cs;     // (2 / N^3) / (-2 pi)
@@ -44,7 +62,7 @@ struct StridedParams {
 template <int N, int W> constexpr int strided_tiles() { return N * (N / 2 / W) + N / W; }
 // one tile buffer for every mode: SOLVE streams its 3 input channels through it (the divergence is
 // accumulated in registers), ADJ streams its 3 output channels
-template <int N, int W> constexpr size_t strided_smem_bytes() { return ((size_t)N * (W + 1) + N) * sizeof(float2); }
+template <int N, int W> constexpr size_t strided_smem_bytes() { return ((size_t)N * (W + 1) + N) * sizeof(float2) + (size_t)N * sizeof(float4); }
 
 struct TileDesc {
     size_t base;   // element offset inside one channel array
@@ -128,7 +146,10 @@ SAP_HD void strided_body(Ctx& ctx, const StridedParams& p, float2* smem, int bx,
     constexpr int OUT_CH = (MODE == MODE_ADJ) ? 3 : 1;
     float2* s = smem;
     float2* tw = smem + N * TILE_PITCH;
+    float4* fx = reinterpret_cast<float4*>(tw + N);  // x-axis frequency entries (SOLVE / ADJ)
     for (int i = ctx.tid; i < N; i += NT) tw[i] = p.tw[i];
+    if constexpr (MODE == MODE_SOLVE || MODE == MODE_ADJ)
+        for (int i = ctx.tid; i < N; i += NT) fx[i] = p.ftab[i];
     ctx.sync();
     const TileDesc d = tile_desc<N, W>(p.axis, bx);
     auto in_plane = [&](int c) {
@@ -140,11 +161,9 @@ SAP_HD void strided_body(Ctx& ctx, const StridedParams& p, float2* smem, int bx,
         return d.nyq ? p.outQ + plane * QPLANE : p.outS + plane * SPLANE;
     };
     // frequency helpers for the stride-1 stage (SOLVE / ADJ)
-    auto col_freq = [&](int c, int& uy, int& uz, float& hy, float& hz) {
-        const int ky = pos2freq<N>(d.nyq ? d.other + c : d.other);
-        const int kz = d.nyq ? H : pos2freq<H>(d.pz0 + c);
-        uy = signed_freq<N>(ky); uz = signed_freq<N>(kz);
-        hy = (ky == H) ? 0.f : (float)uy; hz = (kz == H) ? 0.f : (float)uz;
+    auto col_freq = [&](int c, float4& ey, float4& ez) {
+        ey = p.ftab[d.nyq ? d.other + c : d.other];
+        ez = p.ftab[N + (d.nyq ? H : d.pz0 + c)];
     };
 
     float2 acc[TPT][RL];  // SOLVE: divergence accumulators; ADJ: -i f Gbar'~ ; FWD/INV: unused
@@ -177,14 +196,14 @@ SAP_HD void strided_body(Ctx& ctx, const StridedParams& p, float2* smem, int bx,
                         for (int r = 0; r < RL; ++r)
                             g[d.base + (size_t)(blk * RL + r) * d.sn + (size_t)c * d.sc] = v[r];
                     } else {
-                        int uy, uz; float hy, hz;
-                        col_freq(c, uy, uz, hy, hz);
+                        float4 ey, ez;
+                        col_freq(c, ey, ez);
+                        const float hy = ey.x, hz = ez.x;
                         if (MODE == MODE_ADJ || ch == 2) {
                             // finish: multiply by f = cs g / q (and by i or -i)
 #pragma unroll
                             for (int r = 0; r < RL; ++r) {
-                                const int ux = signed_freq<N>(pos2freq<N>(blk * RL + r));
-                                const float f = mult_f<N>(ux, uy, uz, p.cg, p.cs);
+                                const float f = mult_f(fx[blk * RL + r], ey, ez, p.cs);
                                 if constexpr (MODE == MODE_SOLVE) {
                                     const float dr = f * (acc[i][r].x + hz * v[r].x), di = f * (acc[i][r].y + hz * v[r].y);
                                     acc[i][r] = make_float2(-di, dr);  // chi~ = i (dr + i di)
@@ -195,8 +214,7 @@ SAP_HD void strided_body(Ctx& ctx, const StridedParams& p, float2* smem, int bx,
                         } else if (ch == 0) {
 #pragma unroll
                             for (int r = 0; r < RL; ++r) {
-                                const int kx = pos2freq<N>(blk * RL + r);
-                                const float hx = (kx == H) ? 0.f : (float)signed_freq<N>(kx);
+                                const float hx = fx[blk * RL + r].x;
                                 acc[i][r] = make_float2(hx * v[r].x, hx * v[r].y);
                             }
                         } else {
@@ -229,15 +247,11 @@ SAP_HD void strided_body(Ctx& ctx, const StridedParams& p, float2* smem, int bx,
 #pragma unroll
                         for (int r = 0; r < RL; ++r) v[r] = acc[i][r];
                     } else {
-                        int uy, uz; float hy, hz;
-                        col_freq(c, uy, uz, hy, hz);
+                        float4 ey, ez;
+                        col_freq(c, ey, ez);
 #pragma unroll
                         for (int r = 0; r < RL; ++r) {
-                            float h;
-                            if (ch == 0) {
-                                const int kx = pos2freq<N>(blk * RL + r);
-                                h = (kx == H) ? 0.f : (float)signed_freq<N>(kx);
-                            } else h = (ch == 1) ? hy : hz;
+                            const float h = (ch == 0) ? fx[blk * RL + r].x : (ch == 1) ? ey.x : ez.x;
                             v[r] = make_float2(h * acc[i][r].x, h * acc[i][r].y);
                         }
                     }
