@@ -12,4 +12,4 @@
 #pragma once
 #include "fft_core.cuh"
 #include "zy_pass.cuh"
-#include "strided_pass.cuh"
+#include "spectral.cuh"

@@ -17,11 +17,32 @@
 
 namespace sap {
 
+// Complex arithmetic on float2 = (re, im).  On sm_100a these map to the packed FP32x2 instructions
+// (FADD2 / FMUL2 / FFMA2): one issue slot per complex add, two per complex multiply.  The operand
+// modifiers of those instructions (half swap, per-half negate, scalar broadcast) absorb mul_mi and conj.
+#ifdef __CUDA_ARCH__
+SAP_HD float2 cadd(float2 a, float2 b) { return __fadd2_rn(a, b); }
+SAP_HD float2 csub(float2 a, float2 b) { return __fadd2_rn(a, make_float2(-b.x, -b.y)); }
+SAP_HD float2 cmul(float2 a, float2 w) {
+    return __ffma2_rn(make_float2(a.y, a.y), make_float2(-w.y, w.x), __fmul2_rn(make_float2(a.x, a.x), w));
+}
+// a * conj(w)
+SAP_HD float2 cmulc(float2 a, float2 w) {
+    return __ffma2_rn(make_float2(a.y, a.y), make_float2(w.y, w.x), __fmul2_rn(make_float2(a.x, a.x), make_float2(w.x, -w.y)));
+}
+// s * a (real scale)
+SAP_HD float2 cscale(float s, float2 a) { return __fmul2_rn(make_float2(s, s), a); }
+// c + s * a
+SAP_HD float2 caxpy(float s, float2 a, float2 c) { return __ffma2_rn(make_float2(s, s), a, c); }
+#else
 SAP_HD float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
 SAP_HD float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
 SAP_HD float2 cmul(float2 a, float2 w) { return make_float2(a.x * w.x - a.y * w.y, a.x * w.y + a.y * w.x); }
 // a * conj(w)
 SAP_HD float2 cmulc(float2 a, float2 w) { return make_float2(a.x * w.x + a.y * w.y, a.y * w.x - a.x * w.y); }
+SAP_HD float2 cscale(float s, float2 a) { return make_float2(s * a.x, s * a.y); }
+SAP_HD float2 caxpy(float s, float2 a, float2 c) { return make_float2(c.x + s * a.x, c.y + s * a.y); }
+#endif
 // a * (-i)
 SAP_HD float2 mul_mi(float2 a) { return make_float2(a.y, -a.x); }
 
@@ -31,7 +52,7 @@ template <> struct Plan<16>  { static constexpr int NS = 1, R0 = 16, R1 = 1,  R2
 template <> struct Plan<32>  { static constexpr int NS = 2, R0 = 8,  R1 = 4,  R2 = 1; };
 template <> struct Plan<64>  { static constexpr int NS = 2, R0 = 8,  R1 = 8,  R2 = 1; };
 template <> struct Plan<128> { static constexpr int NS = 2, R0 = 16, R1 = 8,  R2 = 1; };
-template <> struct Plan<256> { static constexpr int NS = 2, R0 = 32, R1 = 8,  R2 = 1; };
+template <> struct Plan<256> { static constexpr int NS = 2, R0 = 16, R1 = 16, R2 = 1; };
 template <> struct Plan<512> { static constexpr int NS = 3, R0 = 8,  R1 = 8,  R2 = 8; };
 
 template <int N, int S> struct StageInfo {
@@ -99,7 +120,11 @@ template <> SAP_HD float2 unit_root<32>(int k) {
     return make_float2(c[k], -sn[k]);
 }
 
-template <int R> SAP_HD void dft_fwd(float2 (&v)[R]) {
+// Forward (INV = false, kernel exp(-2 pi i jk/R)) or unnormalised inverse (INV = true, exp(+...)) DFT of R
+// values, natural order in and out.  The two differ only in the sign of i and the conjugated roots.
+// a * (+i)
+SAP_HD float2 mul_pi(float2 a) { return make_float2(-a.y, a.x); }
+template <int R, bool INV> SAP_HD void dft_dir(float2 (&v)[R]) {
     if constexpr (R == 1) {
     } else if constexpr (R == 2) {
         float2 a = v[0], b = v[1];
@@ -107,7 +132,8 @@ template <int R> SAP_HD void dft_fwd(float2 (&v)[R]) {
         v[1] = csub(a, b);
     } else if constexpr (R == 4) {
         float2 t0 = cadd(v[0], v[2]), t1 = csub(v[0], v[2]);
-        float2 t2 = cadd(v[1], v[3]), t3 = mul_mi(csub(v[1], v[3]));
+        float2 t2 = cadd(v[1], v[3]), d = csub(v[1], v[3]);
+        float2 t3 = INV ? mul_pi(d) : mul_mi(d);
         v[0] = cadd(t0, t2);
         v[2] = csub(t0, t2);
         v[1] = cadd(t1, t3);
@@ -116,27 +142,21 @@ template <int R> SAP_HD void dft_fwd(float2 (&v)[R]) {
         float2 e[R / 2], o[R / 2];
 #pragma unroll
         for (int i = 0; i < R / 2; ++i) { e[i] = v[2 * i]; o[i] = v[2 * i + 1]; }
-        dft_fwd<R / 2>(e);
-        dft_fwd<R / 2>(o);
+        dft_dir<R / 2, INV>(e);
+        dft_dir<R / 2, INV>(o);
 #pragma unroll
         for (int k = 0; k < R / 2; ++k) {
             float2 t;
             if (k == 0) t = o[k];
-            else if (k == R / 4) t = mul_mi(o[k]);
-            else t = cmul(o[k], unit_root<R>(k));
+            else if (k == R / 4) t = INV ? mul_pi(o[k]) : mul_mi(o[k]);
+            else t = INV ? cmulc(o[k], unit_root<R>(k)) : cmul(o[k], unit_root<R>(k));
             v[k] = cadd(e[k], t);
             v[k + R / 2] = csub(e[k], t);
         }
     }
 }
-// inverse (unnormalised) DFT: swap re/im, forward, swap back
-template <int R> SAP_HD void dft_inv(float2 (&v)[R]) {
-#pragma unroll
-    for (int i = 0; i < R; ++i) { float t = v[i].x; v[i].x = v[i].y; v[i].y = t; }
-    dft_fwd<R>(v);
-#pragma unroll
-    for (int i = 0; i < R; ++i) { float t = v[i].x; v[i].x = v[i].y; v[i].y = t; }
-}
+template <int R> SAP_HD void dft_fwd(float2 (&v)[R]) { dft_dir<R, false>(v); }
+template <int R> SAP_HD void dft_inv(float2 (&v)[R]) { dft_dir<R, true>(v); }
 
 // ---- register-level stage butterflies --------------------------------------------------------------
 // Stage S of the length-N plan on R values held in registers.  j is the butterfly's index inside its

@@ -11,6 +11,7 @@
 
 #include "../../include/sap_dpsr.h"
 #include "dpsr_kernels.cuh"
+#include "ring_pass.cuh"
 
 namespace sap {
 
@@ -23,23 +24,19 @@ struct DevCtx {
 // ------------------------------------------------------------------------------------------------
 // __global__ wrappers around the block bodies
 // ------------------------------------------------------------------------------------------------
+// minimum resident CTAs per SM the register allocation must allow (a register cliff halves occupancy)
+template <int N> constexpr int zy_min_blocks() { return N == 128 ? 2 : N == 512 ? 3 : 4; }
 template <int N, int NL, bool DO_Y, int SRC, int NT>
-__global__ void __launch_bounds__(NT) k_zy_fwd(ZyFwdParams p) {
+__global__ void __launch_bounds__(NT, zy_min_blocks<N>()) k_zy_fwd(ZyFwdParams p) {
     extern __shared__ float2 smem[];
     DevCtx ctx{(int)threadIdx.x, NT};
     zy_fwd_body<N, NL, DO_Y, SRC>(ctx, p, smem, (int)blockIdx.x, (int)blockIdx.y);
 }
 template <int N, int NL, bool DO_Y, int NT>
-__global__ void __launch_bounds__(NT) k_zy_inv(ZyInvParams p) {
+__global__ void __launch_bounds__(NT, zy_min_blocks<N>()) k_zy_inv(ZyInvParams p) {
     extern __shared__ float2 smem[];
     DevCtx ctx{(int)threadIdx.x, NT};
     zy_inv_body<N, NL, DO_Y>(ctx, p, smem, (int)blockIdx.x, (int)blockIdx.y);
-}
-template <int N, int MODE, int NT, int W>
-__global__ void __launch_bounds__(NT) k_strided(StridedParams p) {
-    extern __shared__ float2 smem[];
-    DevCtx ctx{(int)threadIdx.x, NT};
-    strided_body<N, MODE, NT, W>(ctx, p, smem, (int)blockIdx.x, (int)blockIdx.y);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -304,6 +301,10 @@ struct sap_dpsr {
     float2* Q1 = nullptr;      // [B][N*N]
     float2* tw = nullptr;      // [N]
     float4* ftab = nullptr;    // [N + N/2 + 1] per-slot frequency table of the spectral multiplier
+    // TMA descriptors of the spectra (ring_pass.cuh): main arrays with the x-pass / y-pass tile box, Nyquist planes
+    CUtensorMap mS3x, mS3y, mS1x, mS1y, mQ3, mQ1, mQT3, mQT1;
+    float2* QT3 = nullptr;     // [B*3][N*N] transposed Nyquist planes (N >= 256: staging between the z/x passes and the y pass)
+    float2* QT1 = nullptr;     // [B][N*N]
     double* acc = nullptr;     // [B][3] reduction accumulators (mean | S0,S1)
     unsigned* ticket = nullptr;  // [B][2]
     float* stats = nullptr;    // [B][4] {mu, a, s, -}
@@ -363,14 +364,44 @@ template <class K> static cudaError_t set_smem(K kernel, size_t bytes) {
     return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
 }
 
+// ---- TMA descriptors -------------------------------------------------------------------------------
+// cuTensorMapEncodeTiled is reached through the runtime's driver entry point (no link against libcuda).
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static EncodeTiledFn encode_tiled_fn(sap_dpsr* h) {
+    static EncodeTiledFn fn = nullptr;
+    if (fn) return fn;
+    void* ptr = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (!cuda_ok(h, cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &q), "cudaGetDriverEntryPoint")) return nullptr;
+    if (q != cudaDriverEntryPointSuccess || !ptr) { h->err = "cuTensorMapEncodeTiled not available in this driver"; return nullptr; }
+    fn = (EncodeTiledFn)ptr;
+    return fn;
+}
+// float view of a complex array: dims[0] counts floats (2 per complex), strides in bytes for dims 1..rank-1
+static bool make_map(sap_dpsr* h, CUtensorMap* m, void* base, int rank, const cuuint64_t* dims, const cuuint64_t* strides,
+                     const cuuint32_t* box) {
+    EncodeTiledFn fn = encode_tiled_fn(h);
+    if (!fn) return false;
+    const cuuint32_t es[4] = {1, 1, 1, 1};
+    const CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, (cuuint32_t)rank, base, dims, strides, box, es,
+                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        char buf[128];
+        snprintf(buf, sizeof buf, "cuTensorMapEncodeTiled failed (CUresult %d)", (int)r);
+        h->err = buf;
+        return false;
+    }
+    return true;
+}
+
 // threads per block of the FFT kernels
 template <int N> struct Cfg {
     static constexpr bool FUSED_ZY = (N <= 128);  // a whole (y,z) plane fits one CTA's shared memory
     static constexpr int NL = FUSED_ZY ? N : 32;
     static constexpr int NT_ZY = 256;
-    // strided tiles: columns per tile (W) and threads, for the plain y pass (Y) and the fused x pass (X)
-    static constexpr int WY = 16, NTY = 256;
-    static constexpr int WX = (N >= 64) ? 32 : 16, NTX = (N >= 256) ? 512 : 256;
 };
 
 template <int N> struct Runner {
@@ -390,25 +421,41 @@ template <int N> struct Runner {
         upd(set_smem(k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_SPLAT, C::NT_ZY>, zy_smem_bytes<N, C::NL>()));
         upd(set_smem(k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_GBAR, C::NT_ZY>, zy_smem_bytes<N, C::NL>()));
         upd(set_smem(k_zy_inv<N, C::NL, C::FUSED_ZY, C::NT_ZY>, zy_smem_bytes<N, C::NL>()));
-        upd(set_smem(k_strided<N, MODE_SOLVE, C::NTX, C::WX>, strided_smem_bytes<N, C::WX>()));
-        upd(set_smem(k_strided<N, MODE_ADJ, C::NTX, C::WX>, strided_smem_bytes<N, C::WX>()));
-        upd(set_smem(k_strided<N, MODE_FWD, C::NTY, C::WY>, strided_smem_bytes<N, C::WY>()));
-        upd(set_smem(k_strided<N, MODE_INV, C::NTY, C::WY>, strided_smem_bytes<N, C::WY>()));
-        return cuda_ok(h, e, "cudaFuncSetAttribute") ? SAP_OK : SAP_ERR_CUDA;
+        upd(set_smem(k_ring<N, MODE_SOLVE>, ring_smem_bytes<N>()));
+        upd(set_smem(k_ring<N, MODE_ADJ>, ring_smem_bytes<N>()));
+        upd(set_smem(k_ring<N, MODE_FWD>, ring_smem_bytes<N>()));
+        upd(set_smem(k_ring<N, MODE_INV>, ring_smem_bytes<N>()));
+        if (!cuda_ok(h, e, "cudaFuncSetAttribute")) return SAP_ERR_CUDA;
+        // TMA descriptors: tile = NB points along the pass axis x W contiguous kz (or y, Nyquist plane) slots
+        constexpr cuuint32_t W2 = 2 * RingCfg<N>::W, NB = ring_box_rows<N>();
+        const cuuint64_t B3 = (cuuint64_t)h->batch * 3, B1 = (cuuint64_t)h->batch;
+        const cuuint64_t sS[3] = {(cuuint64_t)H * 8, (cuuint64_t)N * H * 8, (cuuint64_t)N * N * H * 8};
+        const cuuint64_t sQ[2] = {(cuuint64_t)N * 8, (cuuint64_t)N * N * 8};
+        const cuuint64_t dS3[4] = {(cuuint64_t)2 * H, N, N, B3}, dS1[4] = {(cuuint64_t)2 * H, N, N, B1};
+        const cuuint64_t dQ3[3] = {(cuuint64_t)2 * N, N, B3}, dQ1[3] = {(cuuint64_t)2 * N, N, B1};
+        const cuuint32_t bx[4] = {W2, 1, NB, 1}, by[4] = {W2, NB, 1, 1}, bq[3] = {W2, NB, 1};
+        const bool ok = make_map(h, &h->mS3x, h->S3, 4, dS3, sS, bx) && make_map(h, &h->mS3y, h->S3, 4, dS3, sS, by) &&
+                        make_map(h, &h->mS1x, h->S1, 4, dS1, sS, bx) && make_map(h, &h->mS1y, h->S1, 4, dS1, sS, by) &&
+                        make_map(h, &h->mQ3, h->Q3, 3, dQ3, sQ, bq) && make_map(h, &h->mQ1, h->Q1, 3, dQ1, sQ, bq) &&
+                        (C::FUSED_ZY || (make_map(h, &h->mQT3, h->QT3, 3, dQ3, sQ, bq) && make_map(h, &h->mQT1, h->QT1, 3, dQ1, sQ, bq)));
+        return ok ? SAP_OK : SAP_ERR_CUDA;
     }
 
-    static StridedParams sp(sap_dpsr* h, const float2* inS, const float2* inQ, float2* outS, float2* outQ, int axis) {
-        StridedParams p;
-        p.inS = inS; p.inQ = inQ; p.outS = outS; p.outQ = outQ; p.tw = h->tw; p.ftab = h->ftab; p.axis = axis;
-        p.cg = 2.f * h->sigma * h->sigma / ((float)N * (float)N);
+    // persistent ring pass (ring_pass.cuh).  axis 0: x pass, axis 1: y pass (N >= 256).  Nyquist plane: the z
+    // pass leaves it transposed ([y][x]) for the y pass, which writes it back as [x][y] for the x pass (and the
+    // other way round on the inverse side), so every tile of every pass is a TMA box with contiguous rows.
+    template <int MODE>
+    static void launch_ring(sap_dpsr* h, cudaStream_t st, int units, const CUtensorMap& mS, const CUtensorMap& mQ,
+                            float2* outS, float2* outQ, int axis) {
+        using RC = RingCfg<N>;
+        RingParams p;
+        p.mapS = mS; p.mapQ = mQ; p.outS = outS; p.outQ = outQ; p.tw = h->tw; p.ftab = h->ftab;
+        p.axis = axis; p.units = units; p.nyq_out_t = (axis == 1 || !C::FUSED_ZY) ? 1 : 0;
         p.cs = (float)((2.0 / ((double)N * N * N)) / (-2.0 * 3.14159265358979323846));
-        return p;
-    }
-
-    template <int MODE, int NT, int W>
-    static void launch_strided(sap_dpsr* h, cudaStream_t st, int planes, const StridedParams& p) {
-        (void)h;
-        k_strided<N, MODE, NT, W><<<dim3(strided_tiles<N, W>(), planes), NT, strided_smem_bytes<N, W>(), st>>>(p);
+        const long long total = (long long)units * (N * (H / RC::W) + N / RC::W);
+        long long grid = (long long)RC::MINB * h->num_sms;
+        if (grid > total) grid = total;
+        k_ring<N, MODE><<<(unsigned)grid, ring_threads<N>(), ring_smem_bytes<N>(), st>>>(p);
     }
 
     static sap_status_t forward(sap_dpsr* h, const float* pts, const float* nrm, int P, float* chi, cudaStream_t st) {
@@ -428,24 +475,21 @@ template <int N> struct Runner {
         }
         // F2 z (+y) forward, 3 channels
         {
-            ZyFwdParams p{h->spts, h->snrm, h->bin_start, P, nullptr, nullptr, h->S3, h->Q3, h->tw, 3};
+            ZyFwdParams p{h->spts, h->snrm, h->bin_start, P, nullptr, nullptr, h->S3, C::FUSED_ZY ? h->Q3 : h->QT3, h->tw, 3};
             k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_SPLAT, C::NT_ZY>
                 <<<dim3(N * N / C::NL, B * 3), C::NT_ZY, zy_smem_bytes<N, C::NL>(), st>>>(p);
             SAP_LAUNCH_CHECK(h, "k_zy_fwd");
         }
         if (!C::FUSED_ZY) {
-            launch_strided<MODE_FWD, C::NTY, C::WY>(h, st, B * 3,
-                sp(h, h->S3, h->Q3, h->S3, h->Q3, 1));
-            SAP_LAUNCH_CHECK(h, "k_strided<FWD,y>");
+            launch_ring<MODE_FWD>(h, st, B * 3, h->mS3y, h->mQT3, h->S3, h->Q3, 1);
+            SAP_LAUNCH_CHECK(h, "k_ring<FWD,y>");
         }
         // F2x + F3 + F4x: x forward, spectral solve, x inverse (3 -> 1)
-        launch_strided<MODE_SOLVE, C::NTX, C::WX>(h, st, B,
-                sp(h, h->S3, h->Q3, h->S1, h->Q1, 0));
-        SAP_LAUNCH_CHECK(h, "k_strided<SOLVE>");
+        launch_ring<MODE_SOLVE>(h, st, B, h->mS3x, h->mQ3, h->S1, C::FUSED_ZY ? h->Q1 : h->QT1, 0);
+        SAP_LAUNCH_CHECK(h, "k_ring<SOLVE>");
         if (!C::FUSED_ZY) {
-            launch_strided<MODE_INV, C::NTY, C::WY>(h, st, B,
-                sp(h, h->S1, h->Q1, h->S1, h->Q1, 1));
-            SAP_LAUNCH_CHECK(h, "k_strided<INV,y>");
+            launch_ring<MODE_INV>(h, st, B, h->mS1y, h->mQT1, h->S1, h->Q1, 1);
+            SAP_LAUNCH_CHECK(h, "k_ring<INV,y>");
         }
         // F4 (y +) z inverse -> chi'
         {
@@ -482,24 +526,21 @@ template <int N> struct Runner {
         }
         // B2 + B3: Gbar' assembled on load, z (+y) forward
         {
-            ZyFwdParams p{h->spts, h->snrm, h->bin_start, P, gchi, h->bw, h->S1, h->Q1, h->tw, 1};
+            ZyFwdParams p{h->spts, h->snrm, h->bin_start, P, gchi, h->bw, h->S1, C::FUSED_ZY ? h->Q1 : h->QT1, h->tw, 1};
             k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_GBAR, C::NT_ZY>
                 <<<dim3(N * N / C::NL, B), C::NT_ZY, zy_smem_bytes<N, C::NL>(), st>>>(p);
             SAP_LAUNCH_CHECK(h, "k_zy_fwd<GBAR>");
         }
         if (!C::FUSED_ZY) {
-            launch_strided<MODE_FWD, C::NTY, C::WY>(h, st, B,
-                sp(h, h->S1, h->Q1, h->S1, h->Q1, 1));
-            SAP_LAUNCH_CHECK(h, "k_strided<FWD,y>");
+            launch_ring<MODE_FWD>(h, st, B, h->mS1y, h->mQT1, h->S1, h->Q1, 1);
+            SAP_LAUNCH_CHECK(h, "k_ring<FWD,y>");
         }
         // B3x + B4 + B5x: x forward, transposed multiplier, 3 x inverse
-        launch_strided<MODE_ADJ, C::NTX, C::WX>(h, st, B,
-                sp(h, h->S1, h->Q1, h->S3, h->Q3, 0));
-        SAP_LAUNCH_CHECK(h, "k_strided<ADJ>");
+        launch_ring<MODE_ADJ>(h, st, B, h->mS1x, h->mQ1, h->S3, C::FUSED_ZY ? h->Q3 : h->QT3, 0);
+        SAP_LAUNCH_CHECK(h, "k_ring<ADJ>");
         if (!C::FUSED_ZY) {
-            launch_strided<MODE_INV, C::NTY, C::WY>(h, st, B * 3,
-                sp(h, h->S3, h->Q3, h->S3, h->Q3, 1));
-            SAP_LAUNCH_CHECK(h, "k_strided<INV,y>");
+            launch_ring<MODE_INV>(h, st, B * 3, h->mS3y, h->mQT3, h->S3, h->Q3, 1);
+            SAP_LAUNCH_CHECK(h, "k_ring<INV,y>");
         }
         // B5 (y +) z inverse -> vbar (into the v workspace)
         {
@@ -537,7 +578,7 @@ static bool supported_N(int N) { return N == 32 || N == 64 || N == 128 || N == 2
 
 static void free_all(sap_dpsr* h) {
     for (int i = 0; i < sap_dpsr::MAX_EV; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
-    cudaFree(h->v); cudaFree(h->spts); cudaFree(h->snrm); cudaFree(h->bin_cnt); cudaFree(h->bin_cursor); cudaFree(h->bin_start); cudaFree(h->S3); cudaFree(h->Q3); cudaFree(h->S1); cudaFree(h->Q1); cudaFree(h->tw); cudaFree(h->ftab);
+    cudaFree(h->v); cudaFree(h->spts); cudaFree(h->snrm); cudaFree(h->bin_cnt); cudaFree(h->bin_cursor); cudaFree(h->bin_start); cudaFree(h->S3); cudaFree(h->Q3); cudaFree(h->S1); cudaFree(h->Q1); cudaFree(h->QT3); cudaFree(h->QT1); cudaFree(h->tw); cudaFree(h->ftab);
     cudaFree(h->acc); cudaFree(h->ticket); cudaFree(h->stats); cudaFree(h->bw);
     cudaFree(h->h_pts); cudaFree(h->h_nrm); cudaFree(h->h_chi); cudaFree(h->h_gchi); cudaFree(h->h_gp); cudaFree(h->h_gn);
 }
@@ -572,6 +613,7 @@ extern "C" sap_status_t sap_dpsr_create(int N, float sigma, int batch, int max_p
     upd(dev_alloc(h, &h->Q3, B * 3 * QP));
     upd(dev_alloc(h, &h->S1, B * SP));
     upd(dev_alloc(h, &h->Q1, B * QP));
+    if (N >= 256) { upd(dev_alloc(h, &h->QT3, B * 3 * QP)); upd(dev_alloc(h, &h->QT1, B * QP)); }
     upd(dev_alloc(h, &h->tw, (size_t)N));
     upd(dev_alloc(h, &h->ftab, (size_t)(N + N / 2 + 1)));
     upd(dev_alloc(h, &h->acc, B * 3));

@@ -25,7 +25,7 @@ struct ZyFwdParams {
     const float* G;        // GBAR: [batch][N^3] upstream gradient
     const float* bw;       // GBAR: [batch][4] = {s, beta/P, S1/a, -}
     float2* S;             // [planes][N*N*H]
-    float2* Q;             // [planes][N*N]
+    float2* Q;             // [planes][N*N]  ([x][y] when the plane is fused (N <= 128), transposed [y][x] otherwise)
     const float2* tw;      // exp(-2 pi i t / N), t < N
     int nch;               // planes per batch item (3 for SPLAT, 1 for GBAR)
 };
@@ -83,7 +83,12 @@ SAP_HD void zy_fwd_body(Ctx& ctx, const ZyFwdParams& p, float2* smem, int bx, in
     }
     if (SRC == SRC_SPLAT && total == 0) {  // nothing lands here: the spectrum of zeros is zeros
         for (int i = ctx.tid; i < NL * H; i += ctx.nthr) So[i] = make_float2(0.f, 0.f);
-        for (int l = ctx.tid; l < NL; l += ctx.nthr) Qo[l] = make_float2(0.f, 0.f);
+        if constexpr (DO_Y) {
+            for (int l = ctx.tid; l < NL; l += ctx.nthr) Qo[l] = make_float2(0.f, 0.f);
+        } else {
+            float2* Qt = p.Q + (size_t)by * ((size_t)N * N);
+            for (int l = ctx.tid; l < NL; l += ctx.nthr) Qt[(size_t)(y0 + l) * N + x] = make_float2(0.f, 0.f);
+        }
         return;
     }
     // A1: zero the plane, rasterise the points into it (shared-memory atomics), z = 2m + parity
@@ -172,7 +177,9 @@ SAP_HD void zy_fwd_body(Ctx& ctx, const ZyFwdParams& p, float2* smem, int bx, in
             const int l = i / H, pz = i - l * H;
             So[i] = s[pz * PITCH + l];
         }
-        for (int l = ctx.tid; l < NL; l += ctx.nthr) Qo[l] = s[H * PITCH + l];
+        // Nyquist plane: written transposed ([y][x]) so that the y pass can fetch it with TMA tiles
+        float2* Qt = p.Q + (size_t)by * ((size_t)N * N);
+        for (int l = ctx.tid; l < NL; l += ctx.nthr) Qt[(size_t)(y0 + l) * N + x] = s[H * PITCH + l];
     } else {
         static_assert(!DO_Y || Plan<N>::NS == 2, "fused planes use two-stage y plans");
         // C: r2c split fused into y stage 0.  One task owns the row pair (k, H-k) for R y-values.
