@@ -51,7 +51,7 @@ template <int N> struct Plan;
 template <> struct Plan<16>  { static constexpr int NS = 1, R0 = 16, R1 = 1,  R2 = 1; };
 template <> struct Plan<32>  { static constexpr int NS = 2, R0 = 8,  R1 = 4,  R2 = 1; };
 template <> struct Plan<64>  { static constexpr int NS = 2, R0 = 8,  R1 = 8,  R2 = 1; };
-template <> struct Plan<128> { static constexpr int NS = 2, R0 = 16, R1 = 8,  R2 = 1; };
+template <> struct Plan<128> { static constexpr int NS = 2, R0 = 8,  R1 = 16, R2 = 1; };
 template <> struct Plan<256> { static constexpr int NS = 2, R0 = 16, R1 = 16, R2 = 1; };
 template <> struct Plan<512> { static constexpr int NS = 3, R0 = 8,  R1 = 8,  R2 = 8; };
 

@@ -1,12 +1,13 @@
-// ring_pass.cuh -- persistent, TMA-fed version of the strided-axis passes (x pass with the fused spectral
-// solve, y pass for N >= 256).  One CTA = NTC consumer threads + one producer warp.  The producer streams
-// tiles of N points x W contiguous columns (W*8-byte rows) from HBM into a ring of NSTAGE shared-memory
-// buffers with cp.async.bulk.tensor (one instruction per tile, completion on an mbarrier); the consumers
-// transform a tile IN PLACE in its buffer, write the result to HBM straight from registers and hand the
-// buffer back.  Loads of the next tiles are therefore in flight during all of the arithmetic, whatever the
-// register count -- the earlier one-tile-per-CTA version depended on occupancy for that overlap.
-//   MODE_FWD / MODE_INV : forward / inverse transform along `axis`
-//   MODE_SOLVE (F2x+F3+F4x): forward x on 3 channels, chi~ = i sum_c m_c v~_c, inverse x, 1 channel out
+// ring_pass.cuh -- persistent, TMA-fed strided-axis passes (x pass with the fused spectral solve; y pass for
+// N >= 256).  A CTA owns a ring of NSTAGE shared-memory buffers, each one tile of N points x W contiguous columns
+// (W*8-byte rows) fetched by ONE cp.async.bulk.tensor whose completion lands on an mbarrier.  NG consumer groups
+// take alternate tiles: a group transforms its tile IN PLACE in the buffer, writes the result to HBM straight
+// from registers and releases the buffer; the thread that sees the last warp of the group release it refills it
+// at once with the tile NSTAGE items ahead.  Loads are therefore in flight during all of the arithmetic whatever
+// the register count (the earlier one-tile-per-CTA kernel depended on occupancy for that overlap), and there is
+// no producer warp.
+//   MODE_FWD / MODE_INV : forward / inverse transform along y
+//   MODE_SOLVE (F2x+F3+F4x): forward x on 3 channels side by side, chi~ = i sum_c m_c v~_c, inverse x, 1 channel out
 //   MODE_ADJ   (B3x+B4+B5x): forward x on 1 channel, vbar~_c = -i m_c Gbar'~, 3 inverse x
 // Equations: Eq.3 / Eq.12-17; multiplier and readings as in spectral.cuh.
 #pragma once
@@ -28,10 +29,15 @@ template <> struct RingCfg<256> { static constexpr int W = 16, NTC = 256, NG = 2
 template <> struct RingCfg<512> { static constexpr int W = 16, NTC = 512, NG = 1, NSTAGE = 3, MINB = 1; };
 template <int N> constexpr int ring_threads() { return RingCfg<N>::NTC * RingCfg<N>::NG; }
 
+// twiddle tables in shared memory: per stage with a stride > 1, ST x R entries [j][r] of float4 (see cmul4), one
+// table for the forward direction and one (conjugated) for the inverse
+template <int N> constexpr int ring_tw_entries() {
+    return N + (Plan<N>::NS == 3 ? StageInfo<N, 1>::ST * StageInfo<N, 1>::R : 0);
+}
 template <int N> constexpr size_t ring_smem_bytes() {
     using C = RingCfg<N>;
-    return (size_t)C::NSTAGE * N * C::W * sizeof(float2) + (size_t)N * sizeof(float2) + (size_t)N * sizeof(float4) +
-           2 * C::NSTAGE * sizeof(uint64_t) + 128;
+    return (size_t)C::NSTAGE * N * C::W * sizeof(float2) + 2 * (size_t)ring_tw_entries<N>() * sizeof(float4) +
+           (size_t)N * sizeof(float4) + 2 * C::NSTAGE * sizeof(uint64_t) + 128;
 }
 template <int N> constexpr int ring_box_rows() { return N < 256 ? N : 256; }  // TMA box dimension limit
 
@@ -42,9 +48,8 @@ struct RingParams {
     float2* outQ;
     const float2* tw;
     const float4* ftab;
-    int axis;            // 0: x pass, 1: y pass (main spectrum only)
     int units;           // planes (FWD / INV) or batch items (SOLVE / ADJ)
-    int nyq_out_t;       // Nyquist-plane output is written transposed ([y][x] <-> [x][y]); always so for axis 1
+    int nyq_out_t;       // x pass: Nyquist-plane output is written transposed ([y][x]); the y pass always reads [y][x], writes [x][y]
     float cs;
 };
 
@@ -81,64 +86,121 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map
         ::"r"(dst), "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)) : "memory");
 }
 template <int NTC> __device__ __forceinline__ void consumer_sync(int group) { asm volatile("bar.sync %0, %1;" ::"r"(group + 1), "n"(NTC) : "memory"); }
-// consumers hand a ring buffer back: order their generic-proxy accesses before the producer's next TMA write
-__device__ __forceinline__ void ring_release(uint64_t* empty_bar) {
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    __syncwarp();
-    if ((threadIdx.x & 31) == 0) mbar_arrive(empty_bar);
+// a * w with the table entry t = {w.x, w.y, -w.y, w.x} (forward) or {w.x, -w.y, w.y, w.x} (a * conj w): two
+// packed instructions, no operand fix-ups
+__device__ __forceinline__ float2 cmul4(float2 a, float4 t) {
+    return __ffma2_rn(make_float2(a.y, a.y), make_float2(t.z, t.w), __fmul2_rn(make_float2(a.x, a.x), make_float2(t.x, t.y)));
 }
 
 }  // namespace sap
 
 namespace sap {
 
-// stage 0 of the length-N plan, in place in a dense [N][W] tile; lanes over columns
-template <int N, int W, int NTC, bool INV>
-__device__ __forceinline__ void ring_stage0(float2* s, const float2* tw, int tid) {
-    constexpr int R = StageInfo<N, 0>::R, ST = StageInfo<N, 0>::ST;
-    for (int t = tid; t < ST * W; t += NTC) {
+// ---- in-place stages on a dense [N][W] tile; lanes run over the W columns -------------------------------
+// Stage S (S = 0 or the middle stage of a 3-stage plan).  tab = this stage's twiddle table for this direction.
+template <int N, int S, int W, int NTC, bool INV>
+__device__ __forceinline__ void ring_stage(float2* s, const float4* tab, int tid) {
+    constexpr int R = StageInfo<N, S>::R, ST = StageInfo<N, S>::ST;
+    constexpr int NT = (N / R) * W;  // butterflies of the tile
+#pragma unroll
+    for (int i = 0; i < (NT + NTC - 1) / NTC; ++i) {
+        const int t = tid + i * NTC;
+        if (NT % NTC != 0 && t >= NT) break;
         const int q = t / W, c = t - q * W;
+        const int blk = q / ST, j = q - blk * ST;
+        float2* b = s + (blk * (R * ST) + j) * W + c;
+        const float4* tr = tab + j * R;
         float2 v[R];
 #pragma unroll
-        for (int r = 0; r < R; ++r) v[r] = s[(q + ST * r) * W + c];
-        if (INV) bfly_inv<N, 0, N>(v, q, tw); else bfly_fwd<N, 0, N>(v, q, tw);
+        for (int r = 0; r < R; ++r) v[r] = b[r * ST * W];
+        if (!INV) {
+            dft_fwd<R>(v);
+            if constexpr (ST > 1) {
 #pragma unroll
-        for (int r = 0; r < R; ++r) s[(q + ST * r) * W + c] = v[r];
+                for (int r = 1; r < R; ++r) v[r] = cmul4(v[r], tr[r]);
+            }
+        } else {
+            if constexpr (ST > 1) {
+#pragma unroll
+                for (int r = 1; r < R; ++r) v[r] = cmul4(v[r], tr[r]);
+            }
+            dft_inv<R>(v);
+        }
+#pragma unroll
+        for (int r = 0; r < R; ++r) b[r * ST * W] = v[r];
     }
 }
+// inverse stage 0: smem -> registers -> HBM.  out + off(row n, column c) = out[n * sn + c * sc]
+template <int N, int W, int NTC>
+__device__ __forceinline__ void ring_stage0_inv_store(const float2* s, const float4* tab, int tid, float2* out, unsigned sn, unsigned sc) {
+    constexpr int R = StageInfo<N, 0>::R, ST = StageInfo<N, 0>::ST;
+    constexpr int NT = ST * W;
+#pragma unroll
+    for (int i = 0; i < (NT + NTC - 1) / NTC; ++i) {
+        const int t = tid + i * NTC;
+        if (NT % NTC != 0 && t >= NT) break;
+        const int q = t / W, c = t - q * W;
+        const float2* b = s + q * W + c;
+        const float4* tr = tab + q * R;
+        float2 v[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) v[r] = b[r * ST * W];
+#pragma unroll
+        for (int r = 1; r < R; ++r) v[r] = cmul4(v[r], tr[r]);
+        dft_inv<R>(v);
+        float2* o = out + (q * sn + c * sc);
+#pragma unroll
+        for (int r = 0; r < R; ++r) o[(unsigned)(r * ST) * sn] = v[r];
+    }
+}
+
+}  // namespace sap
+
+namespace sap {
 
 template <int N, int MODE>
 __global__ void __launch_bounds__(ring_threads<N>(), RingCfg<N>::MINB) k_ring(const __grid_constant__ RingParams p) {
     using C = RingCfg<N>;
     constexpr int W = C::W, NTC = C::NTC, NG = C::NG, NSTAGE = C::NSTAGE, H = N / 2;
+    constexpr int AXIS = (MODE == MODE_FWD || MODE == MODE_INV) ? 1 : 0;  // y pass : x pass
     constexpr int NS = Plan<N>::NS, LS = NS - 1, RL = StageInfo<N, LS>::R;
     static_assert(StageInfo<N, LS>::ST == 1 && NS >= 2, "plan");
-    constexpr int R0 = StageInfo<N, 0>::R, ST0 = StageInfo<N, 0>::ST;
+    constexpr int R0 = StageInfo<N, 0>::R, R1 = StageInfo<N, 1>::R;
+    constexpr int TWE = ring_tw_entries<N>();
     constexpr int TILE_ELEMS = N * W;
     constexpr uint32_t TILE_BYTES = TILE_ELEMS * sizeof(float2);
     constexpr int NB = ring_box_rows<N>();
-    constexpr int NTASK = (N / RL) * W, TPT = (NTASK + NTC - 1) / NTC;
+    constexpr int NTASK = (N / RL) * W, TPT = NTASK / NTC;
     static_assert(NTASK % NTC == 0, "last-stage tasks divide evenly over the consumers");
     constexpr int KT = H / W, TILES_MAIN = N * KT, TILES_NYQ = N / W;
     constexpr int IN_CH = (MODE == MODE_SOLVE) ? 3 : 1, OUT_CH = (MODE == MODE_ADJ) ? 3 : 1;
     constexpr size_t SPLANE = (size_t)N * N * H, QPLANE = (size_t)N * N;
+    constexpr int tiles_per_unit = TILES_MAIN + TILES_NYQ;
+    constexpr int IT_PER_TILE = IN_CH;
 
     extern __shared__ __align__(1024) unsigned char ring_smem[];
     float2* bufs = reinterpret_cast<float2*>(ring_smem);
-    float2* tw = bufs + (size_t)NSTAGE * TILE_ELEMS;
-    float4* fx = reinterpret_cast<float4*>(tw + N);
+    float4* tabF = reinterpret_cast<float4*>(bufs + (size_t)NSTAGE * TILE_ELEMS);
+    float4* tabI = tabF + TWE;
+    float4* fx = tabI + TWE;
     uint64_t* full = reinterpret_cast<uint64_t*>(fx + N);
     uint64_t* empty = full + NSTAGE;
     const int group = threadIdx.x / NTC, tid = threadIdx.x - group * NTC;
 
-    for (int i = threadIdx.x; i < N; i += ring_threads<N>()) { tw[i] = p.tw[i]; fx[i] = p.ftab[i]; }
+    for (int i = threadIdx.x; i < TWE; i += ring_threads<N>()) {
+        int e;  // the entry is w_N^e
+        if (i < N) { const int j = i / R0, r = i - j * R0; e = r * j; }
+        else { const int k = i - N, j = k / R1, r = k - j * R1; e = r * j * R0; }
+        const float2 w = p.tw[e];
+        tabF[i] = make_float4(w.x, w.y, -w.y, w.x);
+        tabI[i] = make_float4(w.x, -w.y, w.y, w.x);
+    }
+    for (int i = threadIdx.x; i < N; i += ring_threads<N>()) fx[i] = p.ftab[i];
     if (threadIdx.x == 0) {
         for (int s = 0; s < NSTAGE; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, NTC / 32); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
-    constexpr int tiles_per_unit = TILES_MAIN + TILES_NYQ;
-    constexpr int IT_PER_TILE = IN_CH;
     const long long total = (long long)p.units * tiles_per_unit;
 
     // One item = one (tile, input channel) = one ring buffer fill.  Item `it` of this CTA lives in buffer it % NSTAGE;
@@ -157,7 +219,7 @@ __global__ void __launch_bounds__(ring_threads<N>(), RingCfg<N>::MINB) k_ring(co
             const int o = T / KT, kt = T - o * KT;
 #pragma unroll
             for (int n0 = 0; n0 < N; n0 += NB) {
-                if (p.axis == 0) tma_load_4d(dst + n0 * W * 8, &p.mapS, 2 * kt * W, o, n0, plane, full + s);
+                if (AXIS == 0) tma_load_4d(dst + n0 * W * 8, &p.mapS, 2 * kt * W, o, n0, plane, full + s);
                 else tma_load_4d(dst + n0 * W * 8, &p.mapS, 2 * kt * W, n0, o, plane, full + s);
             }
         } else {
@@ -177,110 +239,155 @@ __global__ void __launch_bounds__(ring_threads<N>(), RingCfg<N>::MINB) k_ring(co
             issue_load(it + NSTAGE);
         }
     };
+    auto acquire = [&](int it) -> float2* {
+        const int s = it % NSTAGE;
+        mbar_wait(full + s, (it / NSTAGE) & 1);
+        return bufs + (size_t)s * TILE_ELEMS;
+    };
     if (threadIdx.x == 0) {
 #pragma unroll 1
         for (int it = 0; it < NSTAGE; ++it) issue_load(it);
     }
 
-    // ---------------- consumers ----------------
-    float2 acc[TPT][RL];  // SOLVE: divergence accumulators; ADJ: -i f Gbar'~
-    (void)acc;
+    // ---------------- per-tile work of a consumer group ----------------
     for (int j = group, g = blockIdx.x + group * gridDim.x; g < total; j += NG, g += NG * gridDim.x) {
-        int it = j * IT_PER_TILE;  // ring position of this tile's first buffer (same order as the producer)
+        const int it = j * IT_PER_TILE;  // ring position of this tile's first item
         const int unit = g / tiles_per_unit, T = g - unit * tiles_per_unit;
-        TileDesc d = tile_desc<N, W>(p.axis, T);
-        if (d.nyq && p.nyq_out_t) { d.base = (size_t)(T - TILES_MAIN) * W * N; d.sn = 1; d.sc = N; }
-        auto out_plane = [&](int c) {
+        TileDesc d = tile_desc<N, W>(AXIS, T);
+        if (AXIS == 0 && d.nyq && p.nyq_out_t) { d.base = (size_t)(T - TILES_MAIN) * W * N; d.sn = 1; d.sc = N; }
+        const unsigned sn = (unsigned)d.sn, sc = (unsigned)d.sc;
+        auto out_tile = [&](int c) {  // first element of this tile in output channel c
             const size_t plane = (size_t)unit * OUT_CH + c;
-            return d.nyq ? p.outQ + plane * QPLANE : p.outS + plane * SPLANE;
+            return (d.nyq ? p.outQ + plane * QPLANE : p.outS + plane * SPLANE) + d.base;
         };
         auto col_freq = [&](int c, float4& ey, float4& ez) {
             ey = __ldg(p.ftab + (d.nyq ? d.other + c : d.other));
             ez = __ldg(p.ftab + N + (d.nyq ? H : d.pz0 + c));
         };
-        float2* buf = nullptr;
-        int s = 0;
-        // ---- forward half
-        if constexpr (MODE != MODE_INV) {
-#pragma unroll
-            for (int ch = 0; ch < IN_CH; ++ch, ++it) {
-                s = it % NSTAGE;
-                buf = bufs + (size_t)s * TILE_ELEMS;
-                mbar_wait(full + s, (it / NSTAGE) & 1);
-                ring_stage0<N, W, NTC, false>(buf, tw, tid);
+
+        if constexpr (MODE == MODE_FWD) {
+            float2* buf = acquire(it);
+            ring_stage<N, 0, W, NTC, false>(buf, tabF, tid);
+            consumer_sync<NTC>(group);
+            if constexpr (NS == 3) {
+                ring_stage<N, 1, W, NTC, false>(buf, tabF + N, tid);
                 consumer_sync<NTC>(group);
-                if constexpr (NS == 3) {
-                    fft_stage<N, 1, false, N, true>(buf, W, 1, W, tw, tid, NTC);
-                    consumer_sync<NTC>(group);
-                }
-#pragma unroll
-                for (int i = 0; i < TPT; ++i) {
-                    const int t = tid + i * NTC;
-                    const int blk = t / W, c = t - blk * W;
-                    float2 v[RL];
-#pragma unroll
-                    for (int r = 0; r < RL; ++r) v[r] = buf[(blk * RL + r) * W + c];
-                    dft_fwd<RL>(v);
-                    if constexpr (MODE == MODE_FWD) {
-                        float2* gout = out_plane(0);
-#pragma unroll
-                        for (int r = 0; r < RL; ++r)
-                            gout[d.base + (size_t)(blk * RL + r) * d.sn + (size_t)c * d.sc] = v[r];
-                    } else {
-                        float4 ey, ez;
-                        col_freq(c, ey, ez);
-                        if (MODE == MODE_ADJ || ch == 2) {
-#pragma unroll
-                            for (int r = 0; r < RL; ++r) {
-                                const float f = mult_f(fx[blk * RL + r], ey, ez, p.cs);
-                                if constexpr (MODE == MODE_SOLVE) {
-                                    const float2 dv = cscale(f, caxpy(ez.x, v[r], acc[i][r]));
-                                    acc[i][r] = make_float2(-dv.y, dv.x);  // chi~ = i (div)
-                                } else {
-                                    acc[i][r] = make_float2(f * v[r].y, -f * v[r].x);  // -i f Gbar'~
-                                }
-                            }
-                        } else if (ch == 0) {
-#pragma unroll
-                            for (int r = 0; r < RL; ++r) acc[i][r] = cscale(fx[blk * RL + r].x, v[r]);
-                        } else {
-#pragma unroll
-                            for (int r = 0; r < RL; ++r) acc[i][r] = caxpy(ey.x, v[r], acc[i][r]);
-                        }
-                    }
-                }
-                if (MODE == MODE_FWD || (MODE == MODE_SOLVE && ch < 2)) release(it);
             }
-        } else {
-            s = it % NSTAGE;
-            buf = bufs + (size_t)s * TILE_ELEMS;
-            mbar_wait(full + s, (it / NSTAGE) & 1);
-            ++it;
-        }
-        // ---- inverse half, in the buffer of the last input channel
-        if constexpr (MODE != MODE_FWD) {
+            float2* out = out_tile(0);
 #pragma unroll
-            for (int ch = 0; ch < OUT_CH; ++ch) {
+            for (int i = 0; i < TPT; ++i) {
+                const int t = tid + i * NTC, blk = t / W, c = t - blk * W;
+                float2 v[RL];
+#pragma unroll
+                for (int r = 0; r < RL; ++r) v[r] = buf[(blk * RL + r) * W + c];
+                dft_fwd<RL>(v);
+                float2* o = out + ((unsigned)(blk * RL) * sn + c * sc);
+#pragma unroll
+                for (int r = 0; r < RL; ++r) o[(unsigned)r * sn] = v[r];
+            }
+            release(it);
+        } else if constexpr (MODE == MODE_INV) {
+            float2* buf = acquire(it);
+            ring_stage<N, LS, W, NTC, true>(buf, nullptr, tid);
+            consumer_sync<NTC>(group);
+            if constexpr (NS == 3) {
+                ring_stage<N, 1, W, NTC, true>(buf, tabI + N, tid);
+                consumer_sync<NTC>(group);
+            }
+            ring_stage0_inv_store<N, W, NTC>(buf, tabI, tid, out_tile(0), sn, sc);
+            release(it);
+        } else if constexpr (MODE == MODE_SOLVE) {
+            // the three channels of the tile are transformed side by side; the divergence, the multiplier and the
+            // first inverse stage happen on the registers of the last forward stage (same slots, no barrier)
+            float2* b0 = acquire(it);
+            ring_stage<N, 0, W, NTC, false>(b0, tabF, tid);
+            float2* b1 = acquire(it + 1);
+            ring_stage<N, 0, W, NTC, false>(b1, tabF, tid);
+            float2* b2 = acquire(it + 2);
+            ring_stage<N, 0, W, NTC, false>(b2, tabF, tid);
+            consumer_sync<NTC>(group);
+            if constexpr (NS == 3) {
+                ring_stage<N, 1, W, NTC, false>(b0, tabF + N, tid);
+                ring_stage<N, 1, W, NTC, false>(b1, tabF + N, tid);
+                ring_stage<N, 1, W, NTC, false>(b2, tabF + N, tid);
+                consumer_sync<NTC>(group);
+            }
+#pragma unroll 1
+            for (int i = 0; i < TPT; ++i) {
+                const int t = tid + i * NTC, blk = t / W, c = t - blk * W;
+                const int e0 = blk * RL * W + c;
+                float4 ey, ez;
+                col_freq(c, ey, ez);
+                float2 v[RL], a[RL];
+#pragma unroll
+                for (int r = 0; r < RL; ++r) v[r] = b0[e0 + r * W];
+                dft_fwd<RL>(v);
+#pragma unroll
+                for (int r = 0; r < RL; ++r) a[r] = cscale(fx[blk * RL + r].x, v[r]);
+#pragma unroll
+                for (int r = 0; r < RL; ++r) v[r] = b1[e0 + r * W];
+                dft_fwd<RL>(v);
+#pragma unroll
+                for (int r = 0; r < RL; ++r) a[r] = caxpy(ey.x, v[r], a[r]);
+#pragma unroll
+                for (int r = 0; r < RL; ++r) v[r] = b2[e0 + r * W];
+                dft_fwd<RL>(v);
+#pragma unroll
+                for (int r = 0; r < RL; ++r) {
+                    const float f = mult_f(fx[blk * RL + r], ey, ez, p.cs);
+                    const float2 dv = cscale(f, caxpy(ez.x, v[r], a[r]));
+                    a[r] = make_float2(-dv.y, dv.x);  // chi~ = i (div)
+                }
+                dft_inv<RL>(a);
+#pragma unroll
+                for (int r = 0; r < RL; ++r) b2[e0 + r * W] = a[r];
+            }
+            release(it);
+            release(it + 1);
+            consumer_sync<NTC>(group);
+            if constexpr (NS == 3) {
+                ring_stage<N, 1, W, NTC, true>(b2, tabI + N, tid);
+                consumer_sync<NTC>(group);
+            }
+            ring_stage0_inv_store<N, W, NTC>(b2, tabI, tid, out_tile(0), sn, sc);
+            release(it + 2);
+        } else {  // MODE_ADJ
+            float2* buf = acquire(it);
+            ring_stage<N, 0, W, NTC, false>(buf, tabF, tid);
+            consumer_sync<NTC>(group);
+            if constexpr (NS == 3) {
+                ring_stage<N, 1, W, NTC, false>(buf, tabF + N, tid);
+                consumer_sync<NTC>(group);
+            }
+            float2 acc[TPT][RL];  // -i f Gbar'~ on the slots of this thread's last-stage butterflies
+#pragma unroll
+            for (int i = 0; i < TPT; ++i) {
+                const int t = tid + i * NTC, blk = t / W, c = t - blk * W;
+                float4 ey, ez;
+                col_freq(c, ey, ez);
+                float2 v[RL];
+#pragma unroll
+                for (int r = 0; r < RL; ++r) v[r] = buf[(blk * RL + r) * W + c];
+                dft_fwd<RL>(v);
+#pragma unroll
+                for (int r = 0; r < RL; ++r) {
+                    const float f = mult_f(fx[blk * RL + r], ey, ez, p.cs);
+                    acc[i][r] = make_float2(f * v[r].y, -f * v[r].x);
+                }
+            }
+#pragma unroll
+            for (int ch = 0; ch < 3; ++ch) {
                 if (ch > 0) consumer_sync<NTC>(group);  // stage-0 reads of the previous channel are done
 #pragma unroll
                 for (int i = 0; i < TPT; ++i) {
-                    const int t = tid + i * NTC;
-                    const int blk = t / W, c = t - blk * W;
+                    const int t = tid + i * NTC, blk = t / W, c = t - blk * W;
+                    float4 ey, ez;
+                    col_freq(c, ey, ez);
                     float2 v[RL];
-                    if constexpr (MODE == MODE_INV) {
 #pragma unroll
-                        for (int r = 0; r < RL; ++r) v[r] = buf[(blk * RL + r) * W + c];
-                    } else if constexpr (MODE == MODE_SOLVE) {
-#pragma unroll
-                        for (int r = 0; r < RL; ++r) v[r] = acc[i][r];
-                    } else {
-                        float4 ey, ez;
-                        col_freq(c, ey, ez);
-#pragma unroll
-                        for (int r = 0; r < RL; ++r) {
-                            const float h = (ch == 0) ? fx[blk * RL + r].x : (ch == 1) ? ey.x : ez.x;
-                            v[r] = cscale(h, acc[i][r]);
-                        }
+                    for (int r = 0; r < RL; ++r) {
+                        const float h = (ch == 0) ? fx[blk * RL + r].x : (ch == 1) ? ey.x : ez.x;
+                        v[r] = cscale(h, acc[i][r]);
                     }
                     dft_inv<RL>(v);
 #pragma unroll
@@ -288,21 +395,12 @@ __global__ void __launch_bounds__(ring_threads<N>(), RingCfg<N>::MINB) k_ring(co
                 }
                 consumer_sync<NTC>(group);
                 if constexpr (NS == 3) {
-                    fft_stage<N, 1, true, N, true>(buf, W, 1, W, tw, tid, NTC);
+                    ring_stage<N, 1, W, NTC, true>(buf, tabI + N, tid);
                     consumer_sync<NTC>(group);
                 }
-                float2* gout = out_plane(ch);
-                for (int t = tid; t < ST0 * W; t += NTC) {
-                    const int q = t / W, c = t - q * W;
-                    float2 v[R0];
-#pragma unroll
-                    for (int r = 0; r < R0; ++r) v[r] = buf[(q + ST0 * r) * W + c];
-                    bfly_inv<N, 0, N>(v, q, tw);
-#pragma unroll
-                    for (int r = 0; r < R0; ++r) gout[d.base + (size_t)(q + ST0 * r) * d.sn + (size_t)c * d.sc] = v[r];
-                }
+                ring_stage0_inv_store<N, W, NTC>(buf, tabI, tid, out_tile(ch), sn, sc);
             }
-            release(it - 1);
+            release(it);
         }
     }
 }

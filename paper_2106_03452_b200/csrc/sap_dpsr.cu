@@ -25,7 +25,7 @@ struct DevCtx {
 // __global__ wrappers around the block bodies
 // ------------------------------------------------------------------------------------------------
 // minimum resident CTAs per SM the register allocation must allow (a register cliff halves occupancy)
-template <int N> constexpr int zy_min_blocks() { return N == 128 ? 2 : N == 512 ? 3 : 4; }
+template <int N> constexpr int zy_min_blocks() { return N == 128 ? 3 : N == 512 ? 3 : 4; }
 template <int N, int NL, bool DO_Y, int SRC, int NT>
 __global__ void __launch_bounds__(NT, zy_min_blocks<N>()) k_zy_fwd(ZyFwdParams p) {
     extern __shared__ float2 smem[];
@@ -423,8 +423,10 @@ template <int N> struct Runner {
         upd(set_smem(k_zy_inv<N, C::NL, C::FUSED_ZY, C::NT_ZY>, zy_smem_bytes<N, C::NL>()));
         upd(set_smem(k_ring<N, MODE_SOLVE>, ring_smem_bytes<N>()));
         upd(set_smem(k_ring<N, MODE_ADJ>, ring_smem_bytes<N>()));
-        upd(set_smem(k_ring<N, MODE_FWD>, ring_smem_bytes<N>()));
-        upd(set_smem(k_ring<N, MODE_INV>, ring_smem_bytes<N>()));
+        if constexpr (!C::FUSED_ZY) {
+            upd(set_smem(k_ring<N, MODE_FWD>, ring_smem_bytes<N>()));
+            upd(set_smem(k_ring<N, MODE_INV>, ring_smem_bytes<N>()));
+        }
         if (!cuda_ok(h, e, "cudaFuncSetAttribute")) return SAP_ERR_CUDA;
         // TMA descriptors: tile = NB points along the pass axis x W contiguous kz (or y, Nyquist plane) slots
         constexpr cuuint32_t W2 = 2 * RingCfg<N>::W, NB = ring_box_rows<N>();
@@ -450,7 +452,8 @@ template <int N> struct Runner {
         using RC = RingCfg<N>;
         RingParams p;
         p.mapS = mS; p.mapQ = mQ; p.outS = outS; p.outQ = outQ; p.tw = h->tw; p.ftab = h->ftab;
-        p.axis = axis; p.units = units; p.nyq_out_t = (axis == 1 || !C::FUSED_ZY) ? 1 : 0;
+        (void)axis;
+        p.units = units; p.nyq_out_t = C::FUSED_ZY ? 0 : 1;
         p.cs = (float)((2.0 / ((double)N * N * N)) / (-2.0 * 3.14159265358979323846));
         const long long total = (long long)units * (N * (H / RC::W) + N / RC::W);
         long long grid = (long long)RC::MINB * h->num_sms;
@@ -480,14 +483,14 @@ template <int N> struct Runner {
                 <<<dim3(N * N / C::NL, B * 3), C::NT_ZY, zy_smem_bytes<N, C::NL>(), st>>>(p);
             SAP_LAUNCH_CHECK(h, "k_zy_fwd");
         }
-        if (!C::FUSED_ZY) {
+        if constexpr (!C::FUSED_ZY) {
             launch_ring<MODE_FWD>(h, st, B * 3, h->mS3y, h->mQT3, h->S3, h->Q3, 1);
             SAP_LAUNCH_CHECK(h, "k_ring<FWD,y>");
         }
         // F2x + F3 + F4x: x forward, spectral solve, x inverse (3 -> 1)
         launch_ring<MODE_SOLVE>(h, st, B, h->mS3x, h->mQ3, h->S1, C::FUSED_ZY ? h->Q1 : h->QT1, 0);
         SAP_LAUNCH_CHECK(h, "k_ring<SOLVE>");
-        if (!C::FUSED_ZY) {
+        if constexpr (!C::FUSED_ZY) {
             launch_ring<MODE_INV>(h, st, B, h->mS1y, h->mQT1, h->S1, h->Q1, 1);
             SAP_LAUNCH_CHECK(h, "k_ring<INV,y>");
         }
@@ -531,14 +534,14 @@ template <int N> struct Runner {
                 <<<dim3(N * N / C::NL, B), C::NT_ZY, zy_smem_bytes<N, C::NL>(), st>>>(p);
             SAP_LAUNCH_CHECK(h, "k_zy_fwd<GBAR>");
         }
-        if (!C::FUSED_ZY) {
+        if constexpr (!C::FUSED_ZY) {
             launch_ring<MODE_FWD>(h, st, B, h->mS1y, h->mQT1, h->S1, h->Q1, 1);
             SAP_LAUNCH_CHECK(h, "k_ring<FWD,y>");
         }
         // B3x + B4 + B5x: x forward, transposed multiplier, 3 x inverse
         launch_ring<MODE_ADJ>(h, st, B, h->mS1x, h->mQ1, h->S3, C::FUSED_ZY ? h->Q3 : h->QT3, 0);
         SAP_LAUNCH_CHECK(h, "k_ring<ADJ>");
-        if (!C::FUSED_ZY) {
+        if constexpr (!C::FUSED_ZY) {
             launch_ring<MODE_INV>(h, st, B * 3, h->mS3y, h->mQT3, h->S3, h->Q3, 1);
             SAP_LAUNCH_CHECK(h, "k_ring<INV,y>");
         }
