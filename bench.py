@@ -40,18 +40,18 @@ KERNEL_BYTES_V = {
     "F:k_bin_scatter": (0.0, 0.0, 0.0),
     # splat fused in: rows "splat" (3V) + z r2c x3 (6V) [+ y x3 (6V) when fused]; it only WRITES 3V itself
     "F:k_zy_fwd": (15.0, 9.0, 3.0),
-    "F:k_strided<FWD,y>": (0.0, 6.0, 6.0),          # row y sweep x3
-    "F:k_strided<SOLVE>": (4.0, 4.0, 4.0),          # row x sweep + solve + x inverse (3V in, 1V out)
-    "F:k_strided<INV,y>": (0.0, 2.0, 2.0),          # row inverse y
+    "F:k_ring<FWD,y>": (0.0, 6.0, 6.0),          # row y sweep x3
+    "F:k_ring<SOLVE>": (4.0, 4.0, 4.0),          # row x sweep + solve + x inverse (3V in, 1V out)
+    "F:k_ring<INV,y>": (0.0, 2.0, 2.0),          # row inverse y
     "F:k_zy_inv": (4.0, 2.0, 2.0),                  # rows [inverse y (2V) +] inverse z c2r (2V)
     "F:k_sample_mean": (0.0, 0.0, 0.0),
     "F:k_scale_shift": (2.0, 2.0, 2.0),             # row normalise
     # backward
     "B:k_reduce_g": (2.0, 2.0, 2.0),                # row reductions
     "B:k_zy_fwd<GBAR>": (5.0, 3.0, 2.0),            # rows z r2c (G+W in, 1 out = 3V) [+ y (2V)]; W is re-rasterised, not read
-    "B:k_strided<FWD,y>": (0.0, 2.0, 2.0),
-    "B:k_strided<ADJ>": (4.0, 4.0, 4.0),            # row x sweep + conj(M) fan-out + 3 x inverse
-    "B:k_strided<INV,y>": (0.0, 6.0, 6.0),
+    "B:k_ring<FWD,y>": (0.0, 2.0, 2.0),
+    "B:k_ring<ADJ>": (4.0, 4.0, 4.0),            # row x sweep + conj(M) fan-out + 3 x inverse
+    "B:k_ring<INV,y>": (0.0, 6.0, 6.0),
     "B:k_zy_inv": (12.0, 6.0, 6.0),                 # rows inverse y x3 + inverse z x3
     "B:k_gather_grads": (4.0, 4.0, 0.0),            # row gather (<= 4V, sparse)
 }

@@ -26,7 +26,7 @@ template <> struct RingCfg<32>  { static constexpr int W = 16, NTC = 128, NG = 1
 template <> struct RingCfg<64>  { static constexpr int W = 32, NTC = 256, NG = 1, NSTAGE = 4, MINB = 3; };
 template <> struct RingCfg<128> { static constexpr int W = 32, NTC = 256, NG = 2, NSTAGE = 6, MINB = 1; };
 template <> struct RingCfg<256> { static constexpr int W = 16, NTC = 256, NG = 2, NSTAGE = 6, MINB = 1; };
-template <> struct RingCfg<512> { static constexpr int W = 16, NTC = 512, NG = 1, NSTAGE = 3, MINB = 1; };
+template <> struct RingCfg<512> { static constexpr int W = 16, NTC = 512, NG = 1, NSTAGE = 3, MINB = 1; };  // 64-byte rows (W = 8) measured 25% slower
 template <int N> constexpr int ring_threads() { return RingCfg<N>::NTC * RingCfg<N>::NG; }
 
 // twiddle tables in shared memory: per stage with a stride > 1, ST x R entries [j][r] of float4 (see cmul4), one
@@ -296,6 +296,58 @@ __global__ void __launch_bounds__(ring_threads<N>(), RingCfg<N>::MINB) k_ring(co
             }
             ring_stage0_inv_store<N, W, NTC>(buf, tabI, tid, out_tile(0), sn, sc);
             release(it);
+        } else if constexpr (MODE == MODE_SOLVE && NSTAGE < 2 * 3) {
+            // ring too short to hold a whole tile and still prefetch (N = 512): one channel at a time, the divergence
+            // accumulated in registers, each buffer released as soon as its last forward stage has been read
+            float2 acc[TPT][RL];
+            float2* buf = nullptr;
+#pragma unroll
+            for (int ch = 0; ch < 3; ++ch) {
+                buf = acquire(it + ch);
+                ring_stage<N, 0, W, NTC, false>(buf, tabF, tid);
+                consumer_sync<NTC>(group);
+                if constexpr (NS == 3) {
+                    ring_stage<N, 1, W, NTC, false>(buf, tabF + N, tid);
+                    consumer_sync<NTC>(group);
+                }
+#pragma unroll
+                for (int i = 0; i < TPT; ++i) {
+                    const int t = tid + i * NTC, blk = t / W, c = t - blk * W;
+                    const int e0 = blk * RL * W + c;
+                    float4 ey, ez;
+                    col_freq(c, ey, ez);
+                    float2 v[RL];
+#pragma unroll
+                    for (int r = 0; r < RL; ++r) v[r] = buf[e0 + r * W];
+                    dft_fwd<RL>(v);
+                    if (ch == 0) {
+#pragma unroll
+                        for (int r = 0; r < RL; ++r) acc[i][r] = cscale(fx[blk * RL + r].x, v[r]);
+                    } else if (ch == 1) {
+#pragma unroll
+                        for (int r = 0; r < RL; ++r) acc[i][r] = caxpy(ey.x, v[r], acc[i][r]);
+                    } else {
+                        float2 a[RL];
+#pragma unroll
+                        for (int r = 0; r < RL; ++r) {
+                            const float f = mult_f(fx[blk * RL + r], ey, ez, p.cs);
+                            const float2 dv = cscale(f, caxpy(ez.x, v[r], acc[i][r]));
+                            a[r] = make_float2(-dv.y, dv.x);  // chi~ = i (div)
+                        }
+                        dft_inv<RL>(a);
+#pragma unroll
+                        for (int r = 0; r < RL; ++r) buf[e0 + r * W] = a[r];
+                    }
+                }
+                if (ch < 2) release(it + ch);
+            }
+            consumer_sync<NTC>(group);
+            if constexpr (NS == 3) {
+                ring_stage<N, 1, W, NTC, true>(buf, tabI + N, tid);
+                consumer_sync<NTC>(group);
+            }
+            ring_stage0_inv_store<N, W, NTC>(buf, tabI, tid, out_tile(0), sn, sc);
+            release(it + 2);
         } else if constexpr (MODE == MODE_SOLVE) {
             // the three channels of the tile are transformed side by side; the divergence, the multiplier and the
             // first inverse stage happen on the registers of the last forward stage (same slots, no barrier)
