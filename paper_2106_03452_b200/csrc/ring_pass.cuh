@@ -24,7 +24,7 @@ template <int N> struct RingCfg;
 // resident CTAs per SM
 template <> struct RingCfg<32>  { static constexpr int W = 16, NTC = 128, NG = 1, NSTAGE = 4, MINB = 4; };
 template <> struct RingCfg<64>  { static constexpr int W = 32, NTC = 256, NG = 1, NSTAGE = 4, MINB = 3; };
-template <> struct RingCfg<128> { static constexpr int W = 32, NTC = 256, NG = 2, NSTAGE = 6, MINB = 1; };
+template <> struct RingCfg<128> { static constexpr int W = 16, NTC = 128, NG = 4, NSTAGE = 12, MINB = 1; };
 template <> struct RingCfg<256> { static constexpr int W = 16, NTC = 256, NG = 2, NSTAGE = 6, MINB = 1; };
 template <> struct RingCfg<512> { static constexpr int W = 16, NTC = 512, NG = 1, NSTAGE = 3, MINB = 1; };  // 64-byte rows (W = 8) measured 25% slower
 template <int N> constexpr int ring_threads() { return RingCfg<N>::NTC * RingCfg<N>::NG; }
