@@ -17,6 +17,15 @@
 
 namespace sap {
 
+// Programmatic dependent launch (all kernels of the path are launched with it, see launch_pdl in sap_dpsr.cu):
+// the launch of kernel n+1 is processed while kernel n runs; pdl_wait() blocks until kernel n has completed and
+// its writes are visible.  Nothing written by a predecessor is touched before pdl_wait().  No kernel triggers its
+// dependents early (griddepcontrol.launch_dependents on entry was measured 20% SLOWER at 128^3: the early CTAs
+// take shared memory and issue slots from the running kernel), so the trigger is the implicit one at grid exit.
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+#endif
+
 // Complex arithmetic on float2 = (re, im).  On sm_100a these map to the packed FP32x2 instructions
 // (FADD2 / FMUL2 / FFMA2): one issue slot per complex add, two per complex multiply.  The operand
 // modifiers of those instructions (half swap, per-half negate, scalar broadcast) absorb mul_mi and conj.

@@ -201,6 +201,7 @@ __global__ void __launch_bounds__(ring_threads<N>(), RingCfg<N>::MINB) k_ring(co
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
+    pdl_wait();  // the tables above are constants of the handle; the spectra below are the predecessor's output
     const long long total = (long long)p.units * tiles_per_unit;
 
     // One item = one (tile, input channel) = one ring buffer fill.  Item `it` of this CTA lives in buffer it % NSTAGE;

@@ -30,12 +30,14 @@ template <int N, int NL, bool DO_Y, int SRC, int NT>
 __global__ void __launch_bounds__(NT, zy_min_blocks<N>()) k_zy_fwd(ZyFwdParams p) {
     extern __shared__ float2 smem[];
     DevCtx ctx{(int)threadIdx.x, NT};
+    pdl_wait();
     zy_fwd_body<N, NL, DO_Y, SRC>(ctx, p, smem, (int)blockIdx.x, (int)blockIdx.y);
 }
 template <int N, int NL, bool DO_Y, int NT>
 __global__ void __launch_bounds__(NT, zy_min_blocks<N>()) k_zy_inv(ZyInvParams p) {
     extern __shared__ float2 smem[];
     DevCtx ctx{(int)threadIdx.x, NT};
+    pdl_wait();
     zy_inv_body<N, NL, DO_Y>(ctx, p, smem, (int)blockIdx.x, (int)blockIdx.y);
 }
 
@@ -73,12 +75,14 @@ __device__ __forceinline__ int bin_key(const float* __restrict__ c, int N, int N
     return jx * (N / NL) + jy / NL;
 }
 __global__ void k_bin_count(const float* __restrict__ pts, int P, int N, int NL, int nbins, int* __restrict__ cnt) {
+    pdl_wait();
     const int i = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y;
     if (i >= P) return;
     atomicAdd(cnt + (size_t)b * nbins + bin_key(pts + ((size_t)b * P + i) * 3, N, NL), 1);
 }
 // one block per item: exclusive scan of the counts -> start[nbins+1]; cursor = start; counts reset to 0
 __global__ void k_bin_scan(int* __restrict__ cnt, int nbins, int P, int* __restrict__ start, int* __restrict__ cursor) {
+    pdl_wait();
     __shared__ int wsum[32];
     const int b = blockIdx.x, tid = threadIdx.x, nt = blockDim.x;
     int* c = cnt + (size_t)b * nbins;
@@ -119,6 +123,7 @@ __global__ void k_bin_scan(int* __restrict__ cnt, int nbins, int P, int* __restr
 __global__ void k_bin_scatter(const float* __restrict__ pts, const float* __restrict__ nrm, int P, int N, int NL,
                               int nbins, int* __restrict__ cursor, float4* __restrict__ spts,
                               float4* __restrict__ snrm) {
+    pdl_wait();
     const int i = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y;
     if (i >= P) return;
     const float* c = pts + ((size_t)b * P + i) * 3;
@@ -153,6 +158,7 @@ __device__ __forceinline__ float block_sum(float x, float* sh) {
 __global__ void k_sample_mean(const float* __restrict__ pts, int P, int N, const float* __restrict__ chi_p,
                               double* __restrict__ acc, unsigned* __restrict__ ticket,
                               float* __restrict__ stats) {
+    pdl_wait();
     __shared__ float sh[32];
     const int b = blockIdx.y;
     const size_t V = (size_t)N * N * N;
@@ -191,6 +197,7 @@ __global__ void k_sample_mean(const float* __restrict__ pts, int P, int N, const
 
 // F5b: chi = s (chi' - mu), in place
 __global__ void k_scale_shift(float4* __restrict__ chi, size_t n4_per_item, const float* __restrict__ stats) {
+    pdl_wait();
     const int b = blockIdx.y;
     const float mu = stats[b * 4 + 0], s = stats[b * 4 + 2];
     float4* p = chi + (size_t)b * n4_per_item;
@@ -207,6 +214,7 @@ __global__ void k_scale_shift(float4* __restrict__ chi, size_t n4_per_item, cons
 __global__ void k_reduce_g(const float4* __restrict__ G, const float4* __restrict__ chi, size_t n4_per_item,
                            int P, const float* __restrict__ stats, double* __restrict__ acc,
                            unsigned* __restrict__ ticket, float* __restrict__ bw) {
+    pdl_wait();
     __shared__ float sh[32];
     const int b = blockIdx.y;
     const float4* g = G + (size_t)b * n4_per_item;
@@ -247,6 +255,7 @@ __global__ void k_reduce_g(const float4* __restrict__ G, const float4* __restric
 __global__ void k_gather_grads(const float* __restrict__ pts, const float* __restrict__ nrm, int P, int N,
                                const float* __restrict__ vbar, const float* __restrict__ chi,
                                const float* __restrict__ bw, float* __restrict__ gp, float* __restrict__ gn) {
+    pdl_wait();
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int b = blockIdx.y;
     if (i >= P) return;
@@ -360,6 +369,19 @@ static void prof_begin(sap_dpsr* h, cudaStream_t st) {
     prof_mark(h, "begin", st);
 }
 
+// Every kernel of the path is launched with programmatic dependent launch (see pdl_wait in fft_core.cuh): the
+// launch latency of kernel n+1 hides behind kernel n.
+template <class... KArgs, class... Args>
+static void launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+
 template <class K> static cudaError_t set_smem(K kernel, size_t bytes) {
     return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
 }
@@ -458,7 +480,7 @@ template <int N> struct Runner {
         const long long total = (long long)units * (N * (H / RC::W) + N / RC::W);
         long long grid = (long long)RC::MINB * h->num_sms;
         if (grid > total) grid = total;
-        k_ring<N, MODE><<<(unsigned)grid, ring_threads<N>(), ring_smem_bytes<N>(), st>>>(p);
+        launch_pdl(k_ring<N, MODE>, dim3((unsigned)grid), dim3(ring_threads<N>()), ring_smem_bytes<N>(), st, p);
     }
 
     static sap_status_t forward(sap_dpsr* h, const float* pts, const float* nrm, int P, float* chi, cudaStream_t st) {
@@ -468,19 +490,18 @@ template <int N> struct Runner {
         // F1a: bin the points (counting sort); the rasterisation itself happens inside k_zy_fwd
         {
             const dim3 gp((P + 255) / 256, B);
-            k_bin_count<<<gp, 256, 0, st>>>(pts, P, N, C::NL, h->nbins, h->bin_cnt);
+            launch_pdl(k_bin_count, dim3(gp), dim3(256), 0, st, pts, P, N, C::NL, h->nbins, h->bin_cnt);
             SAP_LAUNCH_CHECK(h, "k_bin_count");
-            k_bin_scan<<<B, 1024, 0, st>>>(h->bin_cnt, h->nbins, P, h->bin_start, h->bin_cursor);
+            launch_pdl(k_bin_scan, dim3(B), dim3(1024), 0, st, h->bin_cnt, h->nbins, P, h->bin_start, h->bin_cursor);
             SAP_LAUNCH_CHECK(h, "k_bin_scan");
-            k_bin_scatter<<<gp, 256, 0, st>>>(pts, nrm, P, N, C::NL, h->nbins, h->bin_cursor, h->spts, h->snrm);
+            launch_pdl(k_bin_scatter, dim3(gp), dim3(256), 0, st, pts, nrm, P, N, C::NL, h->nbins, h->bin_cursor, h->spts, h->snrm);
             SAP_LAUNCH_CHECK(h, "k_bin_scatter");
             h->binned_P = P;
         }
         // F2 z (+y) forward, 3 channels
         {
             ZyFwdParams p{h->spts, h->snrm, h->bin_start, P, nullptr, nullptr, h->S3, C::FUSED_ZY ? h->Q3 : h->QT3, h->tw, 3};
-            k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_SPLAT, C::NT_ZY>
-                <<<dim3(N * N / C::NL, B * 3), C::NT_ZY, zy_smem_bytes<N, C::NL>(), st>>>(p);
+            launch_pdl(k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_SPLAT, C::NT_ZY>, dim3(dim3(N * N / C::NL, B * 3)), dim3(C::NT_ZY), zy_smem_bytes<N, C::NL>(), st, p);
             SAP_LAUNCH_CHECK(h, "k_zy_fwd");
         }
         if constexpr (!C::FUSED_ZY) {
@@ -497,18 +518,17 @@ template <int N> struct Runner {
         // F4 (y +) z inverse -> chi'
         {
             ZyInvParams p{h->S1, h->Q1, chi, h->tw};
-            k_zy_inv<N, C::NL, C::FUSED_ZY, C::NT_ZY>
-                <<<dim3(N * N / C::NL, B), C::NT_ZY, zy_smem_bytes<N, C::NL>(), st>>>(p);
+            launch_pdl(k_zy_inv<N, C::NL, C::FUSED_ZY, C::NT_ZY>, dim3(dim3(N * N / C::NL, B)), dim3(C::NT_ZY), zy_smem_bytes<N, C::NL>(), st, p);
             SAP_LAUNCH_CHECK(h, "k_zy_inv");
         }
         // F5 normalise
         {
             int nb = (P + 255) / 256; if (nb > 296) nb = 296;
-            k_sample_mean<<<dim3(nb, B), 256, 0, st>>>(pts, P, N, chi, h->acc, h->ticket, h->stats);
+            launch_pdl(k_sample_mean, dim3(dim3(nb, B)), dim3(256), 0, st, pts, P, N, chi, h->acc, h->ticket, h->stats);
             SAP_LAUNCH_CHECK(h, "k_sample_mean");
             const size_t n4 = V / 4;
             int gb = (int)((n4 + 255) / 256); const int cap = (148 * 8 + B - 1) / B; if (gb > cap) gb = cap; if (gb < 1) gb = 1;
-            k_scale_shift<<<dim3(gb, B), 256, 0, st>>>(reinterpret_cast<float4*>(chi), n4, h->stats);
+            launch_pdl(k_scale_shift, dim3(dim3(gb, B)), dim3(256), 0, st, reinterpret_cast<float4*>(chi), n4, h->stats);
             SAP_LAUNCH_CHECK(h, "k_scale_shift");
         }
         return SAP_OK;
@@ -523,15 +543,14 @@ template <int N> struct Runner {
         {
             const size_t n4 = V / 4;
             int gb = (int)((n4 + 255) / 256); const int cap = (148 * 4 + B - 1) / B; if (gb > cap) gb = cap; if (gb < 1) gb = 1;
-            k_reduce_g<<<dim3(gb, B), 256, 0, st>>>(reinterpret_cast<const float4*>(gchi), reinterpret_cast<const float4*>(chi),
+            launch_pdl(k_reduce_g, dim3(dim3(gb, B)), dim3(256), 0, st, reinterpret_cast<const float4*>(gchi), reinterpret_cast<const float4*>(chi),
                                                    n4, P, h->stats, h->acc + B, h->ticket + B, h->bw);
             SAP_LAUNCH_CHECK(h, "k_reduce_g");
         }
         // B2 + B3: Gbar' assembled on load, z (+y) forward
         {
             ZyFwdParams p{h->spts, h->snrm, h->bin_start, P, gchi, h->bw, h->S1, C::FUSED_ZY ? h->Q1 : h->QT1, h->tw, 1};
-            k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_GBAR, C::NT_ZY>
-                <<<dim3(N * N / C::NL, B), C::NT_ZY, zy_smem_bytes<N, C::NL>(), st>>>(p);
+            launch_pdl(k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_GBAR, C::NT_ZY>, dim3(dim3(N * N / C::NL, B)), dim3(C::NT_ZY), zy_smem_bytes<N, C::NL>(), st, p);
             SAP_LAUNCH_CHECK(h, "k_zy_fwd<GBAR>");
         }
         if constexpr (!C::FUSED_ZY) {
@@ -548,12 +567,11 @@ template <int N> struct Runner {
         // B5 (y +) z inverse -> vbar (into the v workspace)
         {
             ZyInvParams p{h->S3, h->Q3, h->v, h->tw};
-            k_zy_inv<N, C::NL, C::FUSED_ZY, C::NT_ZY>
-                <<<dim3(N * N / C::NL, B * 3), C::NT_ZY, zy_smem_bytes<N, C::NL>(), st>>>(p);
+            launch_pdl(k_zy_inv<N, C::NL, C::FUSED_ZY, C::NT_ZY>, dim3(dim3(N * N / C::NL, B * 3)), dim3(C::NT_ZY), zy_smem_bytes<N, C::NL>(), st, p);
             SAP_LAUNCH_CHECK(h, "k_zy_inv");
         }
         // B6 gather
-        k_gather_grads<<<dim3((P + 127) / 128, B), 128, 0, st>>>(pts, nrm, P, N, h->v, chi, h->bw, gp, gn);
+        launch_pdl(k_gather_grads, dim3(dim3((P + 127) / 128, B)), dim3(128), 0, st, pts, nrm, P, N, h->v, chi, h->bw, gp, gn);
         SAP_LAUNCH_CHECK(h, "k_gather_grads");
         return SAP_OK;
     }
