@@ -98,8 +98,9 @@ namespace sap {
 
 // ---- in-place stages on a dense [N][W] tile; lanes run over the W columns -------------------------------
 // Stage S (S = 0 or the middle stage of a 3-stage plan).  tab = this stage's twiddle table for this direction.
+// swz = 15 for a y-pass tile of the main spectrum (row n holds z slot c in column c ^ (n & 15), see kz_swz), else 0.
 template <int N, int S, int W, int NTC, bool INV>
-__device__ __forceinline__ void ring_stage(float2* s, const float4* tab, int tid) {
+__device__ __forceinline__ void ring_stage(float2* s, const float4* tab, int tid, int swz = 0) {
     constexpr int R = StageInfo<N, S>::R, ST = StageInfo<N, S>::ST;
     constexpr int NT = (N / R) * W;  // butterflies of the tile
 #pragma unroll
@@ -108,11 +109,11 @@ __device__ __forceinline__ void ring_stage(float2* s, const float4* tab, int tid
         if (NT % NTC != 0 && t >= NT) break;
         const int q = t / W, c = t - q * W;
         const int blk = q / ST, j = q - blk * ST;
-        float2* b = s + (blk * (R * ST) + j) * W + c;
+        const int row0 = blk * (R * ST) + j;
         const float4* tr = tab + j * R;
         float2 v[R];
 #pragma unroll
-        for (int r = 0; r < R; ++r) v[r] = b[r * ST * W];
+        for (int r = 0; r < R; ++r) v[r] = s[(row0 + r * ST) * W + (c ^ ((row0 + r * ST) & swz))];
         if (!INV) {
             dft_fwd<R>(v);
             if constexpr (ST > 1) {
@@ -127,12 +128,12 @@ __device__ __forceinline__ void ring_stage(float2* s, const float4* tab, int tid
             dft_inv<R>(v);
         }
 #pragma unroll
-        for (int r = 0; r < R; ++r) b[r * ST * W] = v[r];
+        for (int r = 0; r < R; ++r) s[(row0 + r * ST) * W + (c ^ ((row0 + r * ST) & swz))] = v[r];
     }
 }
 // inverse stage 0: smem -> registers -> HBM.  out + off(row n, column c) = out[n * sn + c * sc]
 template <int N, int W, int NTC>
-__device__ __forceinline__ void ring_stage0_inv_store(const float2* s, const float4* tab, int tid, float2* out, unsigned sn, unsigned sc) {
+__device__ __forceinline__ void ring_stage0_inv_store(const float2* s, const float4* tab, int tid, float2* out, unsigned sn, unsigned sc, int swz = 0) {
     constexpr int R = StageInfo<N, 0>::R, ST = StageInfo<N, 0>::ST;
     constexpr int NT = ST * W;
 #pragma unroll
@@ -140,17 +141,15 @@ __device__ __forceinline__ void ring_stage0_inv_store(const float2* s, const flo
         const int t = tid + i * NTC;
         if (NT % NTC != 0 && t >= NT) break;
         const int q = t / W, c = t - q * W;
-        const float2* b = s + q * W + c;
         const float4* tr = tab + q * R;
         float2 v[R];
 #pragma unroll
-        for (int r = 0; r < R; ++r) v[r] = b[r * ST * W];
+        for (int r = 0; r < R; ++r) v[r] = s[(q + r * ST) * W + (c ^ ((q + r * ST) & swz))];
 #pragma unroll
         for (int r = 1; r < R; ++r) v[r] = cmul4(v[r], tr[r]);
         dft_inv<R>(v);
-        float2* o = out + (q * sn + c * sc);
 #pragma unroll
-        for (int r = 0; r < R; ++r) o[(unsigned)(r * ST) * sn] = v[r];
+        for (int r = 0; r < R; ++r) out[(unsigned)(q + r * ST) * sn + (unsigned)(c ^ ((q + r * ST) & swz)) * sc] = v[r];
     }
 }
 
@@ -257,21 +256,23 @@ __global__ void __launch_bounds__(ring_threads<N>(), RingCfg<N>::MINB) k_ring(co
         TileDesc d = tile_desc<N, W>(AXIS, T);
         if (AXIS == 0 && d.nyq && p.nyq_out_t) { d.base = (size_t)(T - TILES_MAIN) * W * N; d.sn = 1; d.sc = N; }
         const unsigned sn = (unsigned)d.sn, sc = (unsigned)d.sc;
+        const int swz = (AXIS == 1 && !d.nyq) ? 15 : 0;  // y-pass tiles of the main spectrum: column swizzle per row
+        const int xswz = (AXIS == 0 && !d.nyq) ? (d.other & 15) : 0;  // x-pass tile at y = d.other: one XOR for the tile
         auto out_tile = [&](int c) {  // first element of this tile in output channel c
             const size_t plane = (size_t)unit * OUT_CH + c;
             return (d.nyq ? p.outQ + plane * QPLANE : p.outS + plane * SPLANE) + d.base;
         };
         auto col_freq = [&](int c, float4& ey, float4& ez) {
             ey = __ldg(p.ftab + (d.nyq ? d.other + c : d.other));
-            ez = __ldg(p.ftab + N + (d.nyq ? H : d.pz0 + c));
+            ez = __ldg(p.ftab + N + (d.nyq ? H : d.pz0 + (c ^ xswz)));
         };
 
         if constexpr (MODE == MODE_FWD) {
             float2* buf = acquire(it);
-            ring_stage<N, 0, W, NTC, false>(buf, tabF, tid);
+            ring_stage<N, 0, W, NTC, false>(buf, tabF, tid, swz);
             consumer_sync<NTC>(group);
             if constexpr (NS == 3) {
-                ring_stage<N, 1, W, NTC, false>(buf, tabF + N, tid);
+                ring_stage<N, 1, W, NTC, false>(buf, tabF + N, tid, swz);
                 consumer_sync<NTC>(group);
             }
             float2* out = out_tile(0);
@@ -280,22 +281,22 @@ __global__ void __launch_bounds__(ring_threads<N>(), RingCfg<N>::MINB) k_ring(co
                 const int t = tid + i * NTC, blk = t / W, c = t - blk * W;
                 float2 v[RL];
 #pragma unroll
-                for (int r = 0; r < RL; ++r) v[r] = buf[(blk * RL + r) * W + c];
+                for (int r = 0; r < RL; ++r) v[r] = buf[(blk * RL + r) * W + (c ^ ((blk * RL + r) & swz))];
                 dft_fwd<RL>(v);
-                float2* o = out + ((unsigned)(blk * RL) * sn + c * sc);
 #pragma unroll
-                for (int r = 0; r < RL; ++r) o[(unsigned)r * sn] = v[r];
+                for (int r = 0; r < RL; ++r)
+                    out[(unsigned)(blk * RL + r) * sn + (unsigned)(c ^ ((blk * RL + r) & swz)) * sc] = v[r];
             }
             release(it);
         } else if constexpr (MODE == MODE_INV) {
             float2* buf = acquire(it);
-            ring_stage<N, LS, W, NTC, true>(buf, nullptr, tid);
+            ring_stage<N, LS, W, NTC, true>(buf, nullptr, tid, swz);
             consumer_sync<NTC>(group);
             if constexpr (NS == 3) {
-                ring_stage<N, 1, W, NTC, true>(buf, tabI + N, tid);
+                ring_stage<N, 1, W, NTC, true>(buf, tabI + N, tid, swz);
                 consumer_sync<NTC>(group);
             }
-            ring_stage0_inv_store<N, W, NTC>(buf, tabI, tid, out_tile(0), sn, sc);
+            ring_stage0_inv_store<N, W, NTC>(buf, tabI, tid, out_tile(0), sn, sc, swz);
             release(it);
         } else if constexpr (MODE == MODE_SOLVE && NSTAGE < 2 * 3) {
             // ring too short to hold a whole tile and still prefetch (N = 512): one channel at a time, the divergence

@@ -36,6 +36,12 @@ struct ZyInvParams {
     const float2* tw;
 };
 
+// Column swizzle of the main spectrum in HBM: the value of z slot pz of line (x, y) is stored in column
+// pz ^ (y & 15).  Within a 16-column group the columns of 16 consecutive lines are then all different, so a tile
+// of lines that a bulk copy drops DENSE into shared memory can be walked "lanes over lines" without bank
+// conflicts.  An involution: the same function maps a stored column back to its slot.
+SAP_HD int kz_swz(int pz, int y) { return pz ^ (y & 15); }
+
 template <int N, int NL> constexpr size_t zy_smem_bytes() { return ((size_t)(N / 2 + 1) * (NL + 1) + N) * sizeof(float2); }
 
 // task t -> (line, q) for the global<->smem z stage: q (ST0 consecutive complex of one line) fastest,
@@ -174,8 +180,8 @@ SAP_HD void zy_fwd_body(Ctx& ctx, const ZyFwdParams& p, float2* smem, int bx, in
         r2c_split<N, N>(ctx, s, PITCH, 1, NL, tw);
         ctx.sync();
         for (int i = ctx.tid; i < NL * H; i += ctx.nthr) {
-            const int l = i / H, pz = i - l * H;
-            So[i] = s[pz * PITCH + l];
+            const int l = i / H, pc = i - l * H;
+            So[i] = s[kz_swz(pc, y0 + l) * PITCH + l];
         }
         // Nyquist plane: written transposed ([y][x]) so that the y pass can fetch it with TMA tiles
         float2* Qt = p.Q + (size_t)by * ((size_t)N * N);
@@ -235,7 +241,7 @@ SAP_HD void zy_fwd_body(Ctx& ctx, const ZyFwdParams& p, float2* smem, int bx, in
             for (int r = 0; r < R1; ++r) v[r] = s[pz * PITCH + blk * R1 + r];
             dft_fwd<R1>(v);
 #pragma unroll
-            for (int r = 0; r < R1; ++r) So[(size_t)(blk * R1 + r) * H + pz] = v[r];
+            for (int r = 0; r < R1; ++r) So[(size_t)(blk * R1 + r) * H + kz_swz(pz, blk * R1 + r)] = v[r];
         }
         for (int blk = ctx.tid; blk < N / R1; blk += ctx.nthr) {  // Nyquist row
             float2 v[R1];
@@ -263,9 +269,10 @@ SAP_HD void zy_inv_body(Ctx& ctx, const ZyInvParams& p, float2* smem, int bx, in
     const float2* Si = p.S + (size_t)by * ((size_t)N * N * H) + line0 * H;
     const float2* Qi = p.Q + (size_t)by * ((size_t)N * N) + line0;
     if constexpr (!DO_Y) {
+        const int y0 = (int)(line0 % N);
         for (int i = ctx.tid; i < NL * H; i += ctx.nthr) {
-            const int l = i / H, pz = i - l * H;
-            s[pz * PITCH + l] = Si[i];
+            const int l = i / H, pc = i - l * H;
+            s[kz_swz(pc, y0 + l) * PITCH + l] = Si[i];
         }
         for (int l = ctx.tid; l < NL; l += ctx.nthr) s[H * PITCH + l] = Qi[l];
         ctx.sync();
@@ -279,7 +286,7 @@ SAP_HD void zy_inv_body(Ctx& ctx, const ZyInvParams& p, float2* smem, int bx, in
             const int blk = t / H, pz = t - blk * H;
             float2 v[R1];
 #pragma unroll
-            for (int r = 0; r < R1; ++r) v[r] = Si[(size_t)(blk * R1 + r) * H + pz];
+            for (int r = 0; r < R1; ++r) v[r] = Si[(size_t)(blk * R1 + r) * H + kz_swz(pz, blk * R1 + r)];
             dft_inv<R1>(v);
 #pragma unroll
             for (int r = 0; r < R1; ++r) s[pz * PITCH + blk * R1 + r] = v[r];
