@@ -12,6 +12,7 @@
 #include "../../include/sap_dpsr.h"
 #include "dpsr_kernels.cuh"
 #include "ring_pass.cuh"
+#include "zline_pass.cuh"
 
 namespace sap {
 
@@ -442,7 +443,7 @@ template <int N> struct Runner {
         auto upd = [&](cudaError_t x) { if (e == cudaSuccess) e = x; };
         upd(set_smem(k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_SPLAT, C::NT_ZY>, zy_smem_bytes<N, C::NL>()));
         upd(set_smem(k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_GBAR, C::NT_ZY>, zy_smem_bytes<N, C::NL>()));
-        upd(set_smem(k_zy_inv<N, C::NL, C::FUSED_ZY, C::NT_ZY>, zy_smem_bytes<N, C::NL>()));
+        upd(set_smem(k_zl_inv<N>, zl_smem_bytes<N>()));
         upd(set_smem(k_ring<N, MODE_SOLVE>, ring_smem_bytes<N>()));
         upd(set_smem(k_ring<N, MODE_ADJ>, ring_smem_bytes<N>()));
         if constexpr (!C::FUSED_ZY) {
@@ -483,6 +484,15 @@ template <int N> struct Runner {
         launch_pdl(k_ring<N, MODE>, dim3((unsigned)grid), dim3(ring_threads<N>()), ring_smem_bytes<N>(), st, p);
     }
 
+    static void launch_zl_inv(sap_dpsr* h, cudaStream_t st, const float2* S, const float2* Q, float* out, int planes) {
+        using ZC = ZlCfg<N>;
+        ZlInvParams p{S, Q, out, h->tw, planes};
+        const long long total = (long long)planes * (N * N / ZC::NL);
+        long long grid = (long long)ZC::MINB * h->num_sms;
+        if (grid > total) grid = total;
+        launch_pdl(k_zl_inv<N>, dim3((unsigned)grid), dim3(zl_threads<N>()), zl_smem_bytes<N>(), st, p);
+    }
+
     static sap_status_t forward(sap_dpsr* h, const float* pts, const float* nrm, int P, float* chi, cudaStream_t st) {
         const int B = h->batch;
         const size_t V = (size_t)N * N * N;
@@ -517,8 +527,7 @@ template <int N> struct Runner {
         }
         // F4 (y +) z inverse -> chi'
         {
-            ZyInvParams p{h->S1, h->Q1, chi, h->tw};
-            launch_pdl(k_zy_inv<N, C::NL, C::FUSED_ZY, C::NT_ZY>, dim3(dim3(N * N / C::NL, B)), dim3(C::NT_ZY), zy_smem_bytes<N, C::NL>(), st, p);
+            launch_zl_inv(h, st, h->S1, h->Q1, chi, B);
             SAP_LAUNCH_CHECK(h, "k_zy_inv");
         }
         // F5 normalise
@@ -566,8 +575,7 @@ template <int N> struct Runner {
         }
         // B5 (y +) z inverse -> vbar (into the v workspace)
         {
-            ZyInvParams p{h->S3, h->Q3, h->v, h->tw};
-            launch_pdl(k_zy_inv<N, C::NL, C::FUSED_ZY, C::NT_ZY>, dim3(dim3(N * N / C::NL, B * 3)), dim3(C::NT_ZY), zy_smem_bytes<N, C::NL>(), st, p);
+            launch_zl_inv(h, st, h->S3, h->Q3, h->v, B * 3);
             SAP_LAUNCH_CHECK(h, "k_zy_inv");
         }
         // B6 gather
