@@ -43,16 +43,17 @@ KERNEL_BYTES_V = {
     "F:k_ring<FWD,y>": (0.0, 6.0, 6.0),          # row y sweep x3
     "F:k_ring<SOLVE>": (4.0, 4.0, 4.0),          # row x sweep + solve + x inverse (3V in, 1V out)
     "F:k_ring<INV,y>": (0.0, 2.0, 2.0),          # row inverse y
-    "F:k_zy_inv": (4.0, 2.0, 2.0),                  # rows [inverse y (2V) +] inverse z c2r (2V)
+    "F:k_zl_inv": (4.0, 2.0, 2.0),                  # rows [inverse y (2V) +] inverse z c2r (2V)
     "F:k_sample_mean": (0.0, 0.0, 0.0),
     "F:k_scale_shift": (2.0, 2.0, 2.0),             # row normalise
     # backward
     "B:k_reduce_g": (2.0, 2.0, 2.0),                # row reductions
+    "B:k_zl_gbar": (5.0, 3.0, 2.0),                 # the same pass as a persistent bulk-copy kernel (N <= 128)
     "B:k_zy_fwd<GBAR>": (5.0, 3.0, 2.0),            # rows z r2c (G+W in, 1 out = 3V) [+ y (2V)]; W is re-rasterised, not read
     "B:k_ring<FWD,y>": (0.0, 2.0, 2.0),
     "B:k_ring<ADJ>": (4.0, 4.0, 4.0),            # row x sweep + conj(M) fan-out + 3 x inverse
     "B:k_ring<INV,y>": (0.0, 6.0, 6.0),
-    "B:k_zy_inv": (12.0, 6.0, 6.0),                 # rows inverse y x3 + inverse z x3
+    "B:k_zl_inv": (12.0, 6.0, 6.0),                 # rows inverse y x3 + inverse z x3
     "B:k_gather_grads": (4.0, 4.0, 0.0),            # row gather (<= 4V, sparse)
 }
 

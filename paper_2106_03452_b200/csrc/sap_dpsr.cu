@@ -34,13 +34,6 @@ __global__ void __launch_bounds__(NT, zy_min_blocks<N>()) k_zy_fwd(ZyFwdParams p
     pdl_wait();
     zy_fwd_body<N, NL, DO_Y, SRC>(ctx, p, smem, (int)blockIdx.x, (int)blockIdx.y);
 }
-template <int N, int NL, bool DO_Y, int NT>
-__global__ void __launch_bounds__(NT, zy_min_blocks<N>()) k_zy_inv(ZyInvParams p) {
-    extern __shared__ float2 smem[];
-    DevCtx ctx{(int)threadIdx.x, NT};
-    pdl_wait();
-    zy_inv_body<N, NL, DO_Y>(ctx, p, smem, (int)blockIdx.x, (int)blockIdx.y);
-}
 
 // ------------------------------------------------------------------------------------------------
 // pointwise / point kernels
@@ -441,9 +434,10 @@ template <int N> struct Runner {
             e = cudaMemcpy(h->ftab, tab, sizeof(tab), cudaMemcpyHostToDevice);
         }
         auto upd = [&](cudaError_t x) { if (e == cudaSuccess) e = x; };
+        upd(set_smem(k_zl_inv<N>, zl_smem_bytes<N, true>()));
         upd(set_smem(k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_SPLAT, C::NT_ZY>, zy_smem_bytes<N, C::NL>()));
-        upd(set_smem(k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_GBAR, C::NT_ZY>, zy_smem_bytes<N, C::NL>()));
-        upd(set_smem(k_zl_inv<N>, zl_smem_bytes<N>()));
+        if constexpr (C::FUSED_ZY) upd(set_smem(k_zl_gbar<N>, zl_smem_bytes<N, false>()));
+        else upd(set_smem(k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_GBAR, C::NT_ZY>, zy_smem_bytes<N, C::NL>()));
         upd(set_smem(k_ring<N, MODE_SOLVE>, ring_smem_bytes<N>()));
         upd(set_smem(k_ring<N, MODE_ADJ>, ring_smem_bytes<N>()));
         if constexpr (!C::FUSED_ZY) {
@@ -484,13 +478,21 @@ template <int N> struct Runner {
         launch_pdl(k_ring<N, MODE>, dim3((unsigned)grid), dim3(ring_threads<N>()), ring_smem_bytes<N>(), st, p);
     }
 
+    static void launch_zl_gbar(sap_dpsr* h, cudaStream_t st, const ZyFwdParams& z, int planes) {
+        using ZC = ZlCfg<N, false>;
+        ZlFwdParams p{z, planes};
+        const long long total = (long long)planes * (N * N / ZC::NL);
+        long long grid = (long long)ZC::MINB * h->num_sms;
+        if (grid > total) grid = total;
+        launch_pdl(k_zl_gbar<N>, dim3((unsigned)grid), dim3(zl_threads<N, false>()), zl_smem_bytes<N, false>(), st, p);
+    }
     static void launch_zl_inv(sap_dpsr* h, cudaStream_t st, const float2* S, const float2* Q, float* out, int planes) {
-        using ZC = ZlCfg<N>;
+        using ZC = ZlCfg<N, true>;
         ZlInvParams p{S, Q, out, h->tw, planes};
         const long long total = (long long)planes * (N * N / ZC::NL);
         long long grid = (long long)ZC::MINB * h->num_sms;
         if (grid > total) grid = total;
-        launch_pdl(k_zl_inv<N>, dim3((unsigned)grid), dim3(zl_threads<N>()), zl_smem_bytes<N>(), st, p);
+        launch_pdl(k_zl_inv<N>, dim3((unsigned)grid), dim3(zl_threads<N, true>()), zl_smem_bytes<N, true>(), st, p);
     }
 
     static sap_status_t forward(sap_dpsr* h, const float* pts, const float* nrm, int P, float* chi, cudaStream_t st) {
@@ -511,7 +513,7 @@ template <int N> struct Runner {
         // F2 z (+y) forward, 3 channels
         {
             ZyFwdParams p{h->spts, h->snrm, h->bin_start, P, nullptr, nullptr, h->S3, C::FUSED_ZY ? h->Q3 : h->QT3, h->tw, 3};
-            launch_pdl(k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_SPLAT, C::NT_ZY>, dim3(dim3(N * N / C::NL, B * 3)), dim3(C::NT_ZY), zy_smem_bytes<N, C::NL>(), st, p);
+            launch_pdl(k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_SPLAT, C::NT_ZY>, dim3(N * N / C::NL, B * 3), dim3(C::NT_ZY), zy_smem_bytes<N, C::NL>(), st, p);
             SAP_LAUNCH_CHECK(h, "k_zy_fwd");
         }
         if constexpr (!C::FUSED_ZY) {
@@ -528,7 +530,7 @@ template <int N> struct Runner {
         // F4 (y +) z inverse -> chi'
         {
             launch_zl_inv(h, st, h->S1, h->Q1, chi, B);
-            SAP_LAUNCH_CHECK(h, "k_zy_inv");
+            SAP_LAUNCH_CHECK(h, "k_zl_inv");
         }
         // F5 normalise
         {
@@ -559,8 +561,9 @@ template <int N> struct Runner {
         // B2 + B3: Gbar' assembled on load, z (+y) forward
         {
             ZyFwdParams p{h->spts, h->snrm, h->bin_start, P, gchi, h->bw, h->S1, C::FUSED_ZY ? h->Q1 : h->QT1, h->tw, 1};
-            launch_pdl(k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_GBAR, C::NT_ZY>, dim3(dim3(N * N / C::NL, B)), dim3(C::NT_ZY), zy_smem_bytes<N, C::NL>(), st, p);
-            SAP_LAUNCH_CHECK(h, "k_zy_fwd<GBAR>");
+            if constexpr (C::FUSED_ZY) launch_zl_gbar(h, st, p, B);
+            else launch_pdl(k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_GBAR, C::NT_ZY>, dim3(N * N / C::NL, B), dim3(C::NT_ZY), zy_smem_bytes<N, C::NL>(), st, p);
+            SAP_LAUNCH_CHECK(h, C::FUSED_ZY ? "k_zl_gbar" : "k_zy_fwd<GBAR>");
         }
         if constexpr (!C::FUSED_ZY) {
             launch_ring<MODE_FWD>(h, st, B, h->mS1y, h->mQT1, h->S1, h->Q1, 1);
@@ -576,7 +579,7 @@ template <int N> struct Runner {
         // B5 (y +) z inverse -> vbar (into the v workspace)
         {
             launch_zl_inv(h, st, h->S3, h->Q3, h->v, B * 3);
-            SAP_LAUNCH_CHECK(h, "k_zy_inv");
+            SAP_LAUNCH_CHECK(h, "k_zl_inv");
         }
         // B6 gather
         launch_pdl(k_gather_grads, dim3(dim3((P + 127) / 128, B)), dim3(128), 0, st, pts, nrm, P, N, h->v, chi, h->bw, gp, gn);

@@ -13,9 +13,10 @@
 // A CTA owns a ring of NBUF tile buffers and NG consumer groups of NTC threads; groups take alternate tiles (one
 // computes while the other waits at a stage barrier or for its tile) and the thread that sees a buffer released
 // refills it at once with the tile NBUF items ahead, so loads are in flight during all of the arithmetic.
-//   k_zl_inv       spectrum -> real lines (F4 / B5)
-//   k_zl_fwd<GBAR> G (bulk-loaded) + re-rasterised W -> Gbar' -> spectrum (B2+B3)
-//   k_zl_fwd<SPLAT> points rasterised in shared memory -> spectrum (F1+F2); no loads, one buffer per group
+//   k_zl_inv   spectrum -> real lines (F4 / B5), every N
+//   k_zl_gbar  G (bulk-loaded) + re-rasterised W -> Gbar' -> spectrum (B2+B3), fused planes (N <= 128)
+// The splat pass (F1+F2) and the N >= 256 Gbar' pass stay one-tile-per-CTA kernels (zy_pass.cuh): they have little
+// or nothing to prefetch and measured faster with 3-4 small CTAs per SM than as a persistent ring.
 #pragma once
 #include "fft_core.cuh"
 #include "zy_pass.cuh"
@@ -23,20 +24,20 @@
 
 namespace sap {
 
-template <int N> struct ZlCfg {
+// INV: the inverse kernel (its tile size is free); the forward kernels tile the lines like the point bins (NL = 32)
+template <int N, bool INV> struct ZlCfg {
     static constexpr bool FUSED = (N <= 128);           // tile = whole plane, y transform fused
-    static constexpr int NL = FUSED ? N : 32;
+    static constexpr int NL = FUSED ? N : 32;            // zline_task needs NL % 32 == 0
     static constexpr int NTC = (N == 512) ? 512 : 256;  // threads per consumer group
     static constexpr int NG = (N == 128 || N == 256) ? 2 : 1;
-    // ring buffers (inverse and GBAR); SPLAT uses NG of them
-    static constexpr int NBUF = (N == 128) ? 3 : (N == 256) ? 6 : (N == 512) ? 3 : 2;
+    static constexpr int NBUF = (N == 128) ? 3 : (N == 256) ? 6 : (N == 512) ? 3 : 2;  // ring buffers
     static constexpr int MINB = (N == 64) ? 3 : (N == 32) ? 4 : 1;
 };
-template <int N> constexpr int zl_threads() { return ZlCfg<N>::NTC * ZlCfg<N>::NG; }
-template <int N> constexpr int zl_buf_elems() { return ZlCfg<N>::NL * (N / 2) + ZlCfg<N>::NL; }  // float2 per buffer
-template <int N> constexpr size_t zl_smem_bytes() {
-    return (size_t)ZlCfg<N>::NBUF * zl_buf_elems<N>() * sizeof(float2) + (size_t)N * sizeof(float2) +
-           2 * ZlCfg<N>::NBUF * sizeof(uint64_t) + 128;
+template <int N, bool INV> constexpr int zl_threads() { return ZlCfg<N, INV>::NTC * ZlCfg<N, INV>::NG; }
+template <int N, bool INV> constexpr int zl_buf_elems() { return ZlCfg<N, INV>::NL * (N / 2) + ZlCfg<N, INV>::NL; }  // float2 per buffer
+template <int N, bool INV> constexpr size_t zl_smem_bytes() {
+    return (size_t)ZlCfg<N, INV>::NBUF * zl_buf_elems<N, INV>() * sizeof(float2) + (size_t)N * sizeof(float2) +
+           2 * ZlCfg<N, INV>::NBUF * sizeof(uint64_t) + 128;
 }
 
 struct ZlInvParams {
@@ -128,16 +129,16 @@ namespace sap {
 
 // ring bookkeeping shared by the inverse and the GBAR kernels: item `it` of this CTA is tile blockIdx.x + it * gridDim.x
 // and lives in buffer it % NBUF (same protocol as k_ring, one item per tile)
-template <int N>
+template <int N, bool INV>
 struct ZlRing {
-    using C = ZlCfg<N>;
-    static constexpr int H = N / 2, NL = C::NL, NBUF = C::NBUF, NTC = C::NTC, BUF = zl_buf_elems<N>();
+    using C = ZlCfg<N, INV>;
+    static constexpr int H = N / 2, NL = C::NL, NBUF = C::NBUF, NTC = C::NTC, BUF = zl_buf_elems<N, INV>();
     float2* bufs;
     uint64_t* full;
     uint64_t* empty;
     long long total;
     const float2* srcS;  // tile g: NL*H complex at srcS + g*NL*H
-    const float2* srcQ;  // tile g: NL complex at srcQ + g*NL
+    const float2* srcQ;  // tile g: NL complex at srcQ + g*NL (nullptr: the tile has no Nyquist part, GBAR input)
     __device__ __forceinline__ void init() const {
         if (threadIdx.x == 0) {
             for (int s = 0; s < NBUF; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, NTC / 32); }
@@ -149,9 +150,9 @@ struct ZlRing {
         if (g >= total) return;
         const int s = it % NBUF;
         float2* b = bufs + (size_t)s * BUF;
-        mbar_expect_tx(full + s, (uint32_t)(BUF * sizeof(float2)));
+        mbar_expect_tx(full + s, (uint32_t)((srcQ ? BUF : NL * H) * sizeof(float2)));
         bulk_load(b, srcS + (size_t)g * NL * H, NL * H * sizeof(float2), full + s);
-        bulk_load(b + NL * H, srcQ + (size_t)g * NL, NL * sizeof(float2), full + s);
+        if (srcQ) bulk_load(b + NL * H, srcQ + (size_t)g * NL, NL * sizeof(float2), full + s);
     }
     __device__ __forceinline__ float2* acquire(int it) const {
         const int s = it % NBUF;
@@ -173,14 +174,14 @@ struct ZlRing {
 
 // ---- inverse: spectrum tile -> real lines ---------------------------------------------------------------------
 template <int N>
-__global__ void __launch_bounds__(zl_threads<N>(), ZlCfg<N>::MINB) k_zl_inv(const ZlInvParams p) {
-    using C = ZlCfg<N>;
-    constexpr int H = N / 2, NL = C::NL, NTC = C::NTC, NG = C::NG, NBUF = C::NBUF, BUF = zl_buf_elems<N>();
+__global__ void __launch_bounds__(zl_threads<N, true>(), ZlCfg<N, true>::MINB) k_zl_inv(const ZlInvParams p) {
+    using C = ZlCfg<N, true>;
+    constexpr int H = N / 2, NL = C::NL, NTC = C::NTC, NG = C::NG, NBUF = C::NBUF, BUF = zl_buf_elems<N, true>();
     constexpr bool FUSED = C::FUSED;
     constexpr int R0 = StageInfo<H, 0>::R, ST0 = StageInfo<H, 0>::ST;
-    static_assert(Plan<H>::NS <= 2 && ST0 <= 16, "z plans have at most two stages");
+    static_assert(Plan<H>::NS <= 2 && ST0 <= 16 && NL % 32 == 0, "z plans have at most two stages; line-group mapping");
     extern __shared__ __align__(1024) unsigned char zl_smem[];
-    ZlRing<N> ring;
+    ZlRing<N, true> ring;
     ring.bufs = reinterpret_cast<float2*>(zl_smem);
     float2* tw = ring.bufs + (size_t)NBUF * BUF;
     ring.full = reinterpret_cast<uint64_t*>(tw + N);
@@ -189,7 +190,7 @@ __global__ void __launch_bounds__(zl_threads<N>(), ZlCfg<N>::MINB) k_zl_inv(cons
     ring.srcS = p.S;
     ring.srcQ = p.Q;
     const int group = threadIdx.x / NTC, tid = threadIdx.x - group * NTC;
-    for (int i = threadIdx.x; i < N; i += zl_threads<N>()) tw[i] = p.tw[i];
+    for (int i = threadIdx.x; i < N; i += zl_threads<N, true>()) tw[i] = p.tw[i];
     ring.init();
     __syncthreads();
     pdl_wait();
@@ -273,6 +274,203 @@ __global__ void __launch_bounds__(zl_threads<N>(), ZlCfg<N>::MINB) k_zl_inv(cons
             bfly_inv<H, 0, N>(v, q, tw);
 #pragma unroll
             for (int r = 0; r < R0; ++r) out2[l * H + q + ST0 * r] = v[r];
+        }
+        ring.release((int)j, tid);
+    }
+}
+
+}  // namespace sap
+
+namespace sap {
+
+// ---- forward: real lines -> spectrum tile ----------------------------------------------------------------------
+// B2+B3: G is bulk-loaded into the tile, W = sum_i w is rasterised on top of it from the binned points (same
+// weights as the splat, Eq.10-11) scaled by (beta/P)/s, and the first stage multiplies by s:
+//   Gbar' = s (G + ((beta/P)/s) W) - (S1/a) delta_0.
+struct ZlFwdParams {
+    ZyFwdParams z;   // points, bins, G, bw, S, Q (N <= 128: [x][y]; N >= 256: transposed [y][x]), tw, nch
+    int planes;      // batch * nch
+};
+
+template <int N>
+__global__ void __launch_bounds__(zl_threads<N, false>(), ZlCfg<N, false>::MINB) k_zl_gbar(const ZlFwdParams pp) {
+    using C = ZlCfg<N, false>;
+    constexpr int H = N / 2, NL = C::NL, NTC = C::NTC, NG = C::NG, BUF = zl_buf_elems<N, false>();
+    constexpr int NBUF = C::NBUF;
+    constexpr bool FUSED = C::FUSED;
+    constexpr int R0 = StageInfo<H, 0>::R, ST0 = StageInfo<H, 0>::ST;
+    constexpr int TPP = N * N / NL;  // tiles per plane
+    constexpr int NTY = N / NL, NBINS = N * NTY, M = N - 1;
+    static_assert(Plan<H>::NS <= 2 && ST0 <= 16 && (NL * ST0) % 32 == 0, "z plan / line-group mapping");
+    const ZyFwdParams& p = pp.z;
+    extern __shared__ __align__(1024) unsigned char zl_smem[];
+    ZlRing<N, false> ring;
+    ring.bufs = reinterpret_cast<float2*>(zl_smem);
+    float2* tw = ring.bufs + (size_t)C::NBUF * BUF;
+    ring.full = reinterpret_cast<uint64_t*>(tw + N);
+    ring.empty = ring.full + C::NBUF;
+    ring.total = (long long)pp.planes * TPP;
+    ring.srcS = reinterpret_cast<const float2*>(p.G);  // GBAR: tile g = NL*N floats = NL*H float2 at G + g*NL*N
+    ring.srcQ = nullptr;
+    const int group = threadIdx.x / NTC, tid = threadIdx.x - group * NTC;
+    for (int i = threadIdx.x; i < N; i += zl_threads<N, false>()) tw[i] = p.tw[i];
+    ring.init();
+    __syncthreads();
+    pdl_wait();
+    if (threadIdx.x == 0) {
+#pragma unroll 1
+        for (int it = 0; it < NBUF; ++it) ring.issue_load(it);
+    }
+    for (long long j = group, g = blockIdx.x + (long long)group * gridDim.x; g < ring.total; j += NG, g += (long long)NG * gridDim.x) {
+        const int by = (int)(g / TPP), bx = (int)(g - (long long)by * TPP);
+        const int item = by / p.nch;
+        const int line0 = bx * NL, x = line0 / N, y0 = line0 - x * N, ty = y0 / NL;
+        float2* So = p.S + (size_t)g * NL * H;
+        // A0: bins that can touch lines [line0, line0 + NL): x-slabs {x, x-1} x y-tiles {ty, ty-1}
+        const int* bs = p.bin_start + (size_t)item * (NBINS + 1);
+        int b_lo[4], b_n[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const int xb = (k & 1) ? ((x - 1) & M) : x;
+            const int tb = (k & 2) ? ((ty + NTY - 1) % NTY) : ty;
+            const bool use = (NTY > 1) || !(k & 2);
+            const int bin = xb * NTY + tb;
+            b_lo[k] = use ? bs[bin] : 0;
+            b_n[k] = use ? bs[bin + 1] - b_lo[k] : 0;
+        }
+        float2* s = ring.acquire((int)j);
+        // A1: rasterise the points of the bins into the tile, natural order: float (l, z) at l*N + z
+        const float gs = p.bw[item * 4 + 0], wscale = p.bw[item * 4 + 1] / gs, gc0 = p.bw[item * 4 + 2];
+        {
+            float* sf = reinterpret_cast<float*>(s);
+            const float4* sp = p.spts + (size_t)item * p.P;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                for (int i = b_lo[k] + tid; i < b_lo[k] + b_n[k]; i += NTC) {
+                    const float4 c = sp[i];
+                    const float val = wscale;
+                    const float tx = c.x * (float)N, tyf = c.y * (float)N, tz = c.z * (float)N;
+                    const float fx0 = floorf(tx), fy0 = floorf(tyf), fz0 = floorf(tz);
+                    const int jx = (int)fx0, jy = (int)fy0, jz = (int)fz0;
+                    const float fx = tx - fx0, fy = tyf - fy0, fz = tz - fz0;
+#pragma unroll
+                    for (int dx = 0; dx < 2; ++dx) {
+                        if (((jx + dx) & M) != x) continue;
+                        const float wx = (dx ? fx : 1.f - fx) * val;
+#pragma unroll
+                        for (int dy = 0; dy < 2; ++dy) {
+                            const int ly = ((jy + dy) & M) - y0;
+                            if ((unsigned)ly >= (unsigned)NL) continue;
+                            const float wxy = wx * (dy ? fy : 1.f - fy);
+#pragma unroll
+                            for (int dz = 0; dz < 2; ++dz)
+                                atomicAdd(sf + ly * N + ((jz + dz) & M), wxy * (dz ? fz : 1.f - fz));
+                        }
+                    }
+                }
+            }
+        }
+        consumer_sync<NTC>(group);
+        // A2: z stage 0.  Reads the natural-order line, writes the swizzled slots: the ST0 butterflies of a line sit
+        // in one warp (zline_task), so a __syncwarp between its loads and its stores is all the ordering needed.
+        for (int t = tid; t < NL * ST0; t += NTC) {
+            int l, q;
+            zline_task<ST0>(t, l, q);
+            float2 v[R0];
+#pragma unroll
+            for (int r = 0; r < R0; ++r) {
+                float2 xv = cscale(gs, s[l * H + q + ST0 * r]);
+                if (line0 == 0 && l == 0 && q == 0 && r == 0) xv.x -= gc0;
+                v[r] = xv;
+            }
+            __syncwarp();
+            bfly_fwd<H, 0, N>(v, q, tw);
+#pragma unroll
+            for (int r = 0; r < R0; ++r) s[zi<H>(l, q + ST0 * r)] = v[r];
+        }
+        consumer_sync<NTC>(group);
+        if constexpr (Plan<H>::NS == 2) {
+            zl_stage_lines<N, NL, 1, false, NTC>(s, tw, tid);
+            consumer_sync<NTC>(group);
+        }
+        if constexpr (!FUSED) {
+            // C: Hermitian split in place, then the tile IS the HBM chunk: straight 16-byte copy out
+            zl_split<N, NL, false, NTC>(s, tw, tid);
+            consumer_sync<NTC>(group);
+            const float4* s4 = reinterpret_cast<const float4*>(s);
+            float4* So4 = reinterpret_cast<float4*>(So);
+            for (int i = tid; i < NL * H / 2; i += NTC) So4[i] = s4[i];
+            float2* Qt = p.Q + (size_t)by * ((size_t)N * N);  // transposed Nyquist plane [y][x]
+            for (int l = tid; l < NL; l += NTC) Qt[(size_t)(y0 + l) * N + x] = s[NL * H + l];
+        } else {
+            static_assert(!FUSED || Plan<N>::NS == 2, "fused planes use two-stage y plans");
+            // C: r2c split fused into y stage 0.  One task owns the slot pair (k, H-k) for RY y-values.
+            constexpr int RY = StageInfo<N, 0>::R, STY = StageInfo<N, 0>::ST;
+            for (int t = tid; t < (H / 2 + 1) * STY; t += NTC) {
+                const int k = t / STY, q = t - k * STY;
+                float2 a[RY], b[RY];
+                int ra, rb;
+                if (k == 0) {
+                    ra = 0; rb = H;
+#pragma unroll
+                    for (int r = 0; r < RY; ++r) {
+                        const float2 z = s[zi<H>(q + STY * r, 0)];
+                        a[r] = make_float2(z.x + z.y, 0.f);
+                        b[r] = make_float2(z.x - z.y, 0.f);
+                    }
+                } else if (k == H / 2) {
+                    ra = rb = freq2pos<H>(k);
+#pragma unroll
+                    for (int r = 0; r < RY; ++r) {
+                        const float2 z = s[zi<H>(q + STY * r, ra)];
+                        a[r] = make_float2(z.x, -z.y);
+                        b[r] = a[r];
+                    }
+                } else {
+                    ra = freq2pos<H>(k); rb = freq2pos<H>(H - k);
+                    const float2 w = tw[k];
+#pragma unroll
+                    for (int r = 0; r < RY; ++r) {
+                        a[r] = s[zi<H>(q + STY * r, ra)];
+                        b[r] = s[zi<H>(q + STY * r, rb)];
+                        r2c_pair(a[r], b[r], w);
+                    }
+                }
+                bfly_fwd<N, 0, N>(a, q, tw);
+#pragma unroll
+                for (int r = 0; r < RY; ++r) s[zi<H>(q + STY * r, ra)] = a[r];
+                if (rb != ra) {
+                    bfly_fwd<N, 0, N>(b, q, tw);
+#pragma unroll
+                    for (int r = 0; r < RY; ++r) {
+                        if (k == 0) s[NL * H + q + STY * r] = b[r];
+                        else s[zi<H>(q + STY * r, rb)] = b[r];
+                    }
+                }
+            }
+            consumer_sync<NTC>(group);
+            // D: last y stage smem -> registers -> HBM; lanes over z slots (the stored column of slot pz in row y is
+            // exactly its shared-memory column)
+            constexpr int R1 = StageInfo<N, 1>::R;
+            static_assert(StageInfo<N, 1>::ST == 1, "last stage");
+            for (int t = tid; t < H * (N / R1); t += NTC) {
+                const int blk = t / H, pz = t - blk * H;
+                float2 v[R1];
+#pragma unroll
+                for (int r = 0; r < R1; ++r) v[r] = s[zi<H>(blk * R1 + r, pz)];
+                dft_fwd<R1>(v);
+#pragma unroll
+                for (int r = 0; r < R1; ++r) So[zi<H>(blk * R1 + r, pz)] = v[r];
+            }
+            float2* Qo = p.Q + (size_t)by * ((size_t)N * N) + line0;
+            for (int blk = tid; blk < N / R1; blk += NTC) {
+                float2 v[R1];
+#pragma unroll
+                for (int r = 0; r < R1; ++r) v[r] = s[NL * H + blk * R1 + r];
+                dft_fwd<R1>(v);
+#pragma unroll
+                for (int r = 0; r < R1; ++r) Qo[blk * R1 + r] = v[r];
+            }
         }
         ring.release((int)j, tid);
     }

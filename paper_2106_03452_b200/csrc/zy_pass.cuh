@@ -1,4 +1,5 @@
-// zy_pass.cuh -- z (+ y) passes: real lines <-> half spectrum (F2/F4 and B3/B5 of SURVEY 8(a)).
+// zy_pass.cuh -- forward z (+ y) pass, one tile per CTA: real lines -> half spectrum (F1+F2, and B2+B3 for N >= 256).
+// (The inverse pass and the fused Gbar' pass are the persistent kernels of zline_pass.cuh.)
 //
 // One block owns NL z-lines (consecutive in memory, NL % 32 == 0).  With DO_Y (N <= 128) NL == N: the
 // block owns a whole x-plane and transforms along z and y in ONE trip through shared memory.
@@ -28,12 +29,6 @@ struct ZyFwdParams {
     float2* Q;             // [planes][N*N]  ([x][y] when the plane is fused (N <= 128), transposed [y][x] otherwise)
     const float2* tw;      // exp(-2 pi i t / N), t < N
     int nch;               // planes per batch item (3 for SPLAT, 1 for GBAR)
-};
-struct ZyInvParams {
-    const float2* S;
-    const float2* Q;
-    float* out;         // [planes][N^3]
-    const float2* tw;
 };
 
 // Column swizzle of the main spectrum in HBM: the value of z slot pz of line (x, y) is stored in column
@@ -251,109 +246,6 @@ SAP_HD void zy_fwd_body(Ctx& ctx, const ZyFwdParams& p, float2* smem, int bx, in
 #pragma unroll
             for (int r = 0; r < R1; ++r) Qo[blk * R1 + r] = v[r];
         }
-    }
-}
-
-// ---- inverse: mirror image -------------------------------------------------------------------------
-template <int N, int NL, bool DO_Y, class Ctx>
-SAP_HD void zy_inv_body(Ctx& ctx, const ZyInvParams& p, float2* smem, int bx, int by) {
-    constexpr int H = N / 2;
-    constexpr int PITCH = NL + 1;
-    constexpr int R0 = StageInfo<H, 0>::R, ST0 = StageInfo<H, 0>::ST;
-    static_assert(NL % 32 == 0 && ST0 <= 16, "line-group mapping");
-    float2* s = smem;
-    float2* tw = smem + (H + 1) * PITCH;
-    const size_t V = (size_t)N * N * N;
-    const size_t line0 = (size_t)bx * NL;
-    for (int i = ctx.tid; i < N; i += ctx.nthr) tw[i] = p.tw[i];
-    const float2* Si = p.S + (size_t)by * ((size_t)N * N * H) + line0 * H;
-    const float2* Qi = p.Q + (size_t)by * ((size_t)N * N) + line0;
-    if constexpr (!DO_Y) {
-        const int y0 = (int)(line0 % N);
-        for (int i = ctx.tid; i < NL * H; i += ctx.nthr) {
-            const int l = i / H, pc = i - l * H;
-            s[kz_swz(pc, y0 + l) * PITCH + l] = Si[i];
-        }
-        for (int l = ctx.tid; l < NL; l += ctx.nthr) s[H * PITCH + l] = Qi[l];
-        ctx.sync();
-        c2r_split<N, N>(ctx, s, PITCH, 1, NL, tw);
-        ctx.sync();
-    } else {
-        static_assert(!DO_Y || Plan<N>::NS == 2, "fused planes use two-stage y plans");
-        // D': global -> registers -> inverse of the last y stage -> smem; lanes over kz slots
-        constexpr int R1 = StageInfo<N, 1>::R;
-        for (int t = ctx.tid; t < H * (N / R1); t += ctx.nthr) {
-            const int blk = t / H, pz = t - blk * H;
-            float2 v[R1];
-#pragma unroll
-            for (int r = 0; r < R1; ++r) v[r] = Si[(size_t)(blk * R1 + r) * H + kz_swz(pz, blk * R1 + r)];
-            dft_inv<R1>(v);
-#pragma unroll
-            for (int r = 0; r < R1; ++r) s[pz * PITCH + blk * R1 + r] = v[r];
-        }
-        for (int blk = ctx.tid; blk < N / R1; blk += ctx.nthr) {
-            float2 v[R1];
-#pragma unroll
-            for (int r = 0; r < R1; ++r) v[r] = Qi[blk * R1 + r];
-            dft_inv<R1>(v);
-#pragma unroll
-            for (int r = 0; r < R1; ++r) s[H * PITCH + blk * R1 + r] = v[r];
-        }
-        ctx.sync();
-        // C': inverse y stage 0 on the row pair (k, H-k), then the c2r split, in registers
-        constexpr int RY = StageInfo<N, 0>::R, STY = StageInfo<N, 0>::ST;
-        for (int t = ctx.tid; t < (H / 2 + 1) * STY; t += ctx.nthr) {
-            const int k = t / STY, q = t - k * STY;
-            float2 a[RY], b[RY];
-            const int ra = (k == 0) ? 0 : freq2pos<H>(k);
-            const int rb = (k == 0) ? H : freq2pos<H>(H - k);
-#pragma unroll
-            for (int r = 0; r < RY; ++r) a[r] = s[ra * PITCH + q + STY * r];
-            bfly_inv<N, 0, N>(a, q, tw);
-            if (rb != ra) {
-#pragma unroll
-                for (int r = 0; r < RY; ++r) b[r] = s[rb * PITCH + q + STY * r];
-                bfly_inv<N, 0, N>(b, q, tw);
-            }
-            if (k == 0) {
-#pragma unroll
-                for (int r = 0; r < RY; ++r)
-                    s[q + STY * r] = make_float2(0.5f * (a[r].x + b[r].x), 0.5f * (a[r].x - b[r].x));
-            } else if (k == H / 2) {
-#pragma unroll
-                for (int r = 0; r < RY; ++r) s[ra * PITCH + q + STY * r] = make_float2(a[r].x, -a[r].y);
-            } else {
-                const float2 w = tw[k];
-#pragma unroll
-                for (int r = 0; r < RY; ++r) {
-                    c2r_pair(a[r], b[r], w);
-                    s[ra * PITCH + q + STY * r] = a[r];
-                    s[rb * PITCH + q + STY * r] = b[r];
-                }
-            }
-        }
-        ctx.sync();
-    }
-    // B': inverse z stages that stay in shared memory (last plan stage first)
-    if constexpr (Plan<H>::NS > 2) {
-        fft_stage<H, 2, true, N, true>(s, PITCH, 1, NL, tw, ctx.tid, ctx.nthr);
-        ctx.sync();
-    }
-    if constexpr (Plan<H>::NS > 1) {
-        fft_stage<H, 1, true, N, true>(s, PITCH, 1, NL, tw, ctx.tid, ctx.nthr);
-        ctx.sync();
-    }
-    // A': smem -> inverse z stage 0 (registers) -> global
-    float2* out2 = reinterpret_cast<float2*>(p.out + (size_t)by * V) + line0 * H;
-    for (int t = ctx.tid; t < NL * ST0; t += ctx.nthr) {
-        int l, q;
-        zline_task<ST0>(t, l, q);
-        float2 v[R0];
-#pragma unroll
-        for (int r = 0; r < R0; ++r) v[r] = s[(q + ST0 * r) * PITCH + l];
-        bfly_inv<H, 0, N>(v, q, tw);
-#pragma unroll
-        for (int r = 0; r < R0; ++r) out2[l * H + q + ST0 * r] = v[r];
     }
 }
 
