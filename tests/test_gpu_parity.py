@@ -92,6 +92,26 @@ def test_config4_256_parity_one_iteration():
     _check_item(cfg.N, cfg.sigma, pts[0], nrm[0], G[0], r["chi"][0], r["stats"][0], r["gp"][0], r["gn"][0])
 
 
+@pytest.mark.slow
+def test_config3_full_batch32_parity():
+    # BASELINE.json configs[2] at full size, the launch configuration bench.py times (batch 32 in one call)
+    cfg, pts, nrm = inputs.make_config(3)
+    G = inputs.upstream_grad(cfg.N, cfg.batch)
+    r = _gpu_run(cfg.N, cfg.sigma, pts, nrm, G)
+    for b in range(cfg.batch):
+        _check_item(cfg.N, cfg.sigma, pts[b], nrm[b], G[b], r["chi"][b], r["stats"][b], r["gp"][b], r["gn"][b])
+
+
+@pytest.mark.slow
+def test_config5_512_parity():
+    # BASELINE.json configs[4] at full size (512^3, 10^6 points), every voxel and every gradient against the naive
+    # float64 oracle (about 3.5 minutes of 16 host cores)
+    cfg, pts, nrm = inputs.make_config(5)
+    G = inputs.upstream_grad(cfg.N, 1)
+    r = _gpu_run(cfg.N, cfg.sigma, pts, nrm, G)
+    _check_item(cfg.N, cfg.sigma, pts[0], nrm[0], G[0], r["chi"][0], r["stats"][0], r["gp"][0], r["gn"][0])
+
+
 def test_repeatable_and_handle_reuse():
     import torch
     from paper_2106_03452_b200.binding import Dpsr
