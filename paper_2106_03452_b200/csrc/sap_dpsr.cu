@@ -123,7 +123,7 @@ __global__ void k_bin_scatter(const float* __restrict__ pts, const float* __rest
     const float* c = pts + ((size_t)b * P + i) * 3;
     const float* n = nrm + ((size_t)b * P + i) * 3;
     const int pos = atomicAdd(cursor + (size_t)b * nbins + bin_key(c, N, NL), 1);
-    spts[(size_t)b * P + pos] = make_float4(c[0], c[1], c[2], 0.f);
+    spts[(size_t)b * P + pos] = make_float4(c[0], c[1], c[2], __int_as_float(i));  // .w: index in the caller's order
     snrm[(size_t)b * P + pos] = make_float4(n[0], n[1], n[2], 0.f);
 }
 
@@ -149,7 +149,8 @@ __device__ __forceinline__ float block_sum(float x, float* sh) {
 
 // F5a: mu = mean_i interp(chi', c_i); a = chi'[0,0,0] - mu; s = 0.5/|a| (Eq.4; R5, R11).
 // Partial sums go to a double accumulator; the last block of an item finalises stats = {mu, a, s, 0}.
-__global__ void k_sample_mean(const float* __restrict__ pts, int P, int N, const float* __restrict__ chi_p,
+// Walks the points in bin order (neighbours in memory are neighbours in space: the 8 gathers hit L1/L2).
+__global__ void k_sample_mean(const float4* __restrict__ spts, int P, int N, const float* __restrict__ chi_p,
                               double* __restrict__ acc, unsigned* __restrict__ ticket,
                               float* __restrict__ stats) {
     pdl_wait();
@@ -159,7 +160,9 @@ __global__ void k_sample_mean(const float* __restrict__ pts, int P, int N, const
     const float* g = chi_p + (size_t)b * V;
     float sum = 0.f;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < P; i += gridDim.x * blockDim.x) {
-        const Corner k = corner_of(pts + ((size_t)b * P + i) * 3, N);
+        const float4 c4 = __ldg(spts + (size_t)b * P + i);
+        const float cc[3] = {c4.x, c4.y, c4.z};
+        const Corner k = corner_of(cc, N);
         float s = 0.f;
 #pragma unroll
         for (int d = 0; d < 8; ++d) {
@@ -246,7 +249,9 @@ __global__ void k_reduce_g(const float4* __restrict__ G, const float4* __restric
 //     dL/dc_i[a] = sum_corners (dw/dc_a) (n_i . vbar[corner] + (beta/(P s)) chi[corner]),
 //     dw/dc_a = N (d_a ? +1 : -1) prod_{b != a} w_b   (adjoint of F1 and F5; the mu part of chi' = chi/s + mu
 //     cancels because sum_corners dw/dc_a = 0).
-__global__ void k_gather_grads(const float* __restrict__ pts, const float* __restrict__ nrm, int P, int N,
+//     Walks the points in bin order (spatial locality of the 32 gathers) and scatters the two gradients back to
+//     the caller's order through the index kept in spts.w.
+__global__ void k_gather_grads(const float4* __restrict__ spts, const float4* __restrict__ snrm, int P, int N,
                                const float* __restrict__ vbar, const float* __restrict__ chi,
                                const float* __restrict__ bw, float* __restrict__ gp, float* __restrict__ gn) {
     pdl_wait();
@@ -254,9 +259,11 @@ __global__ void k_gather_grads(const float* __restrict__ pts, const float* __res
     const int b = blockIdx.y;
     if (i >= P) return;
     const size_t V = (size_t)N * N * N;
-    const size_t o = ((size_t)b * P + i) * 3;
-    const Corner k = corner_of(pts + o, N);
-    const float n0 = nrm[o], n1 = nrm[o + 1], n2 = nrm[o + 2];
+    const float4 c4 = __ldg(spts + (size_t)b * P + i), n4 = __ldg(snrm + (size_t)b * P + i);
+    const size_t o = ((size_t)b * P + __float_as_int(c4.w)) * 3;
+    const float cc[3] = {c4.x, c4.y, c4.z};
+    const Corner k = corner_of(cc, N);
+    const float n0 = n4.x, n1 = n4.y, n2 = n4.z;
     const float cchi = bw[b * 4 + 3];
     const float* vb = vbar + (size_t)b * 3 * V;
     const float* cb = chi + (size_t)b * V;
@@ -535,7 +542,7 @@ template <int N> struct Runner {
         // F5 normalise
         {
             int nb = (P + 255) / 256; if (nb > 296) nb = 296;
-            launch_pdl(k_sample_mean, dim3(dim3(nb, B)), dim3(256), 0, st, pts, P, N, chi, h->acc, h->ticket, h->stats);
+            launch_pdl(k_sample_mean, dim3(dim3(nb, B)), dim3(256), 0, st, (const float4*)h->spts, P, N, (const float*)chi, h->acc, h->ticket, h->stats);
             SAP_LAUNCH_CHECK(h, "k_sample_mean");
             const size_t n4 = V / 4;
             int gb = (int)((n4 + 255) / 256); const int cap = (148 * 8 + B - 1) / B; if (gb > cap) gb = cap; if (gb < 1) gb = 1;
@@ -582,7 +589,7 @@ template <int N> struct Runner {
             SAP_LAUNCH_CHECK(h, "k_zl_inv");
         }
         // B6 gather
-        launch_pdl(k_gather_grads, dim3(dim3((P + 127) / 128, B)), dim3(128), 0, st, pts, nrm, P, N, h->v, chi, h->bw, gp, gn);
+        launch_pdl(k_gather_grads, dim3(dim3((P + 127) / 128, B)), dim3(128), 0, st, (const float4*)h->spts, (const float4*)h->snrm, P, N, (const float*)h->v, chi, (const float*)h->bw, gp, gn);
         SAP_LAUNCH_CHECK(h, "k_gather_grads");
         return SAP_OK;
     }
