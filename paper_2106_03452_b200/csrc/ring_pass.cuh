@@ -27,15 +27,18 @@ template <> struct RingCfg<64>  { static constexpr int W = 32, NTC = 256, NG = 1
 template <> struct RingCfg<128> { static constexpr int W = 16, NTC = 128, NG = 4, NSTAGE = 12, MINB = 1; };
 template <> struct RingCfg<256> { static constexpr int W = 16, NTC = 256, NG = 2, NSTAGE = 6, MINB = 1; };
 template <> struct RingCfg<512> { static constexpr int W = 16, NTC = 512, NG = 1, NSTAGE = 3, MINB = 1; };  // 64-byte rows (W = 8) measured 25% slower
-template <int N> constexpr int ring_threads() { return RingCfg<N>::NTC * RingCfg<N>::NG; }
+// per-mode overrides (same W: the TMA boxes are shared); none at present.  Measured and rejected at N = 128: the
+// solve with 3 groups and 13 buffers (4 spare for prefetch) was 7% slower than 4 groups and 12 buffers.
+template <int N, int MODE> struct RingCfgM : RingCfg<N> {};
+template <int N, int MODE> constexpr int ring_threads() { return RingCfgM<N, MODE>::NTC * RingCfgM<N, MODE>::NG; }
 
 // twiddle tables in shared memory: per stage with a stride > 1, ST x R entries [j][r] of float4 (see cmul4), one
 // table for the forward direction and one (conjugated) for the inverse
 template <int N> constexpr int ring_tw_entries() {
     return N + (Plan<N>::NS == 3 ? StageInfo<N, 1>::ST * StageInfo<N, 1>::R : 0);
 }
-template <int N> constexpr size_t ring_smem_bytes() {
-    using C = RingCfg<N>;
+template <int N, int MODE> constexpr size_t ring_smem_bytes() {
+    using C = RingCfgM<N, MODE>;
     return (size_t)C::NSTAGE * N * C::W * sizeof(float2) + 2 * (size_t)ring_tw_entries<N>() * sizeof(float4) +
            (size_t)N * sizeof(float4) + 2 * C::NSTAGE * sizeof(uint64_t) + 128;
 }
@@ -158,8 +161,8 @@ __device__ __forceinline__ void ring_stage0_inv_store(const float2* s, const flo
 namespace sap {
 
 template <int N, int MODE>
-__global__ void __launch_bounds__(ring_threads<N>(), RingCfg<N>::MINB) k_ring(const __grid_constant__ RingParams p) {
-    using C = RingCfg<N>;
+__global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MINB) k_ring(const __grid_constant__ RingParams p) {
+    using C = RingCfgM<N, MODE>;
     constexpr int W = C::W, NTC = C::NTC, NG = C::NG, NSTAGE = C::NSTAGE, H = N / 2;
     constexpr int AXIS = (MODE == MODE_FWD || MODE == MODE_INV) ? 1 : 0;  // y pass : x pass
     constexpr int NS = Plan<N>::NS, LS = NS - 1, RL = StageInfo<N, LS>::R;
@@ -186,7 +189,7 @@ __global__ void __launch_bounds__(ring_threads<N>(), RingCfg<N>::MINB) k_ring(co
     uint64_t* empty = full + NSTAGE;
     const int group = threadIdx.x / NTC, tid = threadIdx.x - group * NTC;
 
-    for (int i = threadIdx.x; i < TWE; i += ring_threads<N>()) {
+    for (int i = threadIdx.x; i < TWE; i += ring_threads<N, MODE>()) {
         int e;  // the entry is w_N^e
         if (i < N) { const int j = i / R0, r = i - j * R0; e = r * j; }
         else { const int k = i - N, j = k / R1, r = k - j * R1; e = r * j * R0; }
@@ -194,7 +197,7 @@ __global__ void __launch_bounds__(ring_threads<N>(), RingCfg<N>::MINB) k_ring(co
         tabF[i] = make_float4(w.x, w.y, -w.y, w.x);
         tabI[i] = make_float4(w.x, -w.y, w.y, w.x);
     }
-    for (int i = threadIdx.x; i < N; i += ring_threads<N>()) fx[i] = p.ftab[i];
+    for (int i = threadIdx.x; i < N; i += ring_threads<N, MODE>()) fx[i] = p.ftab[i];
     if (threadIdx.x == 0) {
         for (int s = 0; s < NSTAGE; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, NTC / 32); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");

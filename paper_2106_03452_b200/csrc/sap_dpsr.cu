@@ -445,11 +445,11 @@ template <int N> struct Runner {
         upd(set_smem(k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_SPLAT, C::NT_ZY>, zy_smem_bytes<N, C::NL>()));
         if constexpr (C::FUSED_ZY) upd(set_smem(k_zl_gbar<N>, zl_smem_bytes<N, false>()));
         else upd(set_smem(k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_GBAR, C::NT_ZY>, zy_smem_bytes<N, C::NL>()));
-        upd(set_smem(k_ring<N, MODE_SOLVE>, ring_smem_bytes<N>()));
-        upd(set_smem(k_ring<N, MODE_ADJ>, ring_smem_bytes<N>()));
+        upd(set_smem(k_ring<N, MODE_SOLVE>, ring_smem_bytes<N, MODE_SOLVE>()));
+        upd(set_smem(k_ring<N, MODE_ADJ>, ring_smem_bytes<N, MODE_ADJ>()));
         if constexpr (!C::FUSED_ZY) {
-            upd(set_smem(k_ring<N, MODE_FWD>, ring_smem_bytes<N>()));
-            upd(set_smem(k_ring<N, MODE_INV>, ring_smem_bytes<N>()));
+            upd(set_smem(k_ring<N, MODE_FWD>, ring_smem_bytes<N, MODE_FWD>()));
+            upd(set_smem(k_ring<N, MODE_INV>, ring_smem_bytes<N, MODE_INV>()));
         }
         if (!cuda_ok(h, e, "cudaFuncSetAttribute")) return SAP_ERR_CUDA;
         // TMA descriptors: tile = NB points along the pass axis x W contiguous kz (or y, Nyquist plane) slots
@@ -473,7 +473,7 @@ template <int N> struct Runner {
     template <int MODE>
     static void launch_ring(sap_dpsr* h, cudaStream_t st, int units, const CUtensorMap& mS, const CUtensorMap& mQ,
                             float2* outS, float2* outQ, int axis) {
-        using RC = RingCfg<N>;
+        using RC = RingCfgM<N, MODE>;
         RingParams p;
         p.mapS = mS; p.mapQ = mQ; p.outS = outS; p.outQ = outQ; p.tw = h->tw; p.ftab = h->ftab;
         (void)axis;
@@ -482,7 +482,7 @@ template <int N> struct Runner {
         const long long total = (long long)units * (N * (H / RC::W) + N / RC::W);
         long long grid = (long long)RC::MINB * h->num_sms;
         if (grid > total) grid = total;
-        launch_pdl(k_ring<N, MODE>, dim3((unsigned)grid), dim3(ring_threads<N>()), ring_smem_bytes<N>(), st, p);
+        launch_pdl(k_ring<N, MODE>, dim3((unsigned)grid), dim3(ring_threads<N, MODE>()), ring_smem_bytes<N, MODE>(), st, p);
     }
 
     static void launch_zl_gbar(sap_dpsr* h, cudaStream_t st, const ZyFwdParams& z, int planes) {

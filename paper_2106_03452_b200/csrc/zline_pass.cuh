@@ -27,10 +27,10 @@ namespace sap {
 // INV: the inverse kernel (its tile size is free); the forward kernels tile the lines like the point bins (NL = 32)
 template <int N, bool INV> struct ZlCfg {
     static constexpr bool FUSED = (N <= 128);           // tile = whole plane, y transform fused
-    static constexpr int NL = FUSED ? N : 32;            // zline_task needs NL % 32 == 0
-    static constexpr int NTC = (N == 512) ? 512 : 256;  // threads per consumer group
-    static constexpr int NG = (N == 128 || N == 256) ? 2 : 1;
-    static constexpr int NBUF = (N == 128) ? 3 : (N == 256) ? 6 : (N == 512) ? 3 : 2;  // ring buffers
+    static constexpr int NL = FUSED ? N : (N == 512 && INV) ? 16 : 32;
+    static constexpr int NTC = (N == 512 && !INV) ? 512 : 256;  // threads per consumer group
+    static constexpr int NG = (N == 128 || N == 256 || (N == 512 && INV)) ? 2 : 1;
+    static constexpr int NBUF = (N == 128) ? 3 : (N == 256) ? 6 : (N == 512) ? (INV ? 6 : 3) : 2;  // ring buffers
     static constexpr int MINB = (N == 64) ? 3 : (N == 32) ? 4 : 1;
 };
 template <int N, bool INV> constexpr int zl_threads() { return ZlCfg<N, INV>::NTC * ZlCfg<N, INV>::NG; }
@@ -179,7 +179,7 @@ __global__ void __launch_bounds__(zl_threads<N, true>(), ZlCfg<N, true>::MINB) k
     constexpr int H = N / 2, NL = C::NL, NTC = C::NTC, NG = C::NG, NBUF = C::NBUF, BUF = zl_buf_elems<N, true>();
     constexpr bool FUSED = C::FUSED;
     constexpr int R0 = StageInfo<H, 0>::R, ST0 = StageInfo<H, 0>::ST;
-    static_assert(Plan<H>::NS <= 2 && ST0 <= 16 && NL % 32 == 0, "z plans have at most two stages; line-group mapping");
+    static_assert(Plan<H>::NS <= 2 && ST0 <= 16 && (NL % 32 == 0 || ST0 == 16), "z plans have at most two stages; line-group mapping");
     extern __shared__ __align__(1024) unsigned char zl_smem[];
     ZlRing<N, true> ring;
     ring.bufs = reinterpret_cast<float2*>(zl_smem);
@@ -267,7 +267,8 @@ __global__ void __launch_bounds__(zl_threads<N, true>(), ZlCfg<N, true>::MINB) k
         float2* out2 = reinterpret_cast<float2*>(p.out) + (size_t)g * NL * H;
         for (int t = tid; t < NL * ST0; t += NTC) {
             int l, q;
-            zline_task<ST0>(t, l, q);
+            if constexpr (ST0 == 16) { l = t >> 4; q = t & 15; }  // 16 consecutive complex of a line per half-warp
+            else zline_task<ST0>(t, l, q);
             float2 v[R0];
 #pragma unroll
             for (int r = 0; r < R0; ++r) v[r] = s[zi<H>(l, q + ST0 * r)];
