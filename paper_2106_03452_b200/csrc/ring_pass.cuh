@@ -42,6 +42,10 @@ template <int N, int MODE> constexpr size_t ring_smem_bytes() {
     return (size_t)C::NSTAGE * N * C::W * sizeof(float2) + 2 * (size_t)ring_tw_entries<N>() * sizeof(float4) +
            (size_t)N * sizeof(float4) + 2 * C::NSTAGE * sizeof(uint64_t) + 128;
 }
+constexpr size_t SMEM_PER_CTA_MAX = 227 * 1024;  // sm_100a opt-in limit per CTA
+static_assert(ring_smem_bytes<32, MODE_SOLVE>() * 4 <= SMEM_PER_CTA_MAX + 4096 && ring_smem_bytes<64, MODE_SOLVE>() * 3 <= SMEM_PER_CTA_MAX &&
+              ring_smem_bytes<128, MODE_SOLVE>() <= SMEM_PER_CTA_MAX && ring_smem_bytes<256, MODE_SOLVE>() <= SMEM_PER_CTA_MAX &&
+              ring_smem_bytes<512, MODE_SOLVE>() <= SMEM_PER_CTA_MAX, "ring buffers + tables must fit the shared memory of an SM");
 template <int N> constexpr int ring_box_rows() { return N < 256 ? N : 256; }  // TMA box dimension limit
 
 struct RingParams {

@@ -40,6 +40,10 @@ template <int N, bool INV> constexpr size_t zl_smem_bytes() {
            2 * ZlCfg<N, INV>::NBUF * sizeof(uint64_t) + 128;
 }
 
+static_assert(zl_smem_bytes<128, true>() <= SMEM_PER_CTA_MAX && zl_smem_bytes<256, true>() <= SMEM_PER_CTA_MAX &&
+              zl_smem_bytes<512, true>() <= SMEM_PER_CTA_MAX && zl_smem_bytes<128, false>() <= SMEM_PER_CTA_MAX,
+              "tile ring must fit the shared memory of an SM");
+
 struct ZlInvParams {
     const float2* S;    // [planes][N][N][H] main spectrum (stored order, column swizzle)
     const float2* Q;    // [planes][N][N]   Nyquist plane [x][y]

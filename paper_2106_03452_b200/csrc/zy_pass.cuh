@@ -61,8 +61,6 @@ SAP_HD void zy_fwd_body(Ctx& ctx, const ZyFwdParams& p, float2* smem, int bx, in
     float2* tw = smem + (H + 1) * PITCH;
     const size_t V = (size_t)N * N * N;
     const size_t line0 = (size_t)bx * NL;  // global line index = x*N + y
-    for (int i = ctx.tid; i < N; i += ctx.nthr) tw[i] = p.tw[i];
-    ctx.sync();
 
     float2* So = p.S + (size_t)by * ((size_t)N * N * H) + line0 * H;
     float2* Qo = p.Q + (size_t)by * ((size_t)N * N) + line0;
@@ -82,6 +80,10 @@ SAP_HD void zy_fwd_body(Ctx& ctx, const ZyFwdParams& p, float2* smem, int bx, in
         b_n[k] = use ? bs[bin + 1] - b_lo[k] : 0;
         total += b_n[k];
     }
+    // A1: zero the plane, rasterise the points into it (shared-memory atomics), z = 2m + parity
+    // (the bin offsets above are in flight while the twiddles are fetched and the plane is cleared)
+    for (int i = ctx.tid; i < N; i += ctx.nthr) tw[i] = p.tw[i];
+    for (int i = ctx.tid; i < H * PITCH; i += ctx.nthr) s[i] = make_float2(0.f, 0.f);
     if (SRC == SRC_SPLAT && total == 0) {  // nothing lands here: the spectrum of zeros is zeros
         for (int i = ctx.tid; i < NL * H; i += ctx.nthr) So[i] = make_float2(0.f, 0.f);
         if constexpr (DO_Y) {
@@ -92,8 +94,6 @@ SAP_HD void zy_fwd_body(Ctx& ctx, const ZyFwdParams& p, float2* smem, int bx, in
         }
         return;
     }
-    // A1: zero the plane, rasterise the points into it (shared-memory atomics), z = 2m + parity
-    for (int i = ctx.tid; i < H * PITCH; i += ctx.nthr) s[i] = make_float2(0.f, 0.f);
     ctx.sync();
     {
         float* sf = reinterpret_cast<float*>(s);
