@@ -58,6 +58,24 @@ KERNEL_BYTES_V = {
 }
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the `ncu --set full` captures summarised under
+# profiles/r01_full_cfg{2,3,4}.md (one forward+backward each, kernels in launch order).  At 128^3 batch 1 the working
+# set (~50 MB) lives in the 126 MB L2, so DRAM traffic is far BELOW the algorithmic bytes there.
+NCU_TRAFFIC = {
+    "cfg2_torus_128": {"F:k_bin_count": 244736, "F:k_bin_scan": 9216, "F:k_bin_scatter": 484864, "F:k_zy_fwd": 667392,
+                       "F:k_ring<SOLVE>": 25602816, "F:k_zl_inv": 8541952, "F:k_sample_mean": 2118656, "F:k_scale_shift": 8391936,
+                       "B:k_reduce_g": 16787200, "B:k_zl_gbar": 8739328, "B:k_ring<ADJ>": 8561920, "B:k_zl_inv": 25627648,
+                       "B:k_gather_grads": 7804416},
+    "cfg3_ellipsoids_128_b32": {"F:k_zy_fwd": 774172928, "F:k_ring<SOLVE>": 1064461568, "F:k_zl_inv": 490159872,
+                                "F:k_scale_shift": 479321088, "B:k_reduce_g": 540407040, "B:k_zl_gbar": 494904576,
+                                "B:k_ring<ADJ>": 1032813568, "B:k_zl_inv": 1572671488},
+    "cfg4_ellipsoids_256": {"F:k_zy_fwd": 147823872, "F:k_ring<FWD,y>": 348254464, "F:k_ring<SOLVE>": 242811136,
+                            "F:k_ring<INV,y>": 77978624, "F:k_zl_inv": 81739520, "F:k_scale_shift": 76141056,
+                            "B:k_reduce_g": 137704192, "B:k_zy_fwd<GBAR>": 91645440, "B:k_ring<FWD,y>": 78107648,
+                            "B:k_ring<ADJ>": 211087104, "B:k_ring<INV,y>": 348298752, "B:k_zl_inv": 352476928},
+}
+
+
 def read_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -258,7 +276,8 @@ def roofline_of(res, peak_gbs):
     ach = yard_v * V / (km[name] * 1e-3) / 1e9
     comp = comp_v * V / (km[name] * 1e-3) / 1e9
     return {"bound": "hbm", "kernel": name, "kernel_ms": km[name], "share_of_step": km[name] / sum(km.values()),
-            "achieved": ach, "peak": peak_gbs, "unit": "GB/s", "frac": ach / peak_gbs, "traffic": None,
+            "achieved": ach, "peak": peak_gbs, "unit": "GB/s", "frac": ach / peak_gbs,
+            "traffic": NCU_TRAFFIC.get(cfg.name, {}).get(name),
             "algorithmic_bytes": yard_v * V, "achieved_compulsory": comp, "frac_compulsory": comp / peak_gbs,
             "compulsory_bytes": comp_v * V}
 
