@@ -1,15 +1,20 @@
-// dpsr_kernels.cuh -- block bodies of the FFT / spectral-solve kernels of the DPSR path.
+// dpsr_kernels.cuh -- the FFT / spectral-solve kernels of the DPSR path.
 //
-// Data layout in HBM (per batch item, per channel), H = N/2:
+// Data layout in HBM (per batch item, per channel), H = N/2 (DESIGN.md section 6):
 //   real grids      float  [N][N][N]            x slowest, z fastest (the C-ABI layout)
-//   main spectrum   float2 [N][N][H]            slots (px, py, pz) in *stored order* on every axis
-//   Nyquist plane   float2 [N][N]               the kz = N/2 column of every z-line, slots (px, py)
+//   main spectrum   float2 [N][N][H]            slots (px, py, pz) in *stored order* on every axis, the z slot
+//                                               of line (x, y) kept in column pz ^ (y & 15) (kz_swz)
+//   Nyquist plane   float2 [N][N]               the kz = N/2 column of every z-line, slots (px, py);
+//                                               N >= 256 also keeps a transposed copy [py][px] between passes
 // "Stored order": slot p of an axis holds frequency pos2freq<len>(p) (fft_core.cuh); x and y are
 // length-N complex transforms, z is a real transform done as an H-point complex FFT + split.
 //
-// Bodies are templates over a context (thread id, thread count, barrier) so the same source can be
-// stepped on the host by a debugging harness; the library only instantiates them with DevCtx.
+//   zy_pass.cuh     splat + forward z (+ y) pass, one tile per CTA
+//   zline_pass.cuh  persistent bulk-copy z (+ y) passes: inverse, fused Gbar'
+//   ring_pass.cuh   persistent TMA ring: x pass with the fused spectral solve / its adjoint, y pass (N >= 256)
 #pragma once
 #include "fft_core.cuh"
-#include "zy_pass.cuh"
 #include "spectral.cuh"
+#include "zy_pass.cuh"
+#include "ring_pass.cuh"
+#include "zline_pass.cuh"

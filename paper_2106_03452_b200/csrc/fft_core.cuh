@@ -8,8 +8,8 @@
 // all the synchronisation there is.  Spectra are kept in stored order in HBM on all three axes; only
 // the spectral solve needs to know which frequency a slot holds (pos2freq).
 //
-// The functions are __host__ __device__ so that the same source can be exercised thread-by-thread
-// by a host harness; the product only ever runs them on the device.
+// Most functions are __host__ __device__ (plain arithmetic; the host uses pos2freq to build the frequency
+// table of the solve); the product only ever runs the butterflies on the device.
 #pragma once
 #include <cuda_runtime.h>
 
@@ -255,36 +255,6 @@ SAP_HD void fft_stage(float2* s, int ES, int LS, int nlines, const float2* tw, i
     }
 }
 
-// Whole transform of `nlines` lines: all stages with a barrier after each.
-// Forward: stages 0..NS-1 (DIF).  Inverse: stages NS-1..0 (DIT).
-template <int N, bool INV, int TWN, bool LANES_LINES, class Ctx>
-SAP_HD void fft_lines(Ctx& ctx, float2* s, int ES, int LS, int nlines, const float2* tw) {
-    constexpr int NS = Plan<N>::NS;
-    if (!INV) {
-        fft_stage<N, 0, false, TWN, LANES_LINES>(s, ES, LS, nlines, tw, ctx.tid, ctx.nthr);
-        ctx.sync();
-        if constexpr (NS > 1) {
-            fft_stage<N, 1, false, TWN, LANES_LINES>(s, ES, LS, nlines, tw, ctx.tid, ctx.nthr);
-            ctx.sync();
-        }
-        if constexpr (NS > 2) {
-            fft_stage<N, 2, false, TWN, LANES_LINES>(s, ES, LS, nlines, tw, ctx.tid, ctx.nthr);
-            ctx.sync();
-        }
-    } else {
-        if constexpr (NS > 2) {
-            fft_stage<N, 2, true, TWN, LANES_LINES>(s, ES, LS, nlines, tw, ctx.tid, ctx.nthr);
-            ctx.sync();
-        }
-        if constexpr (NS > 1) {
-            fft_stage<N, 1, true, TWN, LANES_LINES>(s, ES, LS, nlines, tw, ctx.tid, ctx.nthr);
-            ctx.sync();
-        }
-        fft_stage<N, 0, true, TWN, LANES_LINES>(s, ES, LS, nlines, tw, ctx.tid, ctx.nthr);
-        ctx.sync();
-    }
-}
-
 // ---- real <-> half-complex split for a length-N real line done as an H = N/2 point complex FFT --
 // After the forward H-point FFT, slot pos(k) holds Z[k] = E[k] + i O[k] (E, O = DFTs of the even and
 // odd samples).  X[k] = E[k] + w^k O[k], w = exp(-2 pi i / N), k = 0..H.  In place: X[k] goes to slot
@@ -318,39 +288,6 @@ SAP_HD void r2c_split(Ctx& ctx, float2* s, int RS, int LS, int nlines, const flo
             *pa = csub(e, f);                     // X[k]   = E - F
             float2 g = cadd(e, f);
             *pb = make_float2(g.x, -g.y);         // X[H-k] = conj(E + F)
-        }
-    }
-}
-
-// Inverse of r2c_split: from X[k] (slot pos(k), k < H; X[H] in row H) rebuild Z[k] = E[k] + i O[k] in
-// place.  The unnormalised inverse H-point FFT of Z then gives (N/2) * (x[2m] + i x[2m+1]).
-template <int N, int TWN, class Ctx>
-SAP_HD void c2r_split(Ctx& ctx, float2* s, int RS, int LS, int nlines, const float2* tw) {
-    constexpr int H = N / 2;
-    constexpr int TWMUL = TWN / N;
-    const int ntasks = nlines * (H / 2 + 1);
-    for (int t = ctx.tid; t < ntasks; t += ctx.nthr) {
-        const int k = t / nlines;
-        const int line = t - k * nlines;
-        float2* col = s + line * LS;
-        if (k == 0) {
-            float x0 = col[0].x, xh = col[H * RS].x;
-            col[0] = make_float2(0.5f * (x0 + xh), 0.5f * (x0 - xh));
-        } else if (k == H / 2) {
-            float2* p = col + freq2pos<H>(k) * RS;
-            float2 x = *p;
-            *p = make_float2(x.x, -x.y);
-        } else {
-            float2* pa = col + freq2pos<H>(k) * RS;
-            float2* pb = col + freq2pos<H>(H - k) * RS;
-            float2 a = *pa, b = *pb;                                         // X[k], X[H-k]
-            float2 e = make_float2(0.5f * (a.x + b.x), 0.5f * (a.y - b.y));  // E = (X[k] + conj X[H-k])/2
-            float2 d = make_float2(0.5f * (a.x - b.x), 0.5f * (a.y + b.y));  // w^k O = (X[k] - conj X[H-k])/2
-            float2 o = cmulc(d, tw[k * TWMUL]);                              // O = conj(w^k) * d
-            float2 io = make_float2(-o.y, o.x);                              // i O
-            *pa = cadd(e, io);                                               // Z[k]   = E + i O
-            float2 g = csub(e, io);
-            *pb = make_float2(g.x, -g.y);                                    // Z[H-k] = conj(E - i O)
         }
     }
 }

@@ -11,8 +11,6 @@
 
 #include "../../include/sap_dpsr.h"
 #include "dpsr_kernels.cuh"
-#include "ring_pass.cuh"
-#include "zline_pass.cuh"
 
 namespace sap {
 

@@ -5,7 +5,7 @@
 // block owns a whole x-plane and transforms along z and y in ONE trip through shared memory.
 // Shared-memory traffic is kept to ~6 passes per plane: the first z stage runs global -> registers ->
 // smem, the r2c split is fused into the first y stage, and the last y stage runs smem -> registers ->
-// global (and the mirror image for the inverse).
+// global.
 // smem: (H+1) rows (kz slots + Nyquist) x PITCH = NL+1 columns (lines); PITCH == 1 (mod 16).
 #pragma once
 #include "fft_core.cuh"
@@ -19,7 +19,7 @@ namespace sap {
 // Points are pre-sorted by bin key j0x * (N/NL) + j0y / NL (k_bin_* kernels); bin_start has NBINS+1 entries.
 enum { SRC_SPLAT = 0, SRC_GBAR = 1 };
 struct ZyFwdParams {
-    const float4* spts;    // [batch][P] sorted points  {cx, cy, cz, -}
+    const float4* spts;    // [batch][P] sorted points  {cx, cy, cz, index in the caller's order (int bits)}
     const float4* snrm;    // [batch][P] sorted normals {nx, ny, nz, -}
     const int* bin_start;  // [batch][NBINS + 1]
     int P;
