@@ -265,6 +265,34 @@ def time_config(cfg_id, steps, warmup, rank, torch, flush, with_e2e=True, with_p
     return res
 
 
+def time_fused_mse(cfg_id, steps, warmup, torch, flush):
+    """Learning-based setting (Eq.9): forward with the loss fused into the normalisation pass + backward from the
+    gradient kept inside the handle (sap_dpsr_forward_mse / sap_dpsr_backward_mse); per grid, device-resident."""
+    from paper_2106_03452_b200.binding import Dpsr
+    cfg, pts, nrm, G = make_device_inputs(cfg_id, 0, torch)
+    B, N, P = cfg.batch, cfg.N, cfg.P
+    h = Dpsr(N, cfg.sigma, B, P)
+    d_pts, d_nrm = torch.from_numpy(pts).cuda(), torch.from_numpy(nrm).cuda()
+    d_gt = torch.from_numpy(np.tanh(G).astype(np.float32) * 0.5).cuda()
+    chi = torch.empty((B, N, N, N), dtype=torch.float32, device="cuda")
+    loss = torch.empty((B,), dtype=torch.float32, device="cuda")
+    gp, gn = torch.empty_like(d_pts), torch.empty_like(d_nrm)
+    stream = torch.cuda.current_stream()
+    tot = 0.0
+    for i in range(warmup + steps):
+        flush.zero_()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        h.forward_mse(d_pts, d_nrm, d_gt, chi, loss, stream)
+        h.backward_mse(d_pts, d_nrm, chi, gp, gn, stream)
+        b.record(stream)
+        torch.cuda.synchronize()
+        if i >= warmup:
+            tot += a.elapsed_time(b)
+    h.close()
+    return {"ms_per_grid": tot / steps / B, "steps": steps, "what": "forward_mse + backward_mse (loss and dL/dchi never leave the handle)"}
+
+
 def roofline_of(res, peak_gbs):
     """Dominant kernel of the step and its achieved bandwidth on the SURVEY 8(d) yardstick bytes."""
     cfg = res["cfg"]
@@ -368,6 +396,8 @@ def main():
                             "path_frac_52V": YARD_FWD_BWD_V * Vc / (per_grid * 1e-3) / 1e9 / peak,
                             "roofline": roofline_of(r, peak), "kernels_ms": r["kernels_ms"]}
         line["also"] = also
+    if rank == 0 and world == 1 and args.also and "3" in args.also.split(","):
+        line["also"]["cfg3_fused_mse_loss"] = time_fused_mse(3, 10, 3, torch, flush)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         from oracle import dpsr_oracle as orc
         from paper_2106_03452_b200 import inputs

@@ -81,6 +81,24 @@ sap_status_t sap_dpsr_backward(sap_dpsr_t* h, const float* points, const float* 
                                float* grad_points, float* grad_normals, void* stream);
 
 /*
+ * Learning-based setting (Sec.3.3, Eq.9): L_DPSR = || chi - chi_gt ||^2, one value per item.
+ * sap_dpsr_forward_mse is sap_dpsr_forward whose normalisation pass also evaluates the loss and its gradient
+ * G = dL/dchi = 2 (chi - chi_gt) together with the grid reductions of the backward; G stays inside the handle
+ * (one more N^3 grid per item, allocated on first use), so it never makes a round trip through the caller.
+ *   chi_gt  dev [batch][N][N][N] float   target indicator grid
+ *   chi     dev [batch][N][N][N] float   overwritten with the prediction (needed by the backward)
+ *   loss    dev [batch] float            overwritten with the squared L2 distance of each item
+ * sap_dpsr_backward_mse returns dL/dpoints and dL/dnormals of that loss; it must follow, on the same handle, the
+ * sap_dpsr_forward_mse it differentiates, with the same points/normals and that call's chi, unmodified.
+ */
+sap_status_t sap_dpsr_forward_mse(sap_dpsr_t* h, const float* points, const float* normals,
+                                  int num_points, const float* chi_gt, float* chi, float* loss,
+                                  void* stream);
+sap_status_t sap_dpsr_backward_mse(sap_dpsr_t* h, const float* points, const float* normals,
+                                   int num_points, const float* chi, float* grad_points,
+                                   float* grad_normals, void* stream);
+
+/*
  * Host-buffer variants (the end-to-end path): the same computation with HOST pointers.  Inputs are
  * copied to handle-owned device staging buffers with cudaMemcpyAsync on `stream`, the kernels run,
  * and the outputs are copied back; the call returns after synchronising `stream`.

@@ -13,7 +13,7 @@ SAP_OK, SAP_ERR_INVALID_ARG, SAP_ERR_UNSUPPORTED, SAP_ERR_OOM, SAP_ERR_CUDA = ra
 STATUS_NAMES = {0: "SAP_OK", 1: "SAP_ERR_INVALID_ARG", 2: "SAP_ERR_UNSUPPORTED", 3: "SAP_ERR_OOM", 4: "SAP_ERR_CUDA"}
 
 EXPORTS = [
-    "sap_dpsr_create", "sap_dpsr_forward", "sap_dpsr_backward", "sap_dpsr_forward_host",
+    "sap_dpsr_create", "sap_dpsr_forward", "sap_dpsr_backward", "sap_dpsr_forward_mse", "sap_dpsr_backward_mse", "sap_dpsr_forward_host",
     "sap_dpsr_backward_host", "sap_dpsr_get_stats", "sap_dpsr_destroy", "sap_dpsr_last_error",
     "sap_dpsr_workspace_bytes", "sap_dpsr_last_launch_count", "sap_dpsr_set_profiling", "sap_dpsr_get_profile",
 ]
@@ -44,6 +44,10 @@ def lib():
     L.sap_dpsr_forward.restype = ci
     L.sap_dpsr_backward.argtypes = [vp, vp, vp, ci, vp, vp, vp, vp, vp]
     L.sap_dpsr_backward.restype = ci
+    L.sap_dpsr_forward_mse.argtypes = [vp, vp, vp, ci, vp, vp, vp, vp]
+    L.sap_dpsr_forward_mse.restype = ci
+    L.sap_dpsr_backward_mse.argtypes = [vp, vp, vp, ci, vp, vp, vp, vp]
+    L.sap_dpsr_backward_mse.restype = ci
     L.sap_dpsr_forward_host.argtypes = [vp, vp, vp, ci, vp, vp]
     L.sap_dpsr_forward_host.restype = ci
     L.sap_dpsr_backward_host.argtypes = [vp, vp, vp, vp, vp]
@@ -120,6 +124,36 @@ class Dpsr:
             self._dev(chi, (B, N, N, N), "chi"), self._dev(grad_chi, (B, N, N, N), "grad_chi"),
             self._dev(grad_points, (B, P, 3), "grad_points"), self._dev(grad_normals, (B, P, 3), "grad_normals"),
             _stream_ptr(stream)))
+        return grad_points, grad_normals
+
+    def forward_mse(self, points, normals, chi_gt, chi=None, loss=None, stream=None):
+        """Forward with the fused loss of Eq.9: returns (chi [batch,N,N,N], loss [batch] = ||chi - chi_gt||^2)."""
+        import torch
+        B, N = self.batch, self.N
+        P = int(points.shape[1])
+        if chi is None:
+            chi = torch.empty((B, N, N, N), dtype=torch.float32, device=points.device)
+        if loss is None:
+            loss = torch.empty((B,), dtype=torch.float32, device=points.device)
+        self._check(lib().sap_dpsr_forward_mse(
+            self._h, self._dev(points, (B, P, 3), "points"), self._dev(normals, (B, P, 3), "normals"), P,
+            self._dev(chi_gt, (B, N, N, N), "chi_gt"), self._dev(chi, (B, N, N, N), "chi"), self._dev(loss, (B,), "loss"),
+            _stream_ptr(stream)))
+        return chi, loss
+
+    def backward_mse(self, points, normals, chi, grad_points=None, grad_normals=None, stream=None):
+        """Gradients of the loss of the preceding forward_mse (dL/dchi is kept inside the handle)."""
+        import torch
+        B, N = self.batch, self.N
+        P = int(points.shape[1])
+        if grad_points is None:
+            grad_points = torch.empty_like(points)
+        if grad_normals is None:
+            grad_normals = torch.empty_like(normals)
+        self._check(lib().sap_dpsr_backward_mse(
+            self._h, self._dev(points, (B, P, 3), "points"), self._dev(normals, (B, P, 3), "normals"), P,
+            self._dev(chi, (B, N, N, N), "chi"), self._dev(grad_points, (B, P, 3), "grad_points"),
+            self._dev(grad_normals, (B, P, 3), "grad_normals"), _stream_ptr(stream)))
         return grad_points, grad_normals
 
     @staticmethod

@@ -204,6 +204,58 @@ __global__ void k_scale_shift(float4* __restrict__ chi, size_t n4_per_item, cons
     }
 }
 
+// F5b fused with the loss of the learning-based setting (Eq.9): L = || chi - chi_gt ||^2.  The same
+// pass writes chi = s (chi' - mu), the upstream gradient G = dL/dchi = 2 (chi - chi_gt) and accumulates L together
+// with the reductions S0 = sum G, S1 = sum G chi of the backward (B1), so G never makes a round trip through the
+// caller and k_reduce_g is not needed.  The last block writes loss[b] and bw = {s, beta/P, S1/a, beta/(P s)}.
+__global__ void k_scale_shift_mse(float4* __restrict__ chi, const float4* __restrict__ chi_gt, float4* __restrict__ G,
+                                  size_t n4_per_item, int P, const float* __restrict__ stats, double* __restrict__ acc,
+                                  unsigned* __restrict__ ticket, float* __restrict__ bw, float* __restrict__ loss) {
+    pdl_wait();
+    __shared__ float sh[32];
+    const int b = blockIdx.y;
+    const float mu = stats[b * 4 + 0], s = stats[b * 4 + 2];
+    float4* c = chi + (size_t)b * n4_per_item;
+    const float4* t = chi_gt + (size_t)b * n4_per_item;
+    float4* g = G + (size_t)b * n4_per_item;
+    float s0 = 0.f, s1 = 0.f, l = 0.f;
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4_per_item; i += stride) {
+        float4 v = c[i];
+        const float4 w = t[i];
+        v.x = s * (v.x - mu); v.y = s * (v.y - mu); v.z = s * (v.z - mu); v.w = s * (v.w - mu);
+        const float4 d = make_float4(v.x - w.x, v.y - w.y, v.z - w.z, v.w - w.w);
+        const float4 gg = make_float4(2.f * d.x, 2.f * d.y, 2.f * d.z, 2.f * d.w);
+        c[i] = v;
+        g[i] = gg;
+        l += (d.x * d.x + d.y * d.y) + (d.z * d.z + d.w * d.w);
+        s0 += (gg.x + gg.y) + (gg.z + gg.w);
+        s1 += (gg.x * v.x + gg.y * v.y) + (gg.z * v.z + gg.w * v.w);
+    }
+    const float b0 = block_sum(s0, sh);
+    const float b1 = block_sum(s1, sh);
+    const float b2 = block_sum(l, sh);
+    if (threadIdx.x == 0) {
+        atomicAdd(acc + 3 * b, (double)b0);
+        atomicAdd(acc + 3 * b + 1, (double)b1);
+        atomicAdd(acc + 3 * b + 2, (double)b2);
+        __threadfence();
+        const unsigned tk = atomicAdd(ticket + b, 1u);
+        if (tk == gridDim.x - 1) {
+            const double S0 = atomicAdd(acc + 3 * b, 0.0), S1 = atomicAdd(acc + 3 * b + 1, 0.0), L = atomicAdd(acc + 3 * b + 2, 0.0);
+            const double a = stats[b * 4 + 1], sd = stats[b * 4 + 2];
+            const double beta = S1 / a - sd * S0;
+            bw[b * 4 + 0] = (float)sd;
+            bw[b * 4 + 1] = (float)(beta / (double)P);
+            bw[b * 4 + 2] = (float)(S1 / a);
+            bw[b * 4 + 3] = (float)(beta / ((double)P * sd));
+            loss[b] = (float)L;
+            acc[3 * b] = 0.0; acc[3 * b + 1] = 0.0; acc[3 * b + 2] = 0.0;
+            ticket[b] = 0u;
+        }
+    }
+}
+
 // B1: S0 = sum G, S1 = sum G chi; the last block writes bw = {s, beta/P, S1/a, beta/(P s)},
 // beta = S1/a - s S0.
 __global__ void k_reduce_g(const float4* __restrict__ G, const float4* __restrict__ chi, size_t n4_per_item,
@@ -321,6 +373,10 @@ struct sap_dpsr {
     float *h_pts = nullptr, *h_nrm = nullptr, *h_chi = nullptr, *h_gchi = nullptr, *h_gp = nullptr, *h_gn = nullptr;
     int host_P = 0;
     int binned_P = 0;          // num_points of the forward whose bins are in the workspace
+    // fused-loss path (sap_dpsr_forward_mse / backward_mse), allocated on first use
+    float* gmse = nullptr;     // [B][N^3] G = 2 (chi - chi_gt)
+    double* acc_mse = nullptr; // [B][3]   S0, S1, L accumulators
+    bool mse_valid = false;    // bw and gmse belong to the last forward
     size_t ws_bytes = 0;
     int launches = 0;
     // optional per-kernel timing (sap_dpsr_set_profiling): one event before the first launch, one after each
@@ -500,7 +556,8 @@ template <int N> struct Runner {
         launch_pdl(k_zl_inv<N>, dim3((unsigned)grid), dim3(zl_threads<N, true>()), zl_smem_bytes<N, true>(), st, p);
     }
 
-    static sap_status_t forward(sap_dpsr* h, const float* pts, const float* nrm, int P, float* chi, cudaStream_t st) {
+    static sap_status_t forward(sap_dpsr* h, const float* pts, const float* nrm, int P, float* chi, cudaStream_t st,
+                                const float* chi_gt = nullptr, float* loss = nullptr) {
         const int B = h->batch;
         const size_t V = (size_t)N * N * N;
         prof_begin(h, st);
@@ -544,19 +601,25 @@ template <int N> struct Runner {
             SAP_LAUNCH_CHECK(h, "k_sample_mean");
             const size_t n4 = V / 4;
             int gb = (int)((n4 + 255) / 256); const int cap = (148 * 8 + B - 1) / B; if (gb > cap) gb = cap; if (gb < 1) gb = 1;
-            launch_pdl(k_scale_shift, dim3(dim3(gb, B)), dim3(256), 0, st, reinterpret_cast<float4*>(chi), n4, h->stats);
-            SAP_LAUNCH_CHECK(h, "k_scale_shift");
+            if (chi_gt) {
+                launch_pdl(k_scale_shift_mse, dim3(gb, B), dim3(256), 0, st, reinterpret_cast<float4*>(chi), reinterpret_cast<const float4*>(chi_gt),
+                           reinterpret_cast<float4*>(h->gmse), n4, P, (const float*)h->stats, h->acc_mse, h->ticket + B, h->bw, loss);
+            } else {
+                launch_pdl(k_scale_shift, dim3(gb, B), dim3(256), 0, st, reinterpret_cast<float4*>(chi), n4, (const float*)h->stats);
+            }
+            h->mse_valid = chi_gt != nullptr;
+            SAP_LAUNCH_CHECK(h, chi_gt ? "k_scale_shift_mse" : "k_scale_shift");
         }
         return SAP_OK;
     }
 
     static sap_status_t backward(sap_dpsr* h, const float* pts, const float* nrm, int P, const float* chi,
-                                 const float* gchi, float* gp, float* gn, cudaStream_t st) {
+                                 const float* gchi, float* gp, float* gn, cudaStream_t st, bool have_bw = false) {
         const int B = h->batch;
         const size_t V = (size_t)N * N * N;
         prof_begin(h, st);
-        // B1 reductions
-        {
+        // B1 reductions (already done by the fused loss pass of sap_dpsr_forward_mse)
+        if (!have_bw) {
             const size_t n4 = V / 4;
             int gb = (int)((n4 + 255) / 256); const int cap = (148 * 4 + B - 1) / B; if (gb > cap) gb = cap; if (gb < 1) gb = 1;
             launch_pdl(k_reduce_g, dim3(dim3(gb, B)), dim3(256), 0, st, reinterpret_cast<const float4*>(gchi), reinterpret_cast<const float4*>(chi),
@@ -616,7 +679,7 @@ static bool supported_N(int N) { return N == 32 || N == 64 || N == 128 || N == 2
 static void free_all(sap_dpsr* h) {
     for (int i = 0; i < sap_dpsr::MAX_EV; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
     cudaFree(h->v); cudaFree(h->spts); cudaFree(h->snrm); cudaFree(h->bin_cnt); cudaFree(h->bin_cursor); cudaFree(h->bin_start); cudaFree(h->S3); cudaFree(h->Q3); cudaFree(h->S1); cudaFree(h->Q1); cudaFree(h->QT3); cudaFree(h->QT1); cudaFree(h->tw); cudaFree(h->ftab);
-    cudaFree(h->acc); cudaFree(h->ticket); cudaFree(h->stats); cudaFree(h->bw);
+    cudaFree(h->gmse); cudaFree(h->acc_mse); cudaFree(h->acc); cudaFree(h->ticket); cudaFree(h->stats); cudaFree(h->bw);
     cudaFree(h->h_pts); cudaFree(h->h_nrm); cudaFree(h->h_chi); cudaFree(h->h_gchi); cudaFree(h->h_gp); cudaFree(h->h_gn);
 }
 
@@ -713,6 +776,47 @@ extern "C" sap_status_t sap_dpsr_backward(sap_dpsr_t* h, const float* points, co
     if (num_points != h->binned_P) { h->err = "backward must follow a forward call on this handle with the same num_points"; return SAP_ERR_INVALID_ARG; }
     return dispatch(h->N, [&](auto r) {
         return decltype(r)::backward(h, points, normals, num_points, chi, grad_chi, grad_points, grad_normals, (cudaStream_t)stream);
+    });
+}
+
+static sap_status_t ensure_mse(sap_dpsr* h) {
+    if (h->gmse) return SAP_OK;
+    const size_t V = (size_t)h->N * h->N * h->N, B = (size_t)h->batch;
+    cudaError_t e = dev_alloc(h, &h->gmse, B * V);
+    if (e == cudaSuccess) e = dev_alloc(h, &h->acc_mse, B * 3);
+    if (e == cudaSuccess) e = cudaMemset(h->acc_mse, 0, sizeof(double) * B * 3);
+    if (e != cudaSuccess) {
+        cuda_ok(h, e, "cudaMalloc(fused-loss workspace)");
+        cudaFree(h->gmse); cudaFree(h->acc_mse);
+        h->gmse = nullptr; h->acc_mse = nullptr;
+        cudaGetLastError();
+        return e == cudaErrorMemoryAllocation ? SAP_ERR_OOM : SAP_ERR_CUDA;
+    }
+    return SAP_OK;
+}
+
+extern "C" sap_status_t sap_dpsr_forward_mse(sap_dpsr_t* h, const float* points, const float* normals, int num_points,
+                                             const float* chi_gt, float* chi, float* loss, void* stream) {
+    sap_status_t st = check_common(h, num_points);
+    if (st != SAP_OK) return st;
+    if (!points || !normals || !chi_gt || !chi || !loss) { h->err = "null pointer argument"; return SAP_ERR_INVALID_ARG; }
+    if ((st = ensure_mse(h)) != SAP_OK) return st;
+    return dispatch(h->N, [&](auto r) {
+        return decltype(r)::forward(h, points, normals, num_points, chi, (cudaStream_t)stream, chi_gt, loss);
+    });
+}
+
+extern "C" sap_status_t sap_dpsr_backward_mse(sap_dpsr_t* h, const float* points, const float* normals, int num_points,
+                                              const float* chi, float* grad_points, float* grad_normals, void* stream) {
+    sap_status_t st = check_common(h, num_points);
+    if (st != SAP_OK) return st;
+    if (!points || !normals || !chi || !grad_points || !grad_normals) { h->err = "null pointer argument"; return SAP_ERR_INVALID_ARG; }
+    if (!h->mse_valid || num_points != h->binned_P) {
+        h->err = "sap_dpsr_backward_mse must follow sap_dpsr_forward_mse on this handle with the same num_points";
+        return SAP_ERR_INVALID_ARG;
+    }
+    return dispatch(h->N, [&](auto r) {
+        return decltype(r)::backward(h, points, normals, num_points, chi, h->gmse, grad_points, grad_normals, (cudaStream_t)stream, true);
     });
 }
 

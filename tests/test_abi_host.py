@@ -51,6 +51,8 @@ def test_create_validates_arguments_before_cuda(lib):
 def test_null_handle_is_rejected(lib):
     assert lib.sap_dpsr_forward(None, None, None, 1, None, None) == 1
     assert lib.sap_dpsr_backward(None, None, None, 1, None, None, None, None, None) == 1
+    assert lib.sap_dpsr_forward_mse(None, None, None, 1, None, None, None, None) == 1
+    assert lib.sap_dpsr_backward_mse(None, None, None, 1, None, None, None, None) == 1
     assert lib.sap_dpsr_forward_host(None, None, None, 1, None, None) == 1
     assert lib.sap_dpsr_backward_host(None, None, None, None, None) == 1
     assert lib.sap_dpsr_get_stats(None, None, None) == 1
