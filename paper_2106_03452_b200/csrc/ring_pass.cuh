@@ -28,7 +28,8 @@ template <> struct RingCfg<128> { static constexpr int W = 16, NTC = 128, NG = 4
 template <> struct RingCfg<256> { static constexpr int W = 16, NTC = 256, NG = 2, NSTAGE = 6, MINB = 1; };
 template <> struct RingCfg<512> { static constexpr int W = 16, NTC = 512, NG = 1, NSTAGE = 3, MINB = 1; };  // 64-byte rows (W = 8) measured 25% slower
 // per-mode overrides (same W: the TMA boxes are shared); none at present.  Measured and rejected at N = 128: the
-// solve with 3 groups and 13 buffers (4 spare for prefetch) was 7% slower than 4 groups and 12 buffers.
+// solve with 3 groups and 13 buffers (4 spare for prefetch) was 7% slower than 4 groups and 12 buffers; at N = 512 the
+// solve with 2 groups of 256 threads (64 accumulator registers per thread, spills) 18% slower than 1 group of 512.
 template <int N, int MODE> struct RingCfgM : RingCfg<N> {};
 template <int N, int MODE> constexpr int ring_threads() { return RingCfgM<N, MODE>::NTC * RingCfgM<N, MODE>::NG; }
 
@@ -40,7 +41,7 @@ template <int N> constexpr int ring_tw_entries() {
 template <int N, int MODE> constexpr size_t ring_smem_bytes() {
     using C = RingCfgM<N, MODE>;
     return (size_t)C::NSTAGE * N * C::W * sizeof(float2) + 2 * (size_t)ring_tw_entries<N>() * sizeof(float4) +
-           (size_t)N * sizeof(float4) + 2 * C::NSTAGE * sizeof(uint64_t) + 128;
+           (size_t)N * sizeof(float4) + 3 * C::NSTAGE * sizeof(uint64_t) + 128;
 }
 constexpr size_t SMEM_PER_CTA_MAX = 227 * 1024;  // sm_100a opt-in limit per CTA
 static_assert(ring_smem_bytes<32, MODE_SOLVE>() * 4 <= SMEM_PER_CTA_MAX + 4096 && ring_smem_bytes<64, MODE_SOLVE>() * 3 <= SMEM_PER_CTA_MAX &&
@@ -191,6 +192,7 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
     float4* fx = tabI + TWE;
     uint64_t* full = reinterpret_cast<uint64_t*>(fx + N);
     uint64_t* empty = full + NSTAGE;
+    volatile int* issued = reinterpret_cast<volatile int*>(empty + NSTAGE);  // fills issued into each buffer so far
     const int group = threadIdx.x / NTC, tid = threadIdx.x - group * NTC;
 
     for (int i = threadIdx.x; i < TWE; i += ring_threads<N, MODE>()) {
@@ -203,7 +205,7 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
     }
     for (int i = threadIdx.x; i < N; i += ring_threads<N, MODE>()) fx[i] = p.ftab[i];
     if (threadIdx.x == 0) {
-        for (int s = 0; s < NSTAGE; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, NTC / 32); }
+        for (int s = 0; s < NSTAGE; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, NTC / 32); issued[s] = 0; }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -220,6 +222,7 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
         const int unit = (int)(g / tiles_per_unit), T = (int)(g - (long long)unit * tiles_per_unit);
         const int s = it % NSTAGE;
         mbar_expect_tx(full + s, TILE_BYTES);
+        issued[s] = it / NSTAGE + 1;
         const int plane = unit * IN_CH + ch;
         const uint32_t dst = smem_u32(bufs + (size_t)s * TILE_ELEMS);
         if (T < TILES_MAIN) {
@@ -246,8 +249,12 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
             issue_load(it + NSTAGE);
         }
     };
+    // A parity wait is only meaningful once the barrier has reached the phase waited for: a group may get here
+    // before the fill it wants has even been issued (the previous fill of the buffer belongs to another group), and a
+    // wait one phase early would return at once.  `issued` says the fill is under way, i.e. the phase is current.
     auto acquire = [&](int it) -> float2* {
         const int s = it % NSTAGE;
+        while (issued[s] <= it / NSTAGE) {}
         mbar_wait(full + s, (it / NSTAGE) & 1);
         return bufs + (size_t)s * TILE_ELEMS;
     };

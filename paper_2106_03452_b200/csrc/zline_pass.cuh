@@ -37,7 +37,7 @@ template <int N, bool INV> constexpr int zl_threads() { return ZlCfg<N, INV>::NT
 template <int N, bool INV> constexpr int zl_buf_elems() { return ZlCfg<N, INV>::NL * (N / 2) + ZlCfg<N, INV>::NL; }  // float2 per buffer
 template <int N, bool INV> constexpr size_t zl_smem_bytes() {
     return (size_t)ZlCfg<N, INV>::NBUF * zl_buf_elems<N, INV>() * sizeof(float2) + (size_t)N * sizeof(float2) +
-           2 * ZlCfg<N, INV>::NBUF * sizeof(uint64_t) + 128;
+           3 * ZlCfg<N, INV>::NBUF * sizeof(uint64_t) + 128;
 }
 
 static_assert(zl_smem_bytes<128, true>() <= SMEM_PER_CTA_MAX && zl_smem_bytes<256, true>() <= SMEM_PER_CTA_MAX &&
@@ -140,12 +140,13 @@ struct ZlRing {
     float2* bufs;
     uint64_t* full;
     uint64_t* empty;
+    volatile int* issued;  // fills issued into each buffer so far (see k_ring's acquire)
     long long total;
     const float2* srcS;  // tile g: NL*H complex at srcS + g*NL*H
     const float2* srcQ;  // tile g: NL complex at srcQ + g*NL (nullptr: the tile has no Nyquist part, GBAR input)
     __device__ __forceinline__ void init() const {
         if (threadIdx.x == 0) {
-            for (int s = 0; s < NBUF; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, NTC / 32); }
+            for (int s = 0; s < NBUF; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, NTC / 32); issued[s] = 0; }
             asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         }
     }
@@ -155,11 +156,13 @@ struct ZlRing {
         const int s = it % NBUF;
         float2* b = bufs + (size_t)s * BUF;
         mbar_expect_tx(full + s, (uint32_t)((srcQ ? BUF : NL * H) * sizeof(float2)));
+        issued[s] = it / NBUF + 1;
         bulk_load(b, srcS + (size_t)g * NL * H, NL * H * sizeof(float2), full + s);
         if (srcQ) bulk_load(b + NL * H, srcQ + (size_t)g * NL, NL * sizeof(float2), full + s);
     }
     __device__ __forceinline__ float2* acquire(int it) const {
         const int s = it % NBUF;
+        while (issued[s] <= it / NBUF) {}  // the fill must be under way before its phase parity means anything
         mbar_wait(full + s, (it / NBUF) & 1);
         return bufs + (size_t)s * BUF;
     }
@@ -190,6 +193,7 @@ __global__ void __launch_bounds__(zl_threads<N, true>(), ZlCfg<N, true>::MINB) k
     float2* tw = ring.bufs + (size_t)NBUF * BUF;
     ring.full = reinterpret_cast<uint64_t*>(tw + N);
     ring.empty = ring.full + NBUF;
+    ring.issued = reinterpret_cast<volatile int*>(ring.empty + NBUF);
     ring.total = (long long)p.planes * (N * N / NL);
     ring.srcS = p.S;
     ring.srcQ = p.Q;
@@ -314,6 +318,7 @@ __global__ void __launch_bounds__(zl_threads<N, false>(), ZlCfg<N, false>::MINB)
     float2* tw = ring.bufs + (size_t)C::NBUF * BUF;
     ring.full = reinterpret_cast<uint64_t*>(tw + N);
     ring.empty = ring.full + C::NBUF;
+    ring.issued = reinterpret_cast<volatile int*>(ring.empty + C::NBUF);
     ring.total = (long long)pp.planes * TPP;
     ring.srcS = reinterpret_cast<const float2*>(p.G);  // GBAR: tile g = NL*N floats = NL*H float2 at G + g*NL*N
     ring.srcQ = nullptr;
