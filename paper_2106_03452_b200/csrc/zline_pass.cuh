@@ -127,6 +127,58 @@ __device__ __forceinline__ void zl_split(float2* s, const float2* tw, int tid) {
     }
 }
 
+// Inverse Hermitian split fused with the inverse of the last z stage (two-stage plans H = R0 x R1, N >= 256 tiles).
+// Stored slot p = k0 R1 + k1 holds frequency k = k0 + R0 k1, and H - k sits in block R0 - k0 at index R1 - 1 - k1
+// (block 0: index R1 - k1), so the partner of a whole block is one other block: a task loads the block pair
+// (k0, R0 - k0), turns X[k], X[H-k] into Z[k], Z[H-k] in registers (c2r_pair) and runs the two R1-point inverse
+// butterflies -- one shared-memory round trip and the per-pair index arithmetic of zl_split less.
+template <int N, int NL, int NTC>
+__device__ __forceinline__ void zl_inv_split_stage1(float2* s, const float2* tw, int tid) {
+    constexpr int H = N / 2;
+    constexpr int R0 = StageInfo<H, 0>::R, R1 = StageInfo<H, 1>::R;
+    static_assert(Plan<H>::NS == 2 && StageInfo<H, 1>::ST == 1 && R0 % 2 == 0 && R1 % 2 == 0, "two-stage z plan");
+    constexpr int NTYPE = R0 / 2 + 1;  // block 0, block R0/2, and the pairs (k0, R0 - k0), 1 <= k0 < R0/2
+    for (int t = tid; t < NL * NTYPE; t += NTC) {
+        const int u = t / NL, l = t - u * NL;
+        float2 a[R1];
+        if (u == 0) {
+            // block 0: k = R0 k1.  k1 = 0 pairs with the Nyquist value, k1 = R1/2 (k = H/2) with itself
+#pragma unroll
+            for (int i = 0; i < R1; ++i) a[i] = s[zi<H>(l, i)];
+            const float xh = s[NL * H + l].x;
+            a[0] = make_float2(0.5f * (a[0].x + xh), 0.5f * (a[0].x - xh));
+            a[R1 / 2] = make_float2(a[R1 / 2].x, -a[R1 / 2].y);
+#pragma unroll
+            for (int i = 1; i < R1 / 2; ++i) c2r_pair(a[i], a[R1 - i], tw[R0 * i]);
+            dft_inv<R1>(a);
+#pragma unroll
+            for (int i = 0; i < R1; ++i) s[zi<H>(l, i)] = a[i];
+        } else if (u == 1) {
+            // block R0/2: k = R0/2 + R0 k1 pairs with index R1 - 1 - k1 of the same block
+            constexpr int B0 = (R0 / 2) * R1;
+#pragma unroll
+            for (int i = 0; i < R1; ++i) a[i] = s[zi<H>(l, B0 + i)];
+#pragma unroll
+            for (int i = 0; i < R1 / 2; ++i) c2r_pair(a[i], a[R1 - 1 - i], tw[R0 / 2 + R0 * i]);
+            dft_inv<R1>(a);
+#pragma unroll
+            for (int i = 0; i < R1; ++i) s[zi<H>(l, B0 + i)] = a[i];
+        } else {
+            const int k0 = u - 1;  // 1 .. R0/2 - 1
+            const int ba = k0 * R1, bb = (R0 - k0) * R1;
+            float2 b[R1];
+#pragma unroll
+            for (int i = 0; i < R1; ++i) { a[i] = s[zi<H>(l, ba + i)]; b[i] = s[zi<H>(l, bb + i)]; }
+#pragma unroll
+            for (int i = 0; i < R1; ++i) c2r_pair(a[i], b[R1 - 1 - i], tw[k0 + R0 * i]);
+            dft_inv<R1>(a);
+            dft_inv<R1>(b);
+#pragma unroll
+            for (int i = 0; i < R1; ++i) { s[zi<H>(l, ba + i)] = a[i]; s[zi<H>(l, bb + i)] = b[i]; }
+        }
+    }
+}
+
 }  // namespace sap
 
 namespace sap {
@@ -263,11 +315,11 @@ __global__ void __launch_bounds__(zl_threads<N, true>(), ZlCfg<N, true>::MINB) k
                 }
             }
             consumer_sync<NTC>(group);
-        } else {
-            zl_split<N, NL, true, NTC>(s, tw, tid);
-            consumer_sync<NTC>(group);
         }
-        if constexpr (Plan<H>::NS == 2) {
+        if constexpr (!FUSED) {
+            zl_inv_split_stage1<N, NL, NTC>(s, tw, tid);  // c2r split + inverse of the last z stage in one pass
+            consumer_sync<NTC>(group);
+        } else if constexpr (Plan<H>::NS == 2) {
             zl_stage_lines<N, NL, 1, true, NTC>(s, tw, tid);
             consumer_sync<NTC>(group);
         }
