@@ -24,7 +24,7 @@ struct DevCtx {
 // __global__ wrappers around the block bodies
 // ------------------------------------------------------------------------------------------------
 // minimum resident CTAs per SM the register allocation must allow (a register cliff halves occupancy)
-template <int N> constexpr int zy_min_blocks() { return N == 128 ? 3 : N == 512 ? 3 : 4; }
+template <int N> constexpr int zy_min_blocks() { return (N == 128 || N == 512) ? 3 : 4; }
 template <int N, int NL, bool DO_Y, int SRC, int NT>
 __global__ void __launch_bounds__(NT, zy_min_blocks<N>()) k_zy_fwd(ZyFwdParams p) {
     extern __shared__ float2 smem[];

@@ -162,18 +162,68 @@ SAP_HD void zy_fwd_body(Ctx& ctx, const ZyFwdParams& p, float2* smem, int bx, in
         ctx.sync();
     }
     // B: remaining z stages in shared memory, one line per lane
-    if constexpr (Plan<H>::NS > 1) {
+    static_assert(Plan<H>::NS <= 2, "z plans have at most two stages");
+    // (the fused variant holds a block pair = 2 R1 complex values per thread: worth it where the kernel has the
+    // registers, i.e. at 3 CTAs per SM (N = 512); at N = 256 the kernel runs 4 CTAs per SM on 64 registers)
+    constexpr bool FUSE_SPLIT = !DO_Y && N >= 512;
+    if constexpr (Plan<H>::NS > 1 && !FUSE_SPLIT) {
         fft_stage<H, 1, false, N, true>(s, PITCH, 1, NL, tw, ctx.tid, ctx.nthr);
         ctx.sync();
     }
-    if constexpr (Plan<H>::NS > 2) {
-        fft_stage<H, 2, false, N, true>(s, PITCH, 1, NL, tw, ctx.tid, ctx.nthr);
+    if constexpr (!DO_Y && !FUSE_SPLIT) {
+        r2c_split<N, N>(ctx, s, PITCH, 1, NL, tw);
+        ctx.sync();
+    }
+    if constexpr (FUSE_SPLIT) {
+        // B+C: last z stage fused with the Hermitian split.  Stored slot p = k0 R1 + k1 holds frequency k0 + R0 k1 and
+        // H - k sits in block R0 - k0 at index R1 - 1 - k1 (block 0: R1 - k1): a task transforms the block pair
+        // (k0, R0 - k0) of one line and applies r2c_pair to the 2 R1 values in registers (mirror of zl_inv_split_stage1).
+        static_assert(DO_Y || Plan<H>::NS == 2, "tiles of N >= 256 use two-stage z plans");
+        constexpr int ZR0 = StageInfo<H, 0>::R, ZR1 = StageInfo<H, 1>::R, NTYPE = ZR0 / 2 + 1;
+        for (int t = ctx.tid; t < NL * NTYPE; t += ctx.nthr) {
+            const int u = t / NL, l = t - u * NL;
+            float2* col = s + l;
+            float2 a[ZR1];
+            if (u == 0) {
+#pragma unroll
+                for (int i = 0; i < ZR1; ++i) a[i] = col[i * PITCH];
+                dft_fwd<ZR1>(a);
+                const float2 z = a[0];
+                a[0] = make_float2(z.x + z.y, 0.f);
+                col[H * PITCH] = make_float2(z.x - z.y, 0.f);
+                a[ZR1 / 2] = make_float2(a[ZR1 / 2].x, -a[ZR1 / 2].y);
+#pragma unroll
+                for (int i = 1; i < ZR1 / 2; ++i) r2c_pair(a[i], a[ZR1 - i], tw[ZR0 * i]);
+#pragma unroll
+                for (int i = 0; i < ZR1; ++i) col[i * PITCH] = a[i];
+            } else if (u == 1) {
+                float2* blk = col + (ZR0 / 2) * ZR1 * PITCH;
+#pragma unroll
+                for (int i = 0; i < ZR1; ++i) a[i] = blk[i * PITCH];
+                dft_fwd<ZR1>(a);
+#pragma unroll
+                for (int i = 0; i < ZR1 / 2; ++i) r2c_pair(a[i], a[ZR1 - 1 - i], tw[ZR0 / 2 + ZR0 * i]);
+#pragma unroll
+                for (int i = 0; i < ZR1; ++i) blk[i * PITCH] = a[i];
+            } else {
+                const int k0 = u - 1;
+                float2* ba = col + k0 * ZR1 * PITCH;
+                float2* bb = col + (ZR0 - k0) * ZR1 * PITCH;
+                float2 b[ZR1];
+#pragma unroll
+                for (int i = 0; i < ZR1; ++i) { a[i] = ba[i * PITCH]; b[i] = bb[i * PITCH]; }
+                dft_fwd<ZR1>(a);
+                dft_fwd<ZR1>(b);
+#pragma unroll
+                for (int i = 0; i < ZR1; ++i) r2c_pair(a[i], b[ZR1 - 1 - i], tw[k0 + ZR0 * i]);
+#pragma unroll
+                for (int i = 0; i < ZR1; ++i) { ba[i * PITCH] = a[i]; bb[i * PITCH] = b[i]; }
+            }
+        }
         ctx.sync();
     }
     if constexpr (!DO_Y) {
-        // C: in-place Hermitian split, then copy out (slot-major rows are contiguous in HBM)
-        r2c_split<N, N>(ctx, s, PITCH, 1, NL, tw);
-        ctx.sync();
+        // copy out (slot-major rows are contiguous in HBM)
         for (int i = ctx.tid; i < NL * H; i += ctx.nthr) {
             const int l = i / H, pc = i - l * H;
             So[i] = s[kz_swz(pc, y0 + l) * PITCH + l];
