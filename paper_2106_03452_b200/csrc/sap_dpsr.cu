@@ -268,7 +268,18 @@ __global__ void k_reduce_g(const float4* __restrict__ G, const float4* __restric
     const float4* c = chi + (size_t)b * n4_per_item;
     float s0 = 0.f, s1 = 0.f;
     const size_t stride = (size_t)gridDim.x * blockDim.x;
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4_per_item; i += stride) {
+    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    for (; i + 3 * stride < n4_per_item; i += 4 * stride) {  // 8 independent 16-byte loads in flight per thread
+        float4 a[4], x[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) { a[u] = __ldcs(g + i + u * stride); x[u] = __ldcs(c + i + u * stride); }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            s0 += (a[u].x + a[u].y) + (a[u].z + a[u].w);
+            s1 += (a[u].x * x[u].x + a[u].y * x[u].y) + (a[u].z * x[u].z + a[u].w * x[u].w);
+        }
+    }
+    for (; i < n4_per_item; i += stride) {
         const float4 a = g[i], x = c[i];
         s0 += (a.x + a.y) + (a.z + a.w);
         s1 += (a.x * x.x + a.y * x.y) + (a.z * x.z + a.w * x.w);
