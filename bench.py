@@ -62,17 +62,9 @@ KERNEL_BYTES_V = {
 # profiles/r01_full_cfg{2,3,4}.md (one forward+backward each, kernels in launch order).  At 128^3 batch 1 the working
 # set (~50 MB) lives in the 126 MB L2, so DRAM traffic is far BELOW the algorithmic bytes there.
 NCU_TRAFFIC = {
-    "cfg2_torus_128": {"F:k_bin_count": 244736, "F:k_bin_scan": 9216, "F:k_bin_scatter": 484864, "F:k_zy_fwd": 667392,
-                       "F:k_ring<SOLVE>": 25602816, "F:k_zl_inv": 8541952, "F:k_sample_mean": 2118656, "F:k_scale_shift": 8391936,
-                       "B:k_reduce_g": 16787200, "B:k_zl_gbar": 8739328, "B:k_ring<ADJ>": 8561920, "B:k_zl_inv": 25627648,
-                       "B:k_gather_grads": 7804416},
-    "cfg3_ellipsoids_128_b32": {"F:k_zy_fwd": 774172928, "F:k_ring<SOLVE>": 1064461568, "F:k_zl_inv": 490159872,
-                                "F:k_scale_shift": 479321088, "B:k_reduce_g": 540407040, "B:k_zl_gbar": 494904576,
-                                "B:k_ring<ADJ>": 1032813568, "B:k_zl_inv": 1572671488},
-    "cfg4_ellipsoids_256": {"F:k_zy_fwd": 147823872, "F:k_ring<FWD,y>": 348254464, "F:k_ring<SOLVE>": 242811136,
-                            "F:k_ring<INV,y>": 77978624, "F:k_zl_inv": 81739520, "F:k_scale_shift": 76141056,
-                            "B:k_reduce_g": 137704192, "B:k_zy_fwd<GBAR>": 91645440, "B:k_ring<FWD,y>": 78107648,
-                            "B:k_ring<ADJ>": 211087104, "B:k_ring<INV,y>": 348298752, "B:k_zl_inv": 352476928},
+    "cfg2_torus_128": {"F:k_bin_count": 244480, "F:k_bin_scan": 8704, "F:k_bin_scatter": 484864, "F:k_zy_fwd": 667648, "F:k_ring<SOLVE>": 25604096, "F:k_zl_inv": 8542976, "F:k_sample_mean": 2118400, "F:k_scale_shift": 8392192, "B:k_reduce_g": 16787968, "B:k_zl_gbar": 8739328, "B:k_ring<ADJ>": 8562944, "B:k_zl_inv": 25624832, "B:k_gather_grads": 7804160},
+    "cfg3_ellipsoids_128_b32": {"F:k_zy_fwd": 773939712, "F:k_ring<SOLVE>": 1066452480, "F:k_zl_inv": 491010304, "F:k_scale_shift": 479487232, "B:k_reduce_g": 540808448, "B:k_zl_gbar": 495542528, "B:k_ring<ADJ>": 1032498688, "B:k_zl_inv": 1574035200},
+    "cfg4_ellipsoids_256": {"F:k_zy_fwd": 147638784, "F:k_ring<FWD,y>": 348749312, "F:k_ring<SOLVE>": 243623680, "F:k_ring<INV,y>": 78010368, "F:k_zl_inv": 83020544, "F:k_scale_shift": 76402944, "B:k_reduce_g": 137846272, "B:k_zy_fwd<GBAR>": 91983616, "B:k_ring<FWD,y>": 78512384, "B:k_ring<ADJ>": 211298560, "B:k_ring<INV,y>": 348777216, "B:k_zl_inv": 350359552},
 }
 
 
