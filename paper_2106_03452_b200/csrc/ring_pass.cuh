@@ -7,8 +7,10 @@
 // the register count (the earlier one-tile-per-CTA kernel depended on occupancy for that overlap), and there is
 // no producer warp.
 //   MODE_FWD / MODE_INV : forward / inverse transform along y
-//   MODE_SOLVE (F2x+F3+F4x): forward x on 3 channels side by side, chi~ = i sum_c m_c v~_c, inverse x, 1 channel out
-//   MODE_ADJ   (B3x+B4+B5x): forward x on 1 channel, vbar~_c = -i m_c Gbar'~, 3 inverse x
+//   MODE_SOLVE (F2x+F3+F4x): chi~ = i sum_c m_c v~_c; the y and z channels are combined before the x transform (their
+//                            factors do not depend on x): 2 forward x transforms, the multiplier, 1 inverse, 1 channel out
+//   MODE_ADJ   (B3x+B4+B5x): forward x on 1 channel, vbar~_c = -i m_c Gbar'~; the y and z channels are one inverse x
+//                            transform scaled per column: 2 inverse x transforms, 3 channels out
 // Equations: Eq.3 / Eq.12-17; multiplier and readings as in spectral.cuh.
 #pragma once
 #include <cuda.h>
@@ -165,6 +167,56 @@ __device__ __forceinline__ void ring_stage0_inv_store(const float2* s, const flo
 
 namespace sap {
 
+// Forward stage 0 of the x pass on the combination wy * s1 + wz * s2 of two channels, result in s1.  The y and z
+// factors of the divergence (and of the adjoint) do not depend on x, so they commute with the transform along x:
+// sum_c h_c v~_c needs two forward x transforms, not three (and the adjoint two inverse ones).
+template <int N, int W, int NTC>
+__device__ __forceinline__ void ring_stage0_fwd2(float2* s1, const float2* s2, const float4* tab, int tid, float wy, float wz) {
+    constexpr int R = StageInfo<N, 0>::R, ST = StageInfo<N, 0>::ST;
+    constexpr int NT = ST * W;
+#pragma unroll
+    for (int i = 0; i < (NT + NTC - 1) / NTC; ++i) {
+        const int t = tid + i * NTC;
+        if (NT % NTC != 0 && t >= NT) break;
+        const int q = t / W, c = t - q * W;
+        const float4* tr = tab + q * R;
+        float2 v[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) v[r] = caxpy(wz, s2[(q + r * ST) * W + c], cscale(wy, s1[(q + r * ST) * W + c]));
+        dft_fwd<R>(v);
+#pragma unroll
+        for (int r = 1; r < R; ++r) v[r] = cmul4(v[r], tr[r]);
+#pragma unroll
+        for (int r = 0; r < R; ++r) s1[(q + r * ST) * W + c] = v[r];
+    }
+}
+// inverse stage 0 whose result goes to two outputs scaled by w1 and w2 (the y and z channels of the adjoint)
+template <int N, int W, int NTC>
+__device__ __forceinline__ void ring_stage0_inv_store2(const float2* s, const float4* tab, int tid, float2* out1, float2* out2,
+                                                       unsigned sn, unsigned sc, float w1, float w2) {
+    constexpr int R = StageInfo<N, 0>::R, ST = StageInfo<N, 0>::ST;
+    constexpr int NT = ST * W;
+#pragma unroll
+    for (int i = 0; i < (NT + NTC - 1) / NTC; ++i) {
+        const int t = tid + i * NTC;
+        if (NT % NTC != 0 && t >= NT) break;
+        const int q = t / W, c = t - q * W;
+        const float4* tr = tab + q * R;
+        float2 v[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) v[r] = s[(q + r * ST) * W + c];
+#pragma unroll
+        for (int r = 1; r < R; ++r) v[r] = cmul4(v[r], tr[r]);
+        dft_inv<R>(v);
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const unsigned o = (unsigned)(q + r * ST) * sn + (unsigned)c * sc;
+            out1[o] = cscale(w1, v[r]);
+            out2[o] = cscale(w2, v[r]);
+        }
+    }
+}
+
 template <int N, int MODE>
 __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MINB) k_ring(const __grid_constant__ RingParams p) {
     using C = RingCfgM<N, MODE>;
@@ -312,114 +364,86 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
             }
             ring_stage0_inv_store<N, W, NTC>(buf, tabI, tid, out_tile(0), sn, sc, swz);
             release(it);
-        } else if constexpr (MODE == MODE_SOLVE && NSTAGE < 2 * 3) {
-            // ring too short to hold a whole tile and still prefetch (N = 512): one channel at a time, the divergence
-            // accumulated in registers, each buffer released as soon as its last forward stage has been read
+        } else if constexpr (MODE == MODE_SOLVE) {
+            // chi~ = i f (h_x v~_x + h_y v~_y + h_z v~_z).  h_y and h_z are constant along x, so the y and z channels
+            // are combined BEFORE the x transform: two forward x transforms per tile, not three.  The multiplier and the
+            // first inverse stage happen on the registers of the last forward stage (same slots, no barrier).
+            float4 ey, ez;
+            col_freq(tid % W, ey, ez);  // NTC % W == 0: every task of this thread is in column tid % W
             float2 acc[TPT][RL];
-            float2* buf = nullptr;
-#pragma unroll
-            for (int ch = 0; ch < 3; ++ch) {
-                buf = acquire(it + ch);
-                ring_stage<N, 0, W, NTC, false>(buf, tabF, tid);
+            (void)acc;
+            constexpr bool SIDE = NSTAGE >= 2 * 3;  // the ring can hold a whole tile and still prefetch
+            float2* b0 = acquire(it);
+            ring_stage<N, 0, W, NTC, false>(b0, tabF, tid);
+            if constexpr (!SIDE) {  // N = 512: finish the x channel and hand its buffer back first
                 consumer_sync<NTC>(group);
                 if constexpr (NS == 3) {
-                    ring_stage<N, 1, W, NTC, false>(buf, tabF + N, tid);
+                    ring_stage<N, 1, W, NTC, false>(b0, tabF + N, tid);
                     consumer_sync<NTC>(group);
                 }
 #pragma unroll
                 for (int i = 0; i < TPT; ++i) {
                     const int t = tid + i * NTC, blk = t / W, c = t - blk * W;
-                    const int e0 = blk * RL * W + c;
-                    float4 ey, ez;
-                    col_freq(c, ey, ez);
                     float2 v[RL];
 #pragma unroll
-                    for (int r = 0; r < RL; ++r) v[r] = buf[e0 + r * W];
+                    for (int r = 0; r < RL; ++r) v[r] = b0[(blk * RL + r) * W + c];
                     dft_fwd<RL>(v);
-                    if (ch == 0) {
 #pragma unroll
-                        for (int r = 0; r < RL; ++r) acc[i][r] = cscale(fx[blk * RL + r].x, v[r]);
-                    } else if (ch == 1) {
-#pragma unroll
-                        for (int r = 0; r < RL; ++r) acc[i][r] = caxpy(ey.x, v[r], acc[i][r]);
-                    } else {
-                        float2 a[RL];
-#pragma unroll
-                        for (int r = 0; r < RL; ++r) {
-                            const float f = mult_f(fx[blk * RL + r], ey, ez, p.cs);
-                            const float2 dv = cscale(f, caxpy(ez.x, v[r], acc[i][r]));
-                            a[r] = make_float2(-dv.y, dv.x);  // chi~ = i (div)
-                        }
-                        dft_inv<RL>(a);
-#pragma unroll
-                        for (int r = 0; r < RL; ++r) buf[e0 + r * W] = a[r];
-                    }
+                    for (int r = 0; r < RL; ++r) acc[i][r] = cscale(fx[blk * RL + r].x, v[r]);
                 }
-                if (ch < 2) release(it + ch);
+                release(it);
             }
-            consumer_sync<NTC>(group);
-            if constexpr (NS == 3) {
-                ring_stage<N, 1, W, NTC, true>(buf, tabI + N, tid);
-                consumer_sync<NTC>(group);
-            }
-            ring_stage0_inv_store<N, W, NTC>(buf, tabI, tid, out_tile(0), sn, sc);
-            release(it + 2);
-        } else if constexpr (MODE == MODE_SOLVE) {
-            // the three channels of the tile are transformed side by side; the divergence, the multiplier and the
-            // first inverse stage happen on the registers of the last forward stage (same slots, no barrier)
-            float2* b0 = acquire(it);
-            ring_stage<N, 0, W, NTC, false>(b0, tabF, tid);
             float2* b1 = acquire(it + 1);
-            ring_stage<N, 0, W, NTC, false>(b1, tabF, tid);
             float2* b2 = acquire(it + 2);
-            ring_stage<N, 0, W, NTC, false>(b2, tabF, tid);
+            ring_stage0_fwd2<N, W, NTC>(b1, b2, tabF, tid, ey.x, ez.x);
             consumer_sync<NTC>(group);
+            release(it + 2);  // the z channel has been folded into b1
             if constexpr (NS == 3) {
-                ring_stage<N, 1, W, NTC, false>(b0, tabF + N, tid);
+                if constexpr (SIDE) ring_stage<N, 1, W, NTC, false>(b0, tabF + N, tid);
                 ring_stage<N, 1, W, NTC, false>(b1, tabF + N, tid);
-                ring_stage<N, 1, W, NTC, false>(b2, tabF + N, tid);
                 consumer_sync<NTC>(group);
             }
-#pragma unroll 1
+#pragma unroll
             for (int i = 0; i < TPT; ++i) {
                 const int t = tid + i * NTC, blk = t / W, c = t - blk * W;
                 const int e0 = blk * RL * W + c;
-                float4 ey, ez;
-                col_freq(c, ey, ez);
                 float2 v[RL], a[RL];
+                if constexpr (SIDE) {
 #pragma unroll
-                for (int r = 0; r < RL; ++r) v[r] = b0[e0 + r * W];
-                dft_fwd<RL>(v);
+                    for (int r = 0; r < RL; ++r) v[r] = b0[e0 + r * W];
+                    dft_fwd<RL>(v);
 #pragma unroll
-                for (int r = 0; r < RL; ++r) a[r] = cscale(fx[blk * RL + r].x, v[r]);
+                    for (int r = 0; r < RL; ++r) a[r] = cscale(fx[blk * RL + r].x, v[r]);
+                } else {
+#pragma unroll
+                    for (int r = 0; r < RL; ++r) a[r] = acc[i][r];
+                }
 #pragma unroll
                 for (int r = 0; r < RL; ++r) v[r] = b1[e0 + r * W];
                 dft_fwd<RL>(v);
 #pragma unroll
-                for (int r = 0; r < RL; ++r) a[r] = caxpy(ey.x, v[r], a[r]);
-#pragma unroll
-                for (int r = 0; r < RL; ++r) v[r] = b2[e0 + r * W];
-                dft_fwd<RL>(v);
-#pragma unroll
                 for (int r = 0; r < RL; ++r) {
                     const float f = mult_f(fx[blk * RL + r], ey, ez, p.cs);
-                    const float2 dv = cscale(f, caxpy(ez.x, v[r], a[r]));
+                    const float2 dv = cscale(f, cadd(a[r], v[r]));
                     a[r] = make_float2(-dv.y, dv.x);  // chi~ = i (div)
                 }
                 dft_inv<RL>(a);
 #pragma unroll
-                for (int r = 0; r < RL; ++r) b2[e0 + r * W] = a[r];
+                for (int r = 0; r < RL; ++r) b1[e0 + r * W] = a[r];
             }
-            release(it);
-            release(it + 1);
+            if constexpr (SIDE) release(it);
             consumer_sync<NTC>(group);
             if constexpr (NS == 3) {
-                ring_stage<N, 1, W, NTC, true>(b2, tabI + N, tid);
+                ring_stage<N, 1, W, NTC, true>(b1, tabI + N, tid);
                 consumer_sync<NTC>(group);
             }
-            ring_stage0_inv_store<N, W, NTC>(b2, tabI, tid, out_tile(0), sn, sc);
-            release(it + 2);
+            ring_stage0_inv_store<N, W, NTC>(b1, tabI, tid, out_tile(0), sn, sc);
+            release(it + 1);
         } else {  // MODE_ADJ
+            // vbar~_c = h_c A, A = -i f Gbar'~.  h_y and h_z are constant along x: the y and z channels are the SAME inverse
+            // x transform of A scaled per column, so a tile needs two inverse x transforms, not three.
+            float4 ey, ez;
+            col_freq(tid % W, ey, ez);
             float2* buf = acquire(it);
             ring_stage<N, 0, W, NTC, false>(buf, tabF, tid);
             consumer_sync<NTC>(group);
@@ -427,12 +451,10 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
                 ring_stage<N, 1, W, NTC, false>(buf, tabF + N, tid);
                 consumer_sync<NTC>(group);
             }
-            float2 acc[TPT][RL];  // -i f Gbar'~ on the slots of this thread's last-stage butterflies
+            float2 acc[TPT][RL];  // A on the slots of this thread's last-stage butterflies
 #pragma unroll
             for (int i = 0; i < TPT; ++i) {
                 const int t = tid + i * NTC, blk = t / W, c = t - blk * W;
-                float4 ey, ez;
-                col_freq(c, ey, ez);
                 float2 v[RL];
 #pragma unroll
                 for (int r = 0; r < RL; ++r) v[r] = buf[(blk * RL + r) * W + c];
@@ -444,19 +466,14 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
                 }
             }
 #pragma unroll
-            for (int ch = 0; ch < 3; ++ch) {
-                if (ch > 0) consumer_sync<NTC>(group);  // stage-0 reads of the previous channel are done
+            for (int pass = 0; pass < 2; ++pass) {  // 0: x channel (h_x varies along x), 1: y and z channels
+                if (pass > 0) consumer_sync<NTC>(group);  // stage-0 reads of the previous pass are done
 #pragma unroll
                 for (int i = 0; i < TPT; ++i) {
                     const int t = tid + i * NTC, blk = t / W, c = t - blk * W;
-                    float4 ey, ez;
-                    col_freq(c, ey, ez);
                     float2 v[RL];
 #pragma unroll
-                    for (int r = 0; r < RL; ++r) {
-                        const float h = (ch == 0) ? fx[blk * RL + r].x : (ch == 1) ? ey.x : ez.x;
-                        v[r] = cscale(h, acc[i][r]);
-                    }
+                    for (int r = 0; r < RL; ++r) v[r] = (pass == 0) ? cscale(fx[blk * RL + r].x, acc[i][r]) : acc[i][r];
                     dft_inv<RL>(v);
 #pragma unroll
                     for (int r = 0; r < RL; ++r) buf[(blk * RL + r) * W + c] = v[r];
@@ -466,7 +483,8 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
                     ring_stage<N, 1, W, NTC, true>(buf, tabI + N, tid);
                     consumer_sync<NTC>(group);
                 }
-                ring_stage0_inv_store<N, W, NTC>(buf, tabI, tid, out_tile(ch), sn, sc);
+                if (pass == 0) ring_stage0_inv_store<N, W, NTC>(buf, tabI, tid, out_tile(0), sn, sc);
+                else ring_stage0_inv_store2<N, W, NTC>(buf, tabI, tid, out_tile(1), out_tile(2), sn, sc, ey.x, ez.x);
             }
             release(it);
         }
