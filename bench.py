@@ -34,27 +34,28 @@ UNIT = "ms/grid"
 #   label: (yardstick V fused (N<=128), yardstick V unfused, compulsory V)   -- per channel-set launch
 YARD_FWD_BWD_V = 52.0
 KERNEL_BYTES_V = {
+    # label: (yardstick V fused (N<=128), yardstick V unfused (N>=256), compulsory V fused, compulsory V unfused)
     # forward
-    "F:k_bin_count": (0.0, 0.0, 0.0),               # counting sort of the points (bytes ~ 72 B/point, ignored)
-    "F:k_bin_scan": (0.0, 0.0, 0.0),
-    "F:k_bin_scatter": (0.0, 0.0, 0.0),
+    "F:k_bin_count": (0.0, 0.0, 0.0, 0.0),               # counting sort of the points (bytes ~ 72 B/point, ignored)
+    "F:k_bin_scan": (0.0, 0.0, 0.0, 0.0),
+    "F:k_bin_scatter": (0.0, 0.0, 0.0, 0.0),
     # splat fused in: rows "splat" (3V) + z r2c x3 (6V) [+ y x3 (6V) when fused]; it only WRITES 3V itself
-    "F:k_zy_fwd": (15.0, 9.0, 3.0),
-    "F:k_ring<FWD,y>": (0.0, 6.0, 6.0),          # row y sweep x3
-    "F:k_ring<SOLVE>": (4.0, 4.0, 4.0),          # row x sweep + solve + x inverse (3V in, 1V out)
-    "F:k_ring<INV,y>": (0.0, 2.0, 2.0),          # row inverse y
-    "F:k_zl_inv": (4.0, 2.0, 2.0),                  # rows [inverse y (2V) +] inverse z c2r (2V)
-    "F:k_sample_mean": (0.0, 0.0, 0.0),
-    "F:k_scale_shift": (2.0, 2.0, 2.0),             # row normalise
+    "F:k_zy_fwd": (15.0, 9.0, 3.0, 3.0),
+    "F:k_ring<FWD,y>": (0.0, 6.0, 0.0, 5.0),             # row y sweep x3; writes 2 spectra (x, u = h_y y + h_z z)
+    "F:k_ring<SOLVE>": (4.0, 4.0, 4.0, 3.0),             # row x sweep + solve + x inverse (3V or 2V in, 1V out)
+    "F:k_ring<INV,y>": (0.0, 2.0, 0.0, 2.0),             # row inverse y
+    "F:k_zl_inv": (4.0, 2.0, 2.0, 2.0),                  # rows [inverse y (2V) +] inverse z c2r (2V)
+    "F:k_sample_mean": (0.0, 0.0, 0.0, 0.0),
+    "F:k_scale_shift": (2.0, 2.0, 2.0, 2.0),             # row normalise
     # backward
-    "B:k_reduce_g": (2.0, 2.0, 2.0),                # row reductions
-    "B:k_zl_gbar": (5.0, 3.0, 2.0),                 # the same pass as a persistent bulk-copy kernel (N <= 128)
-    "B:k_zy_fwd<GBAR>": (5.0, 3.0, 2.0),            # rows z r2c (G+W in, 1 out = 3V) [+ y (2V)]; W is re-rasterised, not read
-    "B:k_ring<FWD,y>": (0.0, 2.0, 2.0),
-    "B:k_ring<ADJ>": (4.0, 4.0, 4.0),            # row x sweep + conj(M) fan-out + 3 x inverse
-    "B:k_ring<INV,y>": (0.0, 6.0, 6.0),
-    "B:k_zl_inv": (12.0, 6.0, 6.0),                 # rows inverse y x3 + inverse z x3
-    "B:k_gather_grads": (4.0, 4.0, 0.0),            # row gather (<= 4V, sparse)
+    "B:k_reduce_g": (2.0, 2.0, 2.0, 2.0),                # row reductions
+    "B:k_zl_gbar": (5.0, 3.0, 2.0, 2.0),                 # rows z r2c (G+W in, 1 out = 3V) + y (2V); W is re-rasterised, not read
+    "B:k_zy_fwd<GBAR>": (5.0, 3.0, 2.0, 2.0),            # the same pass, one tile per CTA (N >= 256)
+    "B:k_ring<FWD,y>": (0.0, 2.0, 0.0, 2.0),
+    "B:k_ring<ADJ>": (4.0, 4.0, 4.0, 3.0),               # row x sweep + conj(M) fan-out + x inverses (1V in, 3V or 2V out)
+    "B:k_ring<INV,y>": (0.0, 6.0, 0.0, 5.0),             # reads 2 spectra (x, B), writes 3
+    "B:k_zl_inv": (12.0, 6.0, 6.0, 6.0),                 # rows inverse y x3 + inverse z x3
+    "B:k_gather_grads": (4.0, 4.0, 0.0, 0.0),            # row gather (<= 4V, sparse)
 }
 
 
@@ -357,7 +358,7 @@ def roofline_of(res, peak_gbs):
     fused = cfg.N <= 128
     km = res["kernels_ms"]
     name = max(km, key=km.get)
-    yard_v, comp_v = (KERNEL_BYTES_V[name][0] if fused else KERNEL_BYTES_V[name][1]), KERNEL_BYTES_V[name][2]
+    yard_v, comp_v = (KERNEL_BYTES_V[name][0], KERNEL_BYTES_V[name][2]) if fused else (KERNEL_BYTES_V[name][1], KERNEL_BYTES_V[name][3])
     ach = yard_v * V / (km[name] * 1e-3) / 1e9
     comp = comp_v * V / (km[name] * 1e-3) / 1e9
     return {"bound": "hbm", "kernel": name, "kernel_ms": km[name], "share_of_step": km[name] / sum(km.values()),

@@ -190,6 +190,51 @@ __device__ __forceinline__ void ring_stage0_fwd2(float2* s1, const float2* s2, c
         for (int r = 0; r < R; ++r) s1[(q + r * ST) * W + c] = v[r];
     }
 }
+// inverse stage 0 of a y-pass tile with a per-column output factor scale(c), c = z slot inside the tile
+template <int N, int W, int NTC, class F>
+__device__ __forceinline__ void ring_stage0_inv_store_scaled(const float2* s, const float4* tab, int tid, float2* out, unsigned sn,
+                                                             unsigned sc, int swz, F scale) {
+    constexpr int R = StageInfo<N, 0>::R, ST = StageInfo<N, 0>::ST;
+    constexpr int NT = ST * W;
+#pragma unroll
+    for (int i = 0; i < (NT + NTC - 1) / NTC; ++i) {
+        const int t = tid + i * NTC;
+        if (NT % NTC != 0 && t >= NT) break;
+        const int q = t / W, c = t - q * W;
+        const float4* tr = tab + q * R;
+        const float w = scale(c);
+        float2 v[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) v[r] = s[(q + r * ST) * W + (c ^ ((q + r * ST) & swz))];
+#pragma unroll
+        for (int r = 1; r < R; ++r) v[r] = cmul4(v[r], tr[r]);
+        dft_inv<R>(v);
+#pragma unroll
+        for (int r = 0; r < R; ++r) out[(unsigned)(q + r * ST) * sn + (unsigned)(c ^ ((q + r * ST) & swz)) * sc] = cscale(w, v[r]);
+    }
+}
+// forward stage 0 of a y-pass tile with a per-column input factor scale(c)
+template <int N, int W, int NTC, class F>
+__device__ __forceinline__ void ring_stage0_fwd_scaled(float2* s, const float4* tab, int tid, int swz, F scale) {
+    constexpr int R = StageInfo<N, 0>::R, ST = StageInfo<N, 0>::ST;
+    constexpr int NT = ST * W;
+#pragma unroll
+    for (int i = 0; i < (NT + NTC - 1) / NTC; ++i) {
+        const int t = tid + i * NTC;
+        if (NT % NTC != 0 && t >= NT) break;
+        const int q = t / W, c = t - q * W;
+        const float4* tr = tab + q * R;
+        const float w = scale(c);
+        float2 v[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) v[r] = cscale(w, s[(q + r * ST) * W + (c ^ ((q + r * ST) & swz))]);
+        dft_fwd<R>(v);
+#pragma unroll
+        for (int r = 1; r < R; ++r) v[r] = cmul4(v[r], tr[r]);
+#pragma unroll
+        for (int r = 0; r < R; ++r) s[(q + r * ST) * W + (c ^ ((q + r * ST) & swz))] = v[r];
+    }
+}
 // inverse stage 0 whose result goes to two outputs scaled by w1 and w2 (the y and z channels of the adjoint)
 template <int N, int W, int NTC>
 __device__ __forceinline__ void ring_stage0_inv_store2(const float2* s, const float4* tab, int tid, float2* out1, float2* out2,
@@ -221,7 +266,8 @@ template <int N, int MODE>
 __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MINB) k_ring(const __grid_constant__ RingParams p) {
     using C = RingCfgM<N, MODE>;
     constexpr int W = C::W, NTC = C::NTC, NG = C::NG, NSTAGE = C::NSTAGE, H = N / 2;
-    constexpr int AXIS = (MODE == MODE_FWD || MODE == MODE_INV) ? 1 : 0;  // y pass : x pass
+    constexpr int AXIS = (MODE == MODE_FWD || MODE == MODE_INV || MODE == MODE_FWD3 || MODE == MODE_INV3) ? 1 : 0;  // y : x pass
+    constexpr bool TWO_SPECTRA = (N >= 256);  // the y and z channels reach / leave the x pass as one spectrum
     constexpr int NS = Plan<N>::NS, LS = NS - 1, RL = StageInfo<N, LS>::R;
     static_assert(StageInfo<N, LS>::ST == 1 && NS >= 2, "plan");
     constexpr int R0 = StageInfo<N, 0>::R, R1 = StageInfo<N, 1>::R;
@@ -232,7 +278,10 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
     constexpr int NTASK = (N / RL) * W, TPT = NTASK / NTC;
     static_assert(NTASK % NTC == 0, "last-stage tasks divide evenly over the consumers");
     constexpr int KT = H / W, TILES_MAIN = N * KT, TILES_NYQ = N / W;
-    constexpr int IN_CH = (MODE == MODE_SOLVE) ? 3 : 1, OUT_CH = (MODE == MODE_ADJ) ? 3 : 1;
+    // input items per tile, and the plane strides of the 3-channel arrays on either side
+    constexpr int IN_CH = (MODE == MODE_SOLVE) ? (TWO_SPECTRA ? 2 : 3) : (MODE == MODE_FWD3 || MODE == MODE_INV3) ? 3 : 1;
+    constexpr int IN_STRIDE = (MODE == MODE_SOLVE || MODE == MODE_FWD3 || MODE == MODE_INV3) ? 3 : 1;
+    constexpr int OUT_CH = (MODE == MODE_ADJ || MODE == MODE_FWD3 || MODE == MODE_INV3) ? 3 : 1;
     constexpr size_t SPLANE = (size_t)N * N * H, QPLANE = (size_t)N * N;
     constexpr int tiles_per_unit = TILES_MAIN + TILES_NYQ;
     constexpr int IT_PER_TILE = IN_CH;
@@ -275,7 +324,7 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
         const int s = it % NSTAGE;
         mbar_expect_tx(full + s, TILE_BYTES);
         issued[s] = it / NSTAGE + 1;
-        const int plane = unit * IN_CH + ch;
+        const int plane = unit * IN_STRIDE + ((MODE == MODE_INV3 && ch == 2) ? 1 : ch);  // INV3 fetches plane 1 twice
         const uint32_t dst = smem_u32(bufs + (size_t)s * TILE_ELEMS);
         if (T < TILES_MAIN) {
             const int o = T / KT, kt = T - o * KT;
@@ -364,6 +413,72 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
             }
             ring_stage0_inv_store<N, W, NTC>(buf, tabI, tid, out_tile(0), sn, sc, swz);
             release(it);
+        } else if constexpr (MODE == MODE_FWD3) {
+            // y pass of the three splat channels: plane 0 = FFT_y(v_x); plane 1 = u = h_y FFT_y(v_y) + FFT_y(h_z v_z)
+            // (h_z is constant along y: applied on the way into the transform; h_y on the way out)
+            auto hz_of = [&](int c) { return __ldg(p.ftab + N + (d.nyq ? H : d.pz0 + c)).x; };  // a thread follows the z SLOT c across rows
+            float2 acc[TPT][RL];
+#pragma unroll
+            for (int ch = 0; ch < 3; ++ch) {
+                float2* buf = acquire(it + ch);
+                if (ch == 2) ring_stage0_fwd_scaled<N, W, NTC>(buf, tabF, tid, swz, hz_of);
+                else ring_stage<N, 0, W, NTC, false>(buf, tabF, tid, swz);
+                consumer_sync<NTC>(group);
+                if constexpr (NS == 3) {
+                    ring_stage<N, 1, W, NTC, false>(buf, tabF + N, tid, swz);
+                    consumer_sync<NTC>(group);
+                }
+                float2* out = out_tile(ch == 0 ? 0 : 1);
+#pragma unroll
+                for (int i = 0; i < TPT; ++i) {
+                    const int t = tid + i * NTC, blk = t / W, c = t - blk * W;
+                    float2 v[RL];
+#pragma unroll
+                    for (int r = 0; r < RL; ++r) v[r] = buf[(blk * RL + r) * W + (c ^ ((blk * RL + r) & swz))];
+                    dft_fwd<RL>(v);
+                    if (ch == 1) {
+#pragma unroll
+                        for (int r = 0; r < RL; ++r) acc[i][r] = cscale(fx[blk * RL + r].x, v[r]);
+                    } else {
+#pragma unroll
+                        for (int r = 0; r < RL; ++r)
+                            out[(unsigned)(blk * RL + r) * sn + (unsigned)(c ^ ((blk * RL + r) & swz)) * sc] =
+                                (ch == 0) ? v[r] : cadd(v[r], acc[i][r]);
+                    }
+                }
+                release(it + ch);
+            }
+        } else if constexpr (MODE == MODE_INV3) {
+            // inverse y pass of the adjoint: plane 0 = IFFT_y(plane 0); from B (plane 1, fetched twice -- the second fetch
+            // is an L2 hit): plane 1 = IFFT_y(h_y B), plane 2 = h_z IFFT_y(B)
+            auto hz_of = [&](int c) { return __ldg(p.ftab + N + (d.nyq ? H : d.pz0 + c)).x; };  // a thread follows the z SLOT c across rows
+#pragma unroll
+            for (int ch = 0; ch < 3; ++ch) {
+                float2* buf = acquire(it + ch);
+                if (ch == 1) {  // inverse of the last plan stage with h_y on the way in
+#pragma unroll
+                    for (int i = 0; i < TPT; ++i) {
+                        const int t = tid + i * NTC, blk = t / W, c = t - blk * W;
+                        float2 v[RL];
+#pragma unroll
+                        for (int r = 0; r < RL; ++r)
+                            v[r] = cscale(fx[blk * RL + r].x, buf[(blk * RL + r) * W + (c ^ ((blk * RL + r) & swz))]);
+                        dft_inv<RL>(v);
+#pragma unroll
+                        for (int r = 0; r < RL; ++r) buf[(blk * RL + r) * W + (c ^ ((blk * RL + r) & swz))] = v[r];
+                    }
+                } else {
+                    ring_stage<N, LS, W, NTC, true>(buf, nullptr, tid, swz);
+                }
+                consumer_sync<NTC>(group);
+                if constexpr (NS == 3) {
+                    ring_stage<N, 1, W, NTC, true>(buf, tabI + N, tid, swz);
+                    consumer_sync<NTC>(group);
+                }
+                if (ch < 2) ring_stage0_inv_store<N, W, NTC>(buf, tabI, tid, out_tile(ch), sn, sc, swz);
+                else ring_stage0_inv_store_scaled<N, W, NTC>(buf, tabI, tid, out_tile(2), sn, sc, swz, hz_of);
+                release(it + ch);
+            }
         } else if constexpr (MODE == MODE_SOLVE) {
             // chi~ = i f (h_x v~_x + h_y v~_y + h_z v~_z).  h_y and h_z are constant along x, so the y and z channels
             // are combined BEFORE the x transform: two forward x transforms per tile, not three.  The multiplier and the
@@ -372,7 +487,7 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
             col_freq(tid % W, ey, ez);  // NTC % W == 0: every task of this thread is in column tid % W
             float2 acc[TPT][RL];
             (void)acc;
-            constexpr bool SIDE = NSTAGE >= 2 * 3;  // the ring can hold a whole tile and still prefetch
+            constexpr bool SIDE = NSTAGE >= 2 * 3;  // the ring can hold whole tiles and still prefetch
             float2* b0 = acquire(it);
             ring_stage<N, 0, W, NTC, false>(b0, tabF, tid);
             if constexpr (!SIDE) {  // N = 512: finish the x channel and hand its buffer back first
@@ -394,10 +509,15 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
                 release(it);
             }
             float2* b1 = acquire(it + 1);
-            float2* b2 = acquire(it + 2);
-            ring_stage0_fwd2<N, W, NTC>(b1, b2, tabF, tid, ey.x, ez.x);
-            consumer_sync<NTC>(group);
-            release(it + 2);  // the z channel has been folded into b1
+            if constexpr (TWO_SPECTRA) {  // the y pass has already formed u = h_y v~_y + h_z v~_z
+                ring_stage<N, 0, W, NTC, false>(b1, tabF, tid);
+                consumer_sync<NTC>(group);
+            } else {
+                float2* b2 = acquire(it + 2);
+                ring_stage0_fwd2<N, W, NTC>(b1, b2, tabF, tid, ey.x, ez.x);
+                consumer_sync<NTC>(group);
+                release(it + 2);  // the z channel has been folded into b1
+            }
             if constexpr (NS == 3) {
                 if constexpr (SIDE) ring_stage<N, 1, W, NTC, false>(b0, tabF + N, tid);
                 ring_stage<N, 1, W, NTC, false>(b1, tabF + N, tid);
@@ -483,7 +603,7 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
                     ring_stage<N, 1, W, NTC, true>(buf, tabI + N, tid);
                     consumer_sync<NTC>(group);
                 }
-                if (pass == 0) ring_stage0_inv_store<N, W, NTC>(buf, tabI, tid, out_tile(0), sn, sc);
+                if (pass == 0 || TWO_SPECTRA) ring_stage0_inv_store<N, W, NTC>(buf, tabI, tid, out_tile(pass), sn, sc);  // B unscaled: the y pass finishes it
                 else ring_stage0_inv_store2<N, W, NTC>(buf, tabI, tid, out_tile(1), out_tile(2), sn, sc, ey.x, ez.x);
             }
             release(it);

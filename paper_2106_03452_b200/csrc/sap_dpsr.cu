@@ -514,6 +514,8 @@ template <int N> struct Runner {
         upd(set_smem(k_ring<N, MODE_ADJ>, ring_smem_bytes<N, MODE_ADJ>()));
         if constexpr (!C::FUSED_ZY) {
             upd(set_smem(k_ring<N, MODE_FWD>, ring_smem_bytes<N, MODE_FWD>()));
+            upd(set_smem(k_ring<N, MODE_FWD3>, ring_smem_bytes<N, MODE_FWD3>()));
+            upd(set_smem(k_ring<N, MODE_INV3>, ring_smem_bytes<N, MODE_INV3>()));
             upd(set_smem(k_ring<N, MODE_INV>, ring_smem_bytes<N, MODE_INV>()));
         }
         if (!cuda_ok(h, e, "cudaFuncSetAttribute")) return SAP_ERR_CUDA;
@@ -590,7 +592,7 @@ template <int N> struct Runner {
             SAP_LAUNCH_CHECK(h, "k_zy_fwd");
         }
         if constexpr (!C::FUSED_ZY) {
-            launch_ring<MODE_FWD>(h, st, B * 3, h->mS3y, h->mQT3, h->S3, h->Q3, 1);
+            launch_ring<MODE_FWD3>(h, st, B, h->mS3y, h->mQT3, h->S3, h->Q3, 1);  // planes (x, u, -) out of (x, y, z)
             SAP_LAUNCH_CHECK(h, "k_ring<FWD,y>");
         }
         // F2x + F3 + F4x: x forward, spectral solve, x inverse (3 -> 1)
@@ -652,7 +654,7 @@ template <int N> struct Runner {
         launch_ring<MODE_ADJ>(h, st, B, h->mS1x, h->mQ1, h->S3, C::FUSED_ZY ? h->Q3 : h->QT3, 0);
         SAP_LAUNCH_CHECK(h, "k_ring<ADJ>");
         if constexpr (!C::FUSED_ZY) {
-            launch_ring<MODE_INV>(h, st, B * 3, h->mS3y, h->mQT3, h->S3, h->Q3, 1);
+            launch_ring<MODE_INV3>(h, st, B, h->mS3y, h->mQT3, h->S3, h->Q3, 1);  // planes (x, y, z) out of (x, B, -)
             SAP_LAUNCH_CHECK(h, "k_ring<INV,y>");
         }
         // B5 (y +) z inverse -> vbar (into the v workspace)

@@ -38,7 +38,11 @@ SAP_HD float mult_f(const float4& ex, const float4& ey, const float4& ez, float 
     return (q == 0.f) ? 0.f : cs * (ex.z * ey.z) * ez.z * fast_rcp(q);
 }
 
-enum { MODE_FWD = 0, MODE_INV = 1, MODE_SOLVE = 2, MODE_ADJ = 3 };
+// MODE_FWD3 / MODE_INV3: the y pass of the three field channels when it is a kernel of its own (N >= 256).  The y and z
+// channels travel between the y pass and the x pass as ONE spectrum (u = h_y v~_y + h_z v~_z forward; B = the inverse x
+// transform of -i f Gbar'~ backward, from which vbar_y and vbar_z differ only by factors that commute with the
+// remaining transforms), which saves one spectrum write and one read in each direction.
+enum { MODE_FWD = 0, MODE_INV = 1, MODE_SOLVE = 2, MODE_ADJ = 3, MODE_FWD3 = 4, MODE_INV3 = 5 };
 
 struct TileDesc {
     size_t base;   // element offset inside one channel array
