@@ -65,7 +65,7 @@ KERNEL_BYTES_V = {
 NCU_TRAFFIC = {
     "cfg2_torus_128": {"F:k_bin_count": 244480, "F:k_bin_scan": 8704, "F:k_bin_scatter": 484864, "F:k_zy_fwd": 667648, "F:k_ring<SOLVE>": 25604096, "F:k_zl_inv": 8542976, "F:k_sample_mean": 2118400, "F:k_scale_shift": 8392192, "B:k_reduce_g": 16787968, "B:k_zl_gbar": 8739328, "B:k_ring<ADJ>": 8562944, "B:k_zl_inv": 25624832, "B:k_gather_grads": 7804160},
     "cfg3_ellipsoids_128_b32": {"F:k_zy_fwd": 773939712, "F:k_ring<SOLVE>": 1066452480, "F:k_zl_inv": 491010304, "F:k_scale_shift": 479487232, "B:k_reduce_g": 540808448, "B:k_zl_gbar": 495542528, "B:k_ring<ADJ>": 1032498688, "B:k_zl_inv": 1574035200},
-    "cfg4_ellipsoids_256": {"F:k_zy_fwd": 147638784, "F:k_ring<FWD,y>": 348749312, "F:k_ring<SOLVE>": 243623680, "F:k_ring<INV,y>": 78010368, "F:k_zl_inv": 83020544, "F:k_scale_shift": 76402944, "B:k_reduce_g": 137846272, "B:k_zy_fwd<GBAR>": 91983616, "B:k_ring<FWD,y>": 78512384, "B:k_ring<ADJ>": 211298560, "B:k_ring<INV,y>": 348777216, "B:k_zl_inv": 350359552},
+    "cfg4_ellipsoids_256": {"F:k_zy_fwd": 147610880, "F:k_ring<FWD,y>": 284943616, "F:k_ring<SOLVE>": 166544896, "F:k_ring<INV,y>": 78128896, "F:k_zl_inv": 82979328, "F:k_scale_shift": 78618880, "B:k_reduce_g": 137347328, "B:k_zy_fwd<GBAR>": 92718336, "B:k_ring<FWD,y>": 78034432, "B:k_ring<ADJ>": 144984832, "B:k_ring<INV,y>": 280314112, "B:k_zl_inv": 350683648},
 }
 
 
