@@ -235,33 +235,6 @@ __device__ __forceinline__ void ring_stage0_fwd_scaled(float2* s, const float4* 
         for (int r = 0; r < R; ++r) s[(q + r * ST) * W + (c ^ ((q + r * ST) & swz))] = v[r];
     }
 }
-// inverse stage 0 whose result goes to two outputs scaled by w1 and w2 (the y and z channels of the adjoint)
-template <int N, int W, int NTC>
-__device__ __forceinline__ void ring_stage0_inv_store2(const float2* s, const float4* tab, int tid, float2* out1, float2* out2,
-                                                       unsigned sn, unsigned sc, float w1, float w2) {
-    constexpr int R = StageInfo<N, 0>::R, ST = StageInfo<N, 0>::ST;
-    constexpr int NT = ST * W;
-#pragma unroll
-    for (int i = 0; i < (NT + NTC - 1) / NTC; ++i) {
-        const int t = tid + i * NTC;
-        if (NT % NTC != 0 && t >= NT) break;
-        const int q = t / W, c = t - q * W;
-        const float4* tr = tab + q * R;
-        float2 v[R];
-#pragma unroll
-        for (int r = 0; r < R; ++r) v[r] = s[(q + r * ST) * W + c];
-#pragma unroll
-        for (int r = 1; r < R; ++r) v[r] = cmul4(v[r], tr[r]);
-        dft_inv<R>(v);
-#pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const unsigned o = (unsigned)(q + r * ST) * sn + (unsigned)c * sc;
-            out1[o] = cscale(w1, v[r]);
-            out2[o] = cscale(w2, v[r]);
-        }
-    }
-}
-
 template <int N, int MODE>
 __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MINB) k_ring(const __grid_constant__ RingParams p) {
     using C = RingCfgM<N, MODE>;
@@ -561,7 +534,7 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
             release(it + 1);
         } else {  // MODE_ADJ
             // vbar~_c = h_c A, A = -i f Gbar'~.  h_y and h_z are constant along x: the y and z channels are the SAME inverse
-            // x transform of A scaled per column, so a tile needs two inverse x transforms, not three.
+            // x transform B of A, so a tile needs two inverse x transforms, not three, and writes two spectra.
             float4 ey, ez;
             col_freq(tid % W, ey, ez);
             float2* buf = acquire(it);
@@ -603,8 +576,9 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
                     ring_stage<N, 1, W, NTC, true>(buf, tabI + N, tid);
                     consumer_sync<NTC>(group);
                 }
-                if (pass == 0 || TWO_SPECTRA) ring_stage0_inv_store<N, W, NTC>(buf, tabI, tid, out_tile(pass), sn, sc);  // B unscaled: the y pass finishes it
-                else ring_stage0_inv_store2<N, W, NTC>(buf, tabI, tid, out_tile(1), out_tile(2), sn, sc, ey.x, ez.x);
+                // pass 1 stores B unscaled as plane 1: the next pass (k_ring<INV3> or the fused k_zl_inv) makes the y and
+                // z channels from it with h_y and h_z on the way into ITS first stage
+                ring_stage0_inv_store<N, W, NTC>(buf, tabI, tid, out_tile(pass), sn, sc);
             }
             release(it);
         }

@@ -560,9 +560,9 @@ template <int N> struct Runner {
         if (grid > total) grid = total;
         launch_pdl(k_zl_gbar<N>, dim3((unsigned)grid), dim3(zl_threads<N, false>()), zl_smem_bytes<N, false>(), st, p);
     }
-    static void launch_zl_inv(sap_dpsr* h, cudaStream_t st, const float2* S, const float2* Q, float* out, int planes) {
+    static void launch_zl_inv(sap_dpsr* h, cudaStream_t st, const float2* S, const float2* Q, float* out, int planes, int adj3 = 0) {
         using ZC = ZlCfg<N, true>;
-        ZlInvParams p{S, Q, out, h->tw, planes};
+        ZlInvParams p{S, Q, out, h->tw, planes, adj3, h->ftab};
         const long long total = (long long)planes * (N * N / ZC::NL);
         long long grid = (long long)ZC::MINB * h->num_sms;
         if (grid > total) grid = total;
@@ -659,7 +659,7 @@ template <int N> struct Runner {
         }
         // B5 (y +) z inverse -> vbar (into the v workspace)
         {
-            launch_zl_inv(h, st, h->S3, h->Q3, h->v, B * 3);
+            launch_zl_inv(h, st, h->S3, h->Q3, h->v, B * 3, C::FUSED_ZY ? 1 : 0);  // fused: planes (x, B, -) -> (x, y, z)
             SAP_LAUNCH_CHECK(h, "k_zl_inv");
         }
         // B6 gather

@@ -37,7 +37,7 @@ template <int N, bool INV> constexpr int zl_threads() { return ZlCfg<N, INV>::NT
 template <int N, bool INV> constexpr int zl_buf_elems() { return ZlCfg<N, INV>::NL * (N / 2) + ZlCfg<N, INV>::NL; }  // float2 per buffer
 template <int N, bool INV> constexpr size_t zl_smem_bytes() {
     return (size_t)ZlCfg<N, INV>::NBUF * zl_buf_elems<N, INV>() * sizeof(float2) + (size_t)N * sizeof(float2) +
-           3 * ZlCfg<N, INV>::NBUF * sizeof(uint64_t) + 128;
+           3 * ZlCfg<N, INV>::NBUF * sizeof(uint64_t) + (size_t)(N + N / 2 + 4) * sizeof(float) + 128;
 }
 
 static_assert(zl_smem_bytes<128, true>() <= SMEM_PER_CTA_MAX && zl_smem_bytes<256, true>() <= SMEM_PER_CTA_MAX &&
@@ -50,6 +50,10 @@ struct ZlInvParams {
     float* out;         // [planes][N^3]
     const float2* tw;   // exp(-2 pi i t / N), t < N
     int planes;
+    // adjoint mode of the fused planes (N <= 128): per item the spectra are (x channel, B, -) and the three output
+    // planes are IFFT(plane 0), IFFT(h_y B), IFFT(h_z B): plane 2 is made from plane 1 (fetched again: an L2 hit)
+    int adj3;
+    const float4* ftab; // per-slot frequency table (spectral.cuh), used in adjoint mode
 };
 
 // plain bulk copy global -> shared, completion on an mbarrier (bytes: multiple of 16, both addresses 16-aligned)
@@ -196,6 +200,7 @@ struct ZlRing {
     long long total;
     const float2* srcS;  // tile g: NL*H complex at srcS + g*NL*H
     const float2* srcQ;  // tile g: NL complex at srcQ + g*NL (nullptr: the tile has no Nyquist part, GBAR input)
+    int adj3;            // fused adjoint planes: the tiles of plane 3i+2 are fetched from plane 3i+1
     __device__ __forceinline__ void init() const {
         if (threadIdx.x == 0) {
             for (int s = 0; s < NBUF; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, NTC / 32); issued[s] = 0; }
@@ -203,8 +208,12 @@ struct ZlRing {
         }
     }
     __device__ __forceinline__ void issue_load(int it) const {
-        const long long g = (long long)blockIdx.x + (long long)it * gridDim.x;
+        long long g = (long long)blockIdx.x + (long long)it * gridDim.x;
         if (g >= total) return;
+        if (adj3) {
+            constexpr int TPP = 2 * H * 2 * H / NL;  // tiles per plane
+            if ((g / TPP) % 3 == 2) g -= TPP;
+        }
         const int s = it % NBUF;
         float2* b = bufs + (size_t)s * BUF;
         mbar_expect_tx(full + s, (uint32_t)((srcQ ? BUF : NL * H) * sizeof(float2)));
@@ -249,8 +258,15 @@ __global__ void __launch_bounds__(zl_threads<N, true>(), ZlCfg<N, true>::MINB) k
     ring.total = (long long)p.planes * (N * N / NL);
     ring.srcS = p.S;
     ring.srcQ = p.Q;
+    ring.adj3 = FUSED ? p.adj3 : 0;
+    float* fy = reinterpret_cast<float*>(const_cast<int*>(ring.issued + NBUF));  // h_y per y slot, h_z per z slot (+ Nyquist)
+    float* fz = fy + N;
     const int group = threadIdx.x / NTC, tid = threadIdx.x - group * NTC;
     for (int i = threadIdx.x; i < N; i += zl_threads<N, true>()) tw[i] = p.tw[i];
+    if (FUSED && p.adj3) {
+        for (int i = threadIdx.x; i < N; i += zl_threads<N, true>()) fy[i] = p.ftab[i].x;
+        for (int i = threadIdx.x; i <= H; i += zl_threads<N, true>()) fz[i] = p.ftab[N + i].x;
+    }
     ring.init();
     __syncthreads();
     pdl_wait();
@@ -264,11 +280,20 @@ __global__ void __launch_bounds__(zl_threads<N, true>(), ZlCfg<N, true>::MINB) k
             static_assert(!FUSED || Plan<N>::NS == 2, "fused planes use two-stage y plans");
             // D': inverse of the last y stage, lanes over z slots
             constexpr int R1 = StageInfo<N, 1>::R;
+            const int ch = p.adj3 ? (int)((g / (N * N / NL)) % 3) : 0;  // adjoint mode: 1 = h_y on the way in, 2 = h_z
             for (int t = tid; t < H * (N / R1); t += NTC) {
                 const int blk = t / H, pz = t - blk * H;
                 float2 v[R1];
 #pragma unroll
                 for (int r = 0; r < R1; ++r) v[r] = s[zi<H>(blk * R1 + r, pz)];
+                if (ch == 1) {
+#pragma unroll
+                    for (int r = 0; r < R1; ++r) v[r] = cscale(fy[blk * R1 + r], v[r]);
+                } else if (ch == 2) {
+                    const float w = fz[pz];
+#pragma unroll
+                    for (int r = 0; r < R1; ++r) v[r] = cscale(w, v[r]);
+                }
                 dft_inv<R1>(v);
 #pragma unroll
                 for (int r = 0; r < R1; ++r) s[zi<H>(blk * R1 + r, pz)] = v[r];
@@ -277,6 +302,13 @@ __global__ void __launch_bounds__(zl_threads<N, true>(), ZlCfg<N, true>::MINB) k
                 float2 v[R1];
 #pragma unroll
                 for (int r = 0; r < R1; ++r) v[r] = s[NL * H + blk * R1 + r];
+                if (ch == 1) {
+#pragma unroll
+                    for (int r = 0; r < R1; ++r) v[r] = cscale(fy[blk * R1 + r], v[r]);
+                } else if (ch == 2) {
+#pragma unroll
+                    for (int r = 0; r < R1; ++r) v[r] = cscale(fz[H], v[r]);  // h_z = 0 on the Nyquist plane (R3)
+                }
                 dft_inv<R1>(v);
 #pragma unroll
                 for (int r = 0; r < R1; ++r) s[NL * H + blk * R1 + r] = v[r];
@@ -374,6 +406,7 @@ __global__ void __launch_bounds__(zl_threads<N, false>(), ZlCfg<N, false>::MINB)
     ring.total = (long long)pp.planes * TPP;
     ring.srcS = reinterpret_cast<const float2*>(p.G);  // GBAR: tile g = NL*N floats = NL*H float2 at G + g*NL*N
     ring.srcQ = nullptr;
+    ring.adj3 = 0;
     const int group = threadIdx.x / NTC, tid = threadIdx.x - group * NTC;
     for (int i = threadIdx.x; i < N; i += zl_threads<N, false>()) tw[i] = p.tw[i];
     ring.init();
