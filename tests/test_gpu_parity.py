@@ -145,6 +145,48 @@ def test_fused_mse_loss_and_gradients():
     h.close()
 
 
+def test_cuda_graph_replay_matches_eager():
+    # forward and backward allocate nothing, never synchronise and keep no host-side state between calls, so a
+    # captured CUDA graph (programmatic-dependent-launch edges included) can be replayed on new inputs
+    import torch
+    from paper_2106_03452_b200.binding import Dpsr
+    N, P = 64, 4000
+    pts, nrm = inputs.make_cloud("torus", P, seed=2)
+    pts2, nrm2 = inputs.make_cloud("ellipsoids3", P, seed=3)
+    G = torch.from_numpy(inputs.upstream_grad(N, 1, seed=4)).cuda()
+    h = Dpsr(N, 2.0, 1, P)
+    c, n = torch.from_numpy(pts[None].copy()).cuda(), torch.from_numpy(nrm[None].copy()).cuda()
+    chi = torch.empty((1, N, N, N), dtype=torch.float32, device="cuda")
+    gp, gn = torch.empty_like(c), torch.empty_like(n)
+
+    def step():
+        h.forward(c, n, chi)
+        h.backward(c, n, chi, G, gp, gn)
+
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        step()
+    torch.cuda.current_stream().wait_stream(side)
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        step()
+    for p_, n_ in ((pts2, nrm2), (pts, nrm)):      # replay on other inputs written into the captured buffers
+        c.copy_(torch.from_numpy(p_[None].copy()))
+        n.copy_(torch.from_numpy(n_[None].copy()))
+        graph.replay()
+        torch.cuda.synchronize()
+        got = (chi.clone(), gp.clone(), gn.clone())
+        step()
+        torch.cuda.synchronize()
+        for a, b in zip(got, (chi, gp, gn)):
+            assert (a - b).abs().max().item() <= 1e-5 * b.abs().max().item()
+        f = orc.forward(N, 2.0, p_, n_)
+        assert np.abs(got[0].cpu().numpy()[0] - f["chi"]).max() <= CHI_TOL * np.abs(f["chi"]).max()
+    del graph
+    h.close()
+
+
 def test_repeatable_and_handle_reuse():
     import torch
     from paper_2106_03452_b200.binding import Dpsr
