@@ -47,7 +47,7 @@ typedef enum {
  * coarse-to-fine schedule, plus 512), Gaussian bandwidth sigma >= 0 of Eq.3
  * (sigma = 0 means no filter, L460), `batch` independent shapes per call (the
  * learning setting uses 32, L419) and at most max_points points per shape.  The scale m of Eq.2 is
- * fixed to 0.5 (L77).  Allocates the workspace (about 9 N^3 floats per batch item) on the current
+ * fixed to 0.5 (L77).  Allocates the workspace (about 8 N^3 floats per batch item) on the current
  * CUDA device.  *out is set only on SAP_OK.
  */
 sap_status_t sap_dpsr_create(int N, float sigma, int batch, int max_points, sap_dpsr_t** out);
@@ -62,7 +62,8 @@ sap_status_t sap_dpsr_create(int N, float sigma, int batch, int max_points, sap_
  *   normals  dev [batch][num_points][3] float, any magnitude (L494)
  *   num_points 1 <= num_points <= max_points, the same for every item of the batch
  *   chi      dev [batch][N][N][N] float, overwritten
- * The handle remembers (mu, a, s) per item and the point density W for the backward.
+ * The handle remembers (mu, a, s) per item and the points sorted into bins (with their original index)
+ * for the backward, which re-rasterises the point density W from them.
  */
 sap_status_t sap_dpsr_forward(sap_dpsr_t* h, const float* points, const float* normals,
                               int num_points, float* chi, void* stream);
