@@ -15,7 +15,12 @@
  *   - Pointers marked "dev" are CUDA device pointers valid on the handle's device; "host" are
  *     ordinary host pointers (pinned memory makes the *_host calls asynchronous copies).
  *   - The caller owns every buffer it passes and the stream.  The handle owns its workspace,
- *     allocated once in sap_dpsr_create; forward/backward never allocate.
+ *     allocated once in sap_dpsr_create; sap_dpsr_forward / sap_dpsr_backward never allocate.  The
+ *     fused-loss and host-buffer variants need extra buffers: allocate them up front with
+ *     sap_dpsr_reserve (then those calls never allocate either and can be captured in a CUDA graph
+ *     from their first call); without it they allocate on their first use.
+ *   - Every call must be made with the handle's device current (the one that was current in
+ *     sap_dpsr_create); otherwise SAP_ERR_INVALID_ARG.
  *   - Work is enqueued on `stream` (a cudaStream_t cast to void*, NULL = default stream) and NOT
  *     synchronised, except where stated.  Device-side faults surface at the caller's next sync.
  *   - Preconditions not checked on the device: coordinates finite and in [0,1) (indices are wrapped
@@ -70,8 +75,13 @@ sap_status_t sap_dpsr_forward(sap_dpsr_t* h, const float* points, const float* n
 
 /*
  * Backward: the exact adjoint of sap_dpsr_forward (dL/dpoints, dL/dnormals from dL/dchi); must
- * follow, on the same handle, the forward call it differentiates, with the same points/normals
- * and that call's chi, unmodified.  Derivation: DESIGN.md "Backward".
+ * follow, on the same handle, the forward call it differentiates, with that call's chi, unmodified,
+ * and NO other forward variant on the handle in between: the backward works from the state the
+ * forward left in the handle (points and normals sorted into bins, mu, a, s).  `points` and `normals`
+ * are accepted for symmetry with the forward and must be that call's inputs; they are not read
+ * again.  A caller that interleaves forwards (two shapes per step, an evaluation forward inside a
+ * training step) detects a stale handle with sap_dpsr_epoch / sap_dpsr_check_epoch below, or uses
+ * one handle per live forward.  Derivation: DESIGN.md "Backward".
  *   chi          dev [batch][N][N][N]   forward output
  *   grad_chi     dev [batch][N][N][N]   dL/dchi
  *   grad_points  dev [batch][num_points][3], overwritten
@@ -112,6 +122,23 @@ sap_status_t sap_dpsr_forward_host(sap_dpsr_t* h, const float* points_host,
 sap_status_t sap_dpsr_backward_host(sap_dpsr_t* h, const float* grad_chi_host,
                                     float* grad_points_host, float* grad_normals_host,
                                     void* stream);
+
+/*
+ * Every forward variant increments the handle's epoch.  sap_dpsr_epoch returns the epoch of the last
+ * forward (0: none yet); sap_dpsr_check_epoch returns SAP_ERR_INVALID_ARG when `epoch` is not the
+ * current one, i.e. when a backward for the forward that returned `epoch` would silently use another
+ * call's bins and statistics.  The Python autograd wrapper keeps the epoch with the saved tensors.
+ */
+unsigned long long sap_dpsr_epoch(const sap_dpsr_t* h);
+sap_status_t sap_dpsr_check_epoch(sap_dpsr_t* h, unsigned long long epoch);
+
+/*
+ * Allocates up front the optional buffers of the fused-loss path (SAP_RESERVE_MSE: one N^3 grid per
+ * item) and / or of the host-buffer path (SAP_RESERVE_HOST: device staging for points, normals,
+ * chi, dL/dchi and the gradients).  `what` is an OR of the flags.  Idempotent.
+ */
+enum { SAP_RESERVE_MSE = 1, SAP_RESERVE_HOST = 2 };
+sap_status_t sap_dpsr_reserve(sap_dpsr_t* h, int what);
 
 /* Copies the per-item statistics of the last forward to host: stats_host[batch][3] = {mu, a, s}.
  * Synchronises `stream`. */

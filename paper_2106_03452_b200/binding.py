@@ -16,7 +16,9 @@ EXPORTS = [
     "sap_dpsr_create", "sap_dpsr_forward", "sap_dpsr_backward", "sap_dpsr_forward_mse", "sap_dpsr_backward_mse", "sap_dpsr_forward_host",
     "sap_dpsr_backward_host", "sap_dpsr_get_stats", "sap_dpsr_destroy", "sap_dpsr_last_error",
     "sap_dpsr_workspace_bytes", "sap_dpsr_last_launch_count", "sap_dpsr_set_profiling", "sap_dpsr_get_profile",
+    "sap_dpsr_epoch", "sap_dpsr_check_epoch", "sap_dpsr_reserve",
 ]
+SAP_RESERVE_MSE, SAP_RESERVE_HOST = 1, 2
 
 _lib = None
 
@@ -66,6 +68,12 @@ def lib():
     L.sap_dpsr_set_profiling.restype = ci
     L.sap_dpsr_get_profile.argtypes = [vp, ctypes.POINTER(cf), ctypes.POINTER(ctypes.c_char_p), ci]
     L.sap_dpsr_get_profile.restype = ci
+    L.sap_dpsr_epoch.argtypes = [vp]
+    L.sap_dpsr_epoch.restype = ctypes.c_ulonglong
+    L.sap_dpsr_check_epoch.argtypes = [vp, ctypes.c_ulonglong]
+    L.sap_dpsr_check_epoch.restype = ci
+    L.sap_dpsr_reserve.argtypes = [vp, ci]
+    L.sap_dpsr_reserve.restype = ci
     _lib = L
     return L
 
@@ -189,6 +197,19 @@ class Dpsr:
         self._check(lib().sap_dpsr_get_stats(self._h, out.ctypes.data_as(ctypes.c_void_p), _stream_ptr(stream)))
         return out
 
+    @property
+    def epoch(self):
+        """Epoch of the last forward on this handle (every forward variant increments it)."""
+        return int(lib().sap_dpsr_epoch(self._h))
+
+    def check_epoch(self, epoch):
+        """Raises if another forward has run on the handle since the one that returned `epoch`."""
+        self._check(lib().sap_dpsr_check_epoch(self._h, int(epoch)))
+
+    def reserve(self, mse=False, host=False):
+        """Allocates the optional buffers of the fused-loss / host-buffer entry points up front."""
+        self._check(lib().sap_dpsr_reserve(self._h, (SAP_RESERVE_MSE if mse else 0) | (SAP_RESERVE_HOST if host else 0)))
+
     def set_profiling(self, on=True):
         self._check(lib().sap_dpsr_set_profiling(self._h, int(bool(on))))
 
@@ -232,11 +253,13 @@ class DpsrFunction:
             def forward(ctx, points, normals):
                 chi = handle.forward(points.contiguous(), normals.contiguous())
                 ctx.save_for_backward(points, normals, chi)
+                ctx.epoch = handle.epoch
                 return chi
 
             @staticmethod
             def backward(ctx, grad_chi):
                 points, normals, chi = ctx.saved_tensors
+                handle.check_epoch(ctx.epoch)   # a later forward on this handle has replaced the bins and statistics
                 gp, gn = handle.backward(points.contiguous(), normals.contiguous(), chi, grad_chi.contiguous())
                 return gp, gn
 

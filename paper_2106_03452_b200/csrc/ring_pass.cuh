@@ -322,6 +322,7 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
             mbar_wait(empty + s, (it / NSTAGE) & 1);
             issue_load(it + NSTAGE);
         }
+        __syncwarp();  // warp 0 is converged again before the next aligned group barrier
     };
     // A parity wait is only meaningful once the barrier has reached the phase waited for: a group may get here
     // before the fill it wants has even been issued (the previous fill of the buffer belongs to another group), and a
@@ -448,6 +449,10 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
                     ring_stage<N, 1, W, NTC, true>(buf, tabI + N, tid, swz);
                     consumer_sync<NTC>(group);
                 }
+                // The pass runs in place and plane 1 is fetched twice (items ch = 1 and ch = 2): the second fetch must have
+                // LANDED before plane 1 of this tile is overwritten (an issued bulk load is not ordered against later
+                // generic stores), so wait for the ch = 2 buffer's full barrier first.  It is a separate buffer: no cost.
+                if (ch == 1) acquire(it + 2);
                 if (ch < 2) ring_stage0_inv_store<N, W, NTC>(buf, tabI, tid, out_tile(ch), sn, sc, swz);
                 else ring_stage0_inv_store_scaled<N, W, NTC>(buf, tabI, tid, out_tile(2), sn, sc, swz, hz_of);
                 release(it + ch);

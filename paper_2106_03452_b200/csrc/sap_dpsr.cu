@@ -384,6 +384,11 @@ struct sap_dpsr {
     float *h_pts = nullptr, *h_nrm = nullptr, *h_chi = nullptr, *h_gchi = nullptr, *h_gp = nullptr, *h_gn = nullptr;
     int host_P = 0;
     int binned_P = 0;          // num_points of the forward whose bins are in the workspace
+    // which forward the workspace state (bins, stats, bw, gmse) belongs to: bumped by EVERY forward variant, so that a
+    // backward can tell whether another forward has run on the handle since the one it differentiates
+    unsigned long long epoch = 0;
+    enum FwdKind { FWD_NONE = 0, FWD_DEVICE = 1, FWD_MSE = 2, FWD_HOST = 3 };
+    int fwd_kind = FWD_NONE;
     // fused-loss path (sap_dpsr_forward_mse / backward_mse), allocated on first use
     float* gmse = nullptr;     // [B][N^3] G = 2 (chi - chi_gt)
     double* acc_mse = nullptr; // [B][3]   S0, S1, L accumulators
@@ -609,11 +614,11 @@ template <int N> struct Runner {
         }
         // F5 normalise
         {
-            int nb = (P + 255) / 256; if (nb > 296) nb = 296;
+            int nb = (P + 255) / 256; if (nb > 2 * h->num_sms) nb = 2 * h->num_sms;
             launch_pdl(k_sample_mean, dim3(dim3(nb, B)), dim3(256), 0, st, (const float4*)h->spts, P, N, (const float*)chi, h->acc, h->ticket, h->stats);
             SAP_LAUNCH_CHECK(h, "k_sample_mean");
             const size_t n4 = V / 4;
-            int gb = (int)((n4 + 255) / 256); const int cap = (148 * 8 + B - 1) / B; if (gb > cap) gb = cap; if (gb < 1) gb = 1;
+            int gb = (int)((n4 + 255) / 256); const int cap = (h->num_sms * 8 + B - 1) / B; if (gb > cap) gb = cap; if (gb < 1) gb = 1;
             if (chi_gt) {
                 launch_pdl(k_scale_shift_mse, dim3(gb, B), dim3(256), 0, st, reinterpret_cast<float4*>(chi), reinterpret_cast<const float4*>(chi_gt),
                            reinterpret_cast<float4*>(h->gmse), n4, P, (const float*)h->stats, h->acc_mse, h->ticket + B, h->bw, loss);
@@ -634,7 +639,7 @@ template <int N> struct Runner {
         // B1 reductions (already done by the fused loss pass of sap_dpsr_forward_mse)
         if (!have_bw) {
             const size_t n4 = V / 4;
-            int gb = (int)((n4 + 255) / 256); const int cap = (148 * 4 + B - 1) / B; if (gb > cap) gb = cap; if (gb < 1) gb = 1;
+            int gb = (int)((n4 + 255) / 256); const int cap = (h->num_sms * 4 + B - 1) / B; if (gb > cap) gb = cap; if (gb < 1) gb = 1;
             launch_pdl(k_reduce_g, dim3(dim3(gb, B)), dim3(256), 0, st, reinterpret_cast<const float4*>(gchi), reinterpret_cast<const float4*>(chi),
                                                    n4, P, h->stats, h->acc + B, h->ticket + B, h->bw);
             SAP_LAUNCH_CHECK(h, "k_reduce_g");
@@ -764,12 +769,26 @@ extern "C" sap_status_t sap_dpsr_create(int N, float sigma, int batch, int max_p
     return SAP_OK;
 }
 
+// the workspace, the TMA descriptors and every buffer the caller passes live on the device the handle was created on
+static sap_status_t check_device(sap_dpsr* h) {
+    int dev = -1;
+    if (!cuda_ok(h, cudaGetDevice(&dev), "cudaGetDevice")) return SAP_ERR_CUDA;
+    if (dev != h->device) {
+        char buf[160];
+        snprintf(buf, sizeof buf, "current CUDA device is %d but the handle was created on device %d (call cudaSetDevice first)", dev, h->device);
+        h->err = buf;
+        return SAP_ERR_INVALID_ARG;
+    }
+    return SAP_OK;
+}
+static void mark_forward(sap_dpsr* h, int kind) { ++h->epoch; h->fwd_kind = kind; }
+
 static sap_status_t check_common(sap_dpsr* h, int num_points) {
     if (!h) return SAP_ERR_INVALID_ARG;
     h->err.clear();
     h->launches = 0;
     if (num_points < 1 || num_points > h->max_points) { h->err = "num_points out of range [1, max_points]"; return SAP_ERR_INVALID_ARG; }
-    return SAP_OK;
+    return check_device(h);
 }
 
 extern "C" sap_status_t sap_dpsr_forward(sap_dpsr_t* h, const float* points, const float* normals, int num_points,
@@ -777,6 +796,7 @@ extern "C" sap_status_t sap_dpsr_forward(sap_dpsr_t* h, const float* points, con
     sap_status_t st = check_common(h, num_points);
     if (st != SAP_OK) return st;
     if (!points || !normals || !chi) { h->err = "null pointer argument"; return SAP_ERR_INVALID_ARG; }
+    mark_forward(h, sap_dpsr::FWD_DEVICE);
     return dispatch(h->N, [&](auto r) { return decltype(r)::forward(h, points, normals, num_points, chi, (cudaStream_t)stream); });
 }
 
@@ -786,7 +806,10 @@ extern "C" sap_status_t sap_dpsr_backward(sap_dpsr_t* h, const float* points, co
     sap_status_t st = check_common(h, num_points);
     if (st != SAP_OK) return st;
     if (!points || !normals || !chi || !grad_chi || !grad_points || !grad_normals) { h->err = "null pointer argument"; return SAP_ERR_INVALID_ARG; }
-    if (num_points != h->binned_P) { h->err = "backward must follow a forward call on this handle with the same num_points"; return SAP_ERR_INVALID_ARG; }
+    if ((h->fwd_kind != sap_dpsr::FWD_DEVICE && h->fwd_kind != sap_dpsr::FWD_MSE) || num_points != h->binned_P) {
+        h->err = "sap_dpsr_backward must follow sap_dpsr_forward (or sap_dpsr_forward_mse) on this handle with the same num_points";
+        return SAP_ERR_INVALID_ARG;
+    }
     return dispatch(h->N, [&](auto r) {
         return decltype(r)::backward(h, points, normals, num_points, chi, grad_chi, grad_points, grad_normals, (cudaStream_t)stream);
     });
@@ -814,6 +837,7 @@ extern "C" sap_status_t sap_dpsr_forward_mse(sap_dpsr_t* h, const float* points,
     if (st != SAP_OK) return st;
     if (!points || !normals || !chi_gt || !chi || !loss) { h->err = "null pointer argument"; return SAP_ERR_INVALID_ARG; }
     if ((st = ensure_mse(h)) != SAP_OK) return st;
+    mark_forward(h, sap_dpsr::FWD_MSE);
     return dispatch(h->N, [&](auto r) {
         return decltype(r)::forward(h, points, normals, num_points, chi, (cudaStream_t)stream, chi_gt, loss);
     });
@@ -824,7 +848,7 @@ extern "C" sap_status_t sap_dpsr_backward_mse(sap_dpsr_t* h, const float* points
     sap_status_t st = check_common(h, num_points);
     if (st != SAP_OK) return st;
     if (!points || !normals || !chi || !grad_points || !grad_normals) { h->err = "null pointer argument"; return SAP_ERR_INVALID_ARG; }
-    if (!h->mse_valid || num_points != h->binned_P) {
+    if (h->fwd_kind != sap_dpsr::FWD_MSE || !h->mse_valid || num_points != h->binned_P) {
         h->err = "sap_dpsr_backward_mse must follow sap_dpsr_forward_mse on this handle with the same num_points";
         return SAP_ERR_INVALID_ARG;
     }
@@ -857,6 +881,7 @@ extern "C" sap_status_t sap_dpsr_forward_host(sap_dpsr_t* h, const float* points
     if (st != SAP_OK) return st;
     if (!points_host || !normals_host) { h->err = "null pointer argument"; return SAP_ERR_INVALID_ARG; }
     if ((st = ensure_staging(h)) != SAP_OK) return st;
+    mark_forward(h, sap_dpsr::FWD_HOST);
     cudaStream_t s = (cudaStream_t)stream;
     const size_t pb = (size_t)h->batch * num_points * 3 * sizeof(float);
     const size_t vb = (size_t)h->batch * h->N * h->N * h->N * sizeof(float);
@@ -875,7 +900,11 @@ extern "C" sap_status_t sap_dpsr_backward_host(sap_dpsr_t* h, const float* grad_
     if (!h) return SAP_ERR_INVALID_ARG;
     h->err.clear();
     const int keep = h->launches;
-    if (!h->h_pts || h->host_P < 1) { h->err = "sap_dpsr_backward_host must follow sap_dpsr_forward_host"; return SAP_ERR_INVALID_ARG; }
+    if (check_device(h) != SAP_OK) return SAP_ERR_INVALID_ARG;
+    if (!h->h_pts || h->host_P < 1 || h->fwd_kind != sap_dpsr::FWD_HOST) {
+        h->err = "sap_dpsr_backward_host must follow sap_dpsr_forward_host (no other forward on this handle in between)";
+        return SAP_ERR_INVALID_ARG;
+    }
     if (!grad_chi_host || !grad_points_host || !grad_normals_host) { h->err = "null pointer argument"; return SAP_ERR_INVALID_ARG; }
     (void)keep;
     h->launches = 0;
@@ -912,6 +941,29 @@ extern "C" void sap_dpsr_destroy(sap_dpsr_t* h) {
     if (!h) return;
     free_all(h);
     delete h;
+}
+
+extern "C" unsigned long long sap_dpsr_epoch(const sap_dpsr_t* h) { return h ? h->epoch : 0ull; }
+extern "C" sap_status_t sap_dpsr_check_epoch(sap_dpsr_t* h, unsigned long long epoch) {
+    if (!h) return SAP_ERR_INVALID_ARG;
+    h->err.clear();
+    if (epoch != h->epoch) {
+        h->err = "stale forward: another forward has run on this handle since the one being differentiated "
+                 "(bins and normalisation statistics now belong to the later call)";
+        return SAP_ERR_INVALID_ARG;
+    }
+    return SAP_OK;
+}
+
+extern "C" sap_status_t sap_dpsr_reserve(sap_dpsr_t* h, int what) {
+    if (!h) return SAP_ERR_INVALID_ARG;
+    h->err.clear();
+    sap_status_t st = check_device(h);
+    if (st != SAP_OK) return st;
+    if ((what & ~(SAP_RESERVE_MSE | SAP_RESERVE_HOST)) != 0) { h->err = "unknown reserve flag"; return SAP_ERR_INVALID_ARG; }
+    if ((what & SAP_RESERVE_MSE) && (st = ensure_mse(h)) != SAP_OK) return st;
+    if ((what & SAP_RESERVE_HOST) && (st = ensure_staging(h)) != SAP_OK) return st;
+    return SAP_OK;
 }
 
 extern "C" const char* sap_dpsr_last_error(const sap_dpsr_t* h) { return h ? h->err.c_str() : g_create_err.c_str(); }

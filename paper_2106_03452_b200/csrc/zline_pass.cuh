@@ -237,6 +237,7 @@ struct ZlRing {
             mbar_wait(empty + s, (it / NBUF) & 1);
             issue_load(it + NBUF);
         }
+        __syncwarp();
     }
 };
 

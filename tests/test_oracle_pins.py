@@ -55,7 +55,7 @@ def test_dft_axis_order_delta_and_parseval():
     # constant <-> delta, inverse carries 1/N^3 (R8)
     ones = np.ones((N, N, N))
     f = orc.dft3(ones, -1)
-    assert abs(f[0, 0, 0] - N ** 3) < 1e-9 and np.abs(f).sum() - N ** 3 < 1e-9
+    assert abs(f[0, 0, 0] - N ** 3) < 1e-9 and abs(np.abs(f).sum() - N ** 3) < 1e-9
     y = RNG.standard_normal((N, N, N))
     fy = orc.dft3(y, -1)
     assert abs((np.abs(fy) ** 2).sum() / N ** 3 - (y ** 2).sum()) < 1e-9  # Parseval
@@ -234,7 +234,7 @@ def test_normalisation_constraints_and_scale_invariance():
     chi = f["chi"]
     assert abs(abs(chi[0, 0, 0]) - 0.5) < 1e-14                      # abs(chi|x=0) = m (Eq.2)
     assert abs(orc.interp(N, pts, chi).mean()) < 1e-13               # mean of chi over the points = 0 (Eq.4)
-    assert abs(f["s"] * f["a"]) - 0.5 < 1e-14
+    assert abs(abs(f["s"] * f["a"]) - 0.5) < 1e-14
     # chi = s (chi' - mu)
     assert np.abs(chi - f["s"] * (f["chi_prime"] - f["mu"])).max() < 1e-13
     # invariance under n -> alpha n, alpha > 0 (normals need not be unit)
