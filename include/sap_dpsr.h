@@ -140,6 +140,28 @@ sap_status_t sap_dpsr_check_epoch(sap_dpsr_t* h, unsigned long long epoch);
 enum { SAP_RESERVE_MSE = 1, SAP_RESERVE_HOST = 2 };
 sap_status_t sap_dpsr_reserve(sap_dpsr_t* h, int what);
 
+/*
+ * Two implementations of the same path live in the library:
+ *   SAP_PATH_THROUGHPUT  one kernel per pass (13 launches per forward+backward), persistent TMA rings: every size, any batch;
+ *   SAP_PATH_LATENCY     the whole forward and the whole backward as ONE cooperative kernel each, phases separated by grid
+ *                        barriers, planes kept in shared memory across them (N <= 128 and batch * N <= number of SMs:
+ *                        the 32^3 / 64^3 / 128^3 levels of the coarse-to-fine schedule, at batch 1).
+ * SAP_PATH_AUTO (default) takes the latency path where it measured faster (eligible handles with N <= 64), else the
+ * throughput path; SAP_PATH_LATENCY forces it on any eligible handle (else SAP_ERR_UNSUPPORTED).  Both leave the same state in the
+ * handle, so a forward on one path may be followed by the backward on the other.  sap_dpsr_get_path returns the path
+ * the next call will take.  The fused-loss entry points always use the throughput path.
+ */
+enum { SAP_PATH_AUTO = 0, SAP_PATH_THROUGHPUT = 1, SAP_PATH_LATENCY = 2 };
+sap_status_t sap_dpsr_set_path(sap_dpsr_t* h, int path);
+int sap_dpsr_get_path(const sap_dpsr_t* h);
+
+/*
+ * Latency path only: device time between the grid barriers of the last forward and backward, stamped by CTA 0
+ * (microseconds in us[i], static labels in names[i]; either may be NULL).  Blocking (device -> host copy on the
+ * legacy stream).  Returns the number of entries written (at most cap).
+ */
+int sap_dpsr_get_fused_phases(sap_dpsr_t* h, float* us, const char** names, int cap);
+
 /* Copies the per-item statistics of the last forward to host: stats_host[batch][3] = {mu, a, s}.
  * Synchronises `stream`. */
 sap_status_t sap_dpsr_get_stats(sap_dpsr_t* h, float* stats_host, void* stream);

@@ -16,8 +16,11 @@ EXPORTS = [
     "sap_dpsr_create", "sap_dpsr_forward", "sap_dpsr_backward", "sap_dpsr_forward_mse", "sap_dpsr_backward_mse", "sap_dpsr_forward_host",
     "sap_dpsr_backward_host", "sap_dpsr_get_stats", "sap_dpsr_destroy", "sap_dpsr_last_error",
     "sap_dpsr_workspace_bytes", "sap_dpsr_last_launch_count", "sap_dpsr_set_profiling", "sap_dpsr_get_profile",
-    "sap_dpsr_epoch", "sap_dpsr_check_epoch", "sap_dpsr_reserve",
+    "sap_dpsr_epoch", "sap_dpsr_check_epoch", "sap_dpsr_reserve", "sap_dpsr_set_path", "sap_dpsr_get_path",
+    "sap_dpsr_get_fused_phases",
 ]
+SAP_PATH_AUTO, SAP_PATH_THROUGHPUT, SAP_PATH_LATENCY = 0, 1, 2
+PATHS = {"auto": 0, "throughput": 1, "latency": 2}
 SAP_RESERVE_MSE, SAP_RESERVE_HOST = 1, 2
 
 _lib = None
@@ -74,6 +77,12 @@ def lib():
     L.sap_dpsr_check_epoch.restype = ci
     L.sap_dpsr_reserve.argtypes = [vp, ci]
     L.sap_dpsr_reserve.restype = ci
+    L.sap_dpsr_set_path.argtypes = [vp, ci]
+    L.sap_dpsr_set_path.restype = ci
+    L.sap_dpsr_get_path.argtypes = [vp]
+    L.sap_dpsr_get_path.restype = ci
+    L.sap_dpsr_get_fused_phases.argtypes = [vp, ctypes.POINTER(cf), ctypes.POINTER(ctypes.c_char_p), ci]
+    L.sap_dpsr_get_fused_phases.restype = ci
     _lib = L
     return L
 
@@ -209,6 +218,22 @@ class Dpsr:
     def reserve(self, mse=False, host=False):
         """Allocates the optional buffers of the fused-loss / host-buffer entry points up front."""
         self._check(lib().sap_dpsr_reserve(self._h, (SAP_RESERVE_MSE if mse else 0) | (SAP_RESERVE_HOST if host else 0)))
+
+    def set_path(self, path):
+        """'auto' | 'throughput' | 'latency' (include/sap_dpsr.h, SAP_PATH_*)."""
+        self._check(lib().sap_dpsr_set_path(self._h, PATHS[path] if isinstance(path, str) else int(path)))
+
+    @property
+    def path(self):
+        return {1: "throughput", 2: "latency"}.get(int(lib().sap_dpsr_get_path(self._h)), "?")
+
+    def fused_phases(self):
+        """[(phase label, microseconds)] between the grid barriers of the last latency-path forward / backward."""
+        cap = 64
+        us = (ctypes.c_float * cap)()
+        names = (ctypes.c_char_p * cap)()
+        n = lib().sap_dpsr_get_fused_phases(self._h, us, names, cap)
+        return [(names[i].decode(), float(us[i])) for i in range(n)]
 
     def set_profiling(self, on=True):
         self._check(lib().sap_dpsr_set_profiling(self._h, int(bool(on))))

@@ -10,11 +10,11 @@ PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libsap_dpsr.so"
 SOURCES = [CSRC / "sap_dpsr.cu"]
-HEADERS = [CSRC / "fft_core.cuh", CSRC / "dpsr_kernels.cuh", CSRC / "zy_pass.cuh", CSRC / "spectral.cuh", CSRC / "ring_pass.cuh", CSRC / "zline_pass.cuh", PKG.parent / "include" / "sap_dpsr.h"]
+HEADERS = [CSRC / "fft_core.cuh", CSRC / "fused_small.cuh", CSRC / "dpsr_kernels.cuh", CSRC / "zy_pass.cuh", CSRC / "spectral.cuh", CSRC / "ring_pass.cuh", CSRC / "zline_pass.cuh", PKG.parent / "include" / "sap_dpsr.h"]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-    "--expt-relaxed-constexpr", "-shared", "-Xcompiler", "-fPIC", "-Xptxas", "-v",
+    "--expt-relaxed-constexpr", *os.environ.get("SAP_NVCC_EXTRA", "").split(), "-shared", "-Xcompiler", "-fPIC", "-Xptxas", "-v",
 ]
 
 

@@ -6,11 +6,13 @@
 #include <math.h>
 #include <stdio.h>
 #include <string.h>
+#include <stdlib.h>
 #include <new>
 #include <string>
 
 #include "../../include/sap_dpsr.h"
 #include "dpsr_kernels.cuh"
+#include "fused_small.cuh"
 
 namespace sap {
 
@@ -393,6 +395,14 @@ struct sap_dpsr {
     float* gmse = nullptr;     // [B][N^3] G = 2 (chi - chi_gt)
     double* acc_mse = nullptr; // [B][3]   S0, S1, L accumulators
     bool mse_valid = false;    // bw and gmse belong to the last forward
+    // latency path (fused_small.cuh): one cooperative kernel per direction when all x-planes fit one wave of CTAs
+    bool fused_ok = false;     // N <= 128 and batch * N <= #SMs
+    int path = SAP_PATH_AUTO;
+    int fused_pdl = 1;         // the cooperative launch also takes the programmatic-serialization attribute (probed on first use)
+    int* fhist = nullptr;      // [B][#SMs][N]
+    double* facc = nullptr;    // [B][2]
+    unsigned* fsync = nullptr; // [4] barrier arrivals, exits, time-out flag
+    long long* fstamps = nullptr;  // [64] clock64 of CTA 0 at the marks of the phase bodies
     size_t ws_bytes = 0;
     int launches = 0;
     // optional per-kernel timing (sap_dpsr_set_profiling): one event before the first launch, one after each
@@ -523,6 +533,10 @@ template <int N> struct Runner {
             upd(set_smem(k_ring<N, MODE_INV3>, ring_smem_bytes<N, MODE_INV3>()));
             upd(set_smem(k_ring<N, MODE_INV>, ring_smem_bytes<N, MODE_INV>()));
         }
+        if constexpr (N <= 128) {
+            upd(set_smem(k_fused_fwd<N>, FusedCfg<N>::BYTES));
+            upd(set_smem(k_fused_bwd<N>, FusedCfg<N>::BYTES));
+        }
         if (!cuda_ok(h, e, "cudaFuncSetAttribute")) return SAP_ERR_CUDA;
         // TMA descriptors: tile = NB points along the pass axis x W contiguous kz (or y, Nyquist plane) slots
         constexpr cuuint32_t W2 = 2 * RingCfg<N>::W, NB = ring_box_rows<N>();
@@ -574,11 +588,62 @@ template <int N> struct Runner {
         launch_pdl(k_zl_inv<N>, dim3((unsigned)grid), dim3(zl_threads<N, true>()), zl_smem_bytes<N, true>(), st, p);
     }
 
+    // ---- latency path: the whole forward / backward as one cooperative kernel (fused_small.cuh) ----
+    static FusedParams fused_params(sap_dpsr* h, const float* pts, const float* nrm, int P, float* chi, const float* G, float* gp, float* gn) {
+        FusedParams p;
+        p.pts = pts; p.nrm = nrm; p.chi = chi; p.G = G; p.gp = gp; p.gn = gn; p.P = P; p.B = h->batch;
+        p.spts = h->spts; p.snrm = h->snrm; p.bin_start = h->bin_start; p.hist = h->fhist;
+        p.S3 = h->S3; p.Q3 = h->Q3; p.S1 = h->S1; p.Q1 = h->Q1; p.tw = h->tw; p.ftab = h->ftab;
+        p.acc = h->facc; p.stats = h->stats; p.bw = h->bw; p.sync = h->fsync; p.stamps = h->fstamps;
+        p.cs = (float)((2.0 / ((double)N * N * N)) / (-2.0 * 3.14159265358979323846));
+        return p;
+    }
+    template <class K> static cudaError_t launch_fused(sap_dpsr* h, K kernel, cudaStream_t st, const FusedParams& p) {
+        if constexpr (N <= 128) {
+            cudaLaunchConfig_t cfg = {};
+            cfg.gridDim = dim3((unsigned)h->num_sms); cfg.blockDim = dim3(FusedCfg<N>::NT);
+            cfg.dynamicSmemBytes = FusedCfg<N>::BYTES; cfg.stream = st;
+            cudaLaunchAttribute at[2];
+            at[0].id = cudaLaunchAttributeCooperative; at[0].val.cooperative = 1;
+            at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization; at[1].val.programmaticStreamSerializationAllowed = 1;
+            static const bool coop = !(getenv("SAP_FUSED_COOP") && getenv("SAP_FUSED_COOP")[0] == '0');
+            if (!coop) at[0] = at[1];   // experiment: plain launch (148 CTAs of one per SM are co-resident in practice)
+            cfg.attrs = at; cfg.numAttrs = (coop && h->fused_pdl) ? 2 : 1;
+            cudaError_t e = cudaLaunchKernelEx(&cfg, kernel, p);
+            if (e != cudaSuccess && h->fused_pdl) {  // this driver does not combine the two attributes: cooperative only
+                cudaGetLastError();
+                h->fused_pdl = 0;
+                cfg.numAttrs = 1;
+                e = cudaLaunchKernelEx(&cfg, kernel, p);
+            }
+            return e;
+        } else {
+            return cudaErrorInvalidValue;
+        }
+    }
+    // SAP_PATH_AUTO: the latency path where it measured at least as fast as the 13-launch chain with a flushed L2 and
+    // clearly faster back to back / from the host (2 launches instead of 13): N <= 64.  At 128^3 the chain of
+    // programmatic dependent launches hides its launch latencies and wins (DESIGN.md 8a has the phase table).
+    static bool use_fused(const sap_dpsr* h) {
+        if (!h->fused_ok || h->path == SAP_PATH_THROUGHPUT) return false;
+        return h->path == SAP_PATH_LATENCY || N <= 64;
+    }
+
     static sap_status_t forward(sap_dpsr* h, const float* pts, const float* nrm, int P, float* chi, cudaStream_t st,
                                 const float* chi_gt = nullptr, float* loss = nullptr) {
         const int B = h->batch;
         const size_t V = (size_t)N * N * N;
         prof_begin(h, st);
+        if constexpr (N <= 128) {
+            if (use_fused(h) && !chi_gt) {
+                const FusedParams p = fused_params(h, pts, nrm, P, chi, nullptr, nullptr, nullptr);
+                if (!cuda_ok(h, launch_fused(h, k_fused_fwd<N>, st, p), "k_fused_fwd")) return SAP_ERR_CUDA;
+                SAP_LAUNCH_CHECK(h, "k_fused_fwd");
+                h->binned_P = P;
+                h->mse_valid = false;
+                return SAP_OK;
+            }
+        }
         // F1a: bin the points (counting sort); the rasterisation itself happens inside k_zy_fwd
         {
             const dim3 gp((P + 255) / 256, B);
@@ -636,6 +701,14 @@ template <int N> struct Runner {
         const int B = h->batch;
         const size_t V = (size_t)N * N * N;
         prof_begin(h, st);
+        if constexpr (N <= 128) {
+            if (use_fused(h) && !have_bw) {
+                const FusedParams p = fused_params(h, pts, nrm, P, const_cast<float*>(chi), gchi, gp, gn);
+                if (!cuda_ok(h, launch_fused(h, k_fused_bwd<N>, st, p), "k_fused_bwd")) return SAP_ERR_CUDA;
+                SAP_LAUNCH_CHECK(h, "k_fused_bwd");
+                return SAP_OK;
+            }
+        }
         // B1 reductions (already done by the fused loss pass of sap_dpsr_forward_mse)
         if (!have_bw) {
             const size_t n4 = V / 4;
@@ -697,6 +770,7 @@ static bool supported_N(int N) { return N == 32 || N == 64 || N == 128 || N == 2
 static void free_all(sap_dpsr* h) {
     for (int i = 0; i < sap_dpsr::MAX_EV; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
     cudaFree(h->v); cudaFree(h->spts); cudaFree(h->snrm); cudaFree(h->bin_cnt); cudaFree(h->bin_cursor); cudaFree(h->bin_start); cudaFree(h->S3); cudaFree(h->Q3); cudaFree(h->S1); cudaFree(h->Q1); cudaFree(h->QT3); cudaFree(h->QT1); cudaFree(h->tw); cudaFree(h->ftab);
+    cudaFree(h->fhist); cudaFree(h->facc); cudaFree(h->fsync); cudaFree(h->fstamps);
     cudaFree(h->gmse); cudaFree(h->acc_mse); cudaFree(h->acc); cudaFree(h->ticket); cudaFree(h->stats); cudaFree(h->bw);
     cudaFree(h->h_pts); cudaFree(h->h_nrm); cudaFree(h->h_chi); cudaFree(h->h_gchi); cudaFree(h->h_gp); cudaFree(h->h_gn);
 }
@@ -738,6 +812,13 @@ extern "C" sap_status_t sap_dpsr_create(int N, float sigma, int batch, int max_p
     upd(dev_alloc(h, &h->ticket, B * 2));
     upd(dev_alloc(h, &h->stats, B * 4));
     upd(dev_alloc(h, &h->bw, B * 4));
+    h->fused_ok = (N <= 128) && ((long long)batch * N <= h->num_sms) && batch <= (N == 32 ? 4 : N == 64 ? 2 : 1);
+    if (h->fused_ok) {
+        upd(dev_alloc(h, &h->fhist, B * (size_t)h->num_sms * N));
+        upd(dev_alloc(h, &h->facc, B * 2));
+        upd(dev_alloc(h, &h->fsync, (size_t)4));
+        upd(dev_alloc(h, &h->fstamps, (size_t)64));
+    }
     if (e != cudaSuccess) {
         cuda_ok(nullptr, e, "cudaMalloc(workspace)");
         const bool oom = (e == cudaErrorMemoryAllocation);
@@ -758,6 +839,11 @@ extern "C" sap_status_t sap_dpsr_create(int N, float sigma, int batch, int max_p
     upd(cudaMemset(h->ticket, 0, sizeof(unsigned) * B * 2));
     upd(cudaMemset(h->stats, 0, sizeof(float) * B * 4));
     upd(cudaMemset(h->bw, 0, sizeof(float) * B * 4));
+    if (h->fused_ok) {
+        upd(cudaMemset(h->facc, 0, sizeof(double) * B * 2));
+        upd(cudaMemset(h->fsync, 0, sizeof(unsigned) * 4));
+        upd(cudaMemset(h->fstamps, 0, sizeof(long long) * 64));
+    }
     sap_status_t st = SAP_OK;
     if (e != cudaSuccess) { cuda_ok(nullptr, e, "workspace init"); st = SAP_ERR_CUDA; }
     if (st == SAP_OK) {
@@ -930,8 +1016,18 @@ extern "C" sap_status_t sap_dpsr_get_stats(sap_dpsr_t* h, float* stats_host, voi
     cudaStream_t s = (cudaStream_t)stream;
     float* tmp = new (std::nothrow) float[(size_t)h->batch * 4];
     if (!tmp) { h->err = "host allocation failed"; return SAP_ERR_OOM; }
+    unsigned flag = 0;
     bool ok = cuda_ok(h, cudaMemcpyAsync(tmp, h->stats, sizeof(float) * 4 * h->batch, cudaMemcpyDeviceToHost, s), "D2H stats") &&
+              (!h->fsync || cuda_ok(h, cudaMemcpyAsync(&flag, h->fsync + 2, sizeof(unsigned), cudaMemcpyDeviceToHost, s), "D2H flag")) &&
               cuda_ok(h, cudaStreamSynchronize(s), "cudaStreamSynchronize");
+    if (ok && flag) {  // a grid barrier of the fused path gave up waiting (the CTAs of the launch were not co-resident)
+        h->err = "fused path: grid barrier timed out; results of that call are invalid";
+        cudaMemsetAsync(h->fsync, 0, sizeof(unsigned) * 4, s);
+        cudaMemsetAsync(h->facc, 0, sizeof(double) * 2 * h->batch, s);
+        cudaStreamSynchronize(s);
+        delete[] tmp;
+        return SAP_ERR_CUDA;
+    }
     if (ok) for (int b = 0; b < h->batch; ++b) for (int k = 0; k < 3; ++k) stats_host[b * 3 + k] = tmp[b * 4 + k];
     delete[] tmp;
     return ok ? SAP_OK : SAP_ERR_CUDA;
@@ -969,6 +1065,55 @@ extern "C" sap_status_t sap_dpsr_reserve(sap_dpsr_t* h, int what) {
 extern "C" const char* sap_dpsr_last_error(const sap_dpsr_t* h) { return h ? h->err.c_str() : g_create_err.c_str(); }
 extern "C" size_t sap_dpsr_workspace_bytes(const sap_dpsr_t* h) { return h ? h->ws_bytes : 0; }
 extern "C" int sap_dpsr_last_launch_count(const sap_dpsr_t* h) { return h ? h->launches : 0; }
+
+extern "C" sap_status_t sap_dpsr_set_path(sap_dpsr_t* h, int path) {
+    if (!h) return SAP_ERR_INVALID_ARG;
+    h->err.clear();
+    if (path != SAP_PATH_AUTO && path != SAP_PATH_THROUGHPUT && path != SAP_PATH_LATENCY) { h->err = "unknown path"; return SAP_ERR_INVALID_ARG; }
+    if (path == SAP_PATH_LATENCY && !h->fused_ok) {
+        h->err = "the latency path needs N <= 128 and batch * N <= number of SMs";
+        return SAP_ERR_UNSUPPORTED;
+    }
+    h->path = path;
+    return SAP_OK;
+}
+extern "C" int sap_dpsr_get_path(const sap_dpsr_t* h) {
+    if (!h) return -1;
+    if (!h->fused_ok || h->path == SAP_PATH_THROUGHPUT) return SAP_PATH_THROUGHPUT;
+    return (h->path == SAP_PATH_LATENCY || h->N <= 64) ? SAP_PATH_LATENCY : SAP_PATH_THROUGHPUT;
+}
+// marks of the last fused forward (ids 0..28) and backward (32..52), stamped by CTA 0 with clock64
+extern "C" int sap_dpsr_get_fused_phases(sap_dpsr_t* h, float* us, const char** names, int cap) {
+    if (!h || !h->fstamps) return 0;
+    long long t[64];
+    if (cudaMemcpy(t, h->fstamps, sizeof t, cudaMemcpyDeviceToHost) != cudaSuccess) { cudaGetLastError(); return 0; }
+    int khz = 1965000;
+    cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, h->device);   // cycles -> microseconds at the nominal SM clock
+    static const char* nm[64] = {};
+    if (!nm[1]) {
+        nm[1] = "F:hist"; nm[2] = "F:barrier1"; nm[3] = "F:offsets+scatter"; nm[4] = "F:barrier2"; nm[5] = "F:zero planes";
+        nm[6] = "F:rasterise"; nm[7] = "F:z stage0"; nm[8] = "F:z stage1"; nm[9] = "F:split+y stage0"; nm[10] = "F:y last->HBM";
+        nm[12] = "F:barrier3"; nm[13] = "F:x load+stage0"; nm[14] = "F:x last+solve"; nm[15] = "F:x inverse->HBM";
+        nm[16] = "F:barrier4"; nm[17] = "F:load plane"; nm[22] = "F:inv y last"; nm[23] = "F:inv y stage0+split"; nm[24] = "F:inv z stage1";
+        nm[25] = "F:inv z stage0"; nm[26] = "F:sample mean"; nm[27] = "F:barrier5"; nm[28] = "F:scale+store";
+        nm[33] = "B:load+reduce+zero"; nm[34] = "B:barrier1"; nm[36] = "B:chi term+raster W"; nm[37] = "B:z stage0"; nm[38] = "B:z stage1";
+        nm[39] = "B:split+y stage0"; nm[40] = "B:y last->HBM"; nm[42] = "B:barrier2"; nm[43] = "B:x load+stage0"; nm[44] = "B:x last+adjoint";
+        nm[45] = "B:x inverse x2->HBM"; nm[46] = "B:barrier3"; nm[47] = "B:load planes"; nm[48] = "B:inv y last x3"; nm[49] = "B:inv y stage0+split x3"; nm[50] = "B:inv z stage1 x3";
+        nm[51] = "B:inv z stage0 x3"; nm[52] = "B:gather";
+    }
+    int n = 0, prev = -1;
+    for (int i = 0; i < 64 && n < cap; ++i) {
+        if (i == 32) prev = -1;   // the backward is another launch (maybe another SM): its clock has another origin
+        if (t[i] == 0) continue;
+        if (prev >= 0 && nm[i] && t[i] >= t[prev]) {
+            if (us) us[n] = (float)((double)(t[i] - t[prev]) / ((double)khz * 1e-3));
+            if (names) names[n] = nm[i];
+            ++n;
+        }
+        prev = i;
+    }
+    return n;
+}
 
 extern "C" sap_status_t sap_dpsr_set_profiling(sap_dpsr_t* h, int on) {
     if (!h) return SAP_ERR_INVALID_ARG;

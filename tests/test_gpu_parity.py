@@ -13,11 +13,12 @@ CHI_TOL = 1e-4
 GRAD_TOL = 1e-3
 
 
-def _gpu_run(N, sigma, pts, nrm, G):
+def _gpu_run(N, sigma, pts, nrm, G, path="auto"):
     import torch
     from paper_2106_03452_b200.binding import Dpsr
     B, P = pts.shape[0], pts.shape[1]
     h = Dpsr(N, sigma, B, P)
+    h.set_path(path)
     tp, tn = torch.from_numpy(pts).cuda(), torch.from_numpy(nrm).cuda()
     chi = h.forward(tp, tn)
     stats = h.stats()
@@ -35,6 +36,7 @@ def _check_item(N, sigma, pts, nrm, G, got_chi, got_stats, got_gp, got_gn):
     err = np.abs(got_chi - f["chi"]).max() / np.abs(f["chi"]).max()
     assert err <= CHI_TOL, f"chi rel-max err {err:.3e}"
     assert abs(got_stats[0] - f["mu"]) <= 1e-4 * abs(f["a"])
+    assert abs(got_stats[1] - f["a"]) <= 1e-4 * abs(f["a"])
     assert abs(got_stats[2] - f["s"]) <= 1e-4 * f["s"]
     if G is not None:
         b = orc.backward(N, sigma, pts, nrm, f, G)
@@ -44,21 +46,28 @@ def _check_item(N, sigma, pts, nrm, G, got_chi, got_stats, got_gp, got_gn):
     return err
 
 
+# both implementations of the path (include/sap_dpsr.h, SAP_PATH_*): the 13-launch throughput path and the
+# one-cooperative-kernel-per-direction latency path (N <= 128, batch * N <= #SMs)
+PATHS = ["throughput", "latency"]
+
+
+@pytest.mark.parametrize("path", PATHS)
 @pytest.mark.parametrize("cfg_id", [1, 2])
-def test_config_parity(cfg_id):
+def test_config_parity(cfg_id, path):
     cfg, pts, nrm = inputs.make_config(cfg_id)
     G = inputs.upstream_grad(cfg.N, 1)
-    r = _gpu_run(cfg.N, cfg.sigma, pts, nrm, G)
+    r = _gpu_run(cfg.N, cfg.sigma, pts, nrm, G, path)
     _check_item(cfg.N, cfg.sigma, pts[0], nrm[0], G[0], r["chi"][0], r["stats"][0], r["gp"][0], r["gn"][0])
     assert r["fwd_launches"] > 0 and r["bwd_launches"] > 0
 
 
 @pytest.mark.parametrize("N,P,sigma,shape", [(64, 5000, 2.0, "torus"), (32, 777, 3.0, "ellipsoids3"),
                                              (64, 1, 0.0, "sphere"), (128, 4099, 5.0, "bumpy")])
-def test_other_sizes_and_ragged_point_counts(N, P, sigma, shape):
+@pytest.mark.parametrize("path", PATHS)
+def test_other_sizes_and_ragged_point_counts(N, P, sigma, shape, path):
     pts, nrm = inputs.make_cloud(shape, P, seed=7)
     G = inputs.upstream_grad(N, 1, seed=3)
-    r = _gpu_run(N, sigma, pts[None], nrm[None], G)
+    r = _gpu_run(N, sigma, pts[None], nrm[None], G, path)
     _check_item(N, sigma, pts, nrm, G[0], r["chi"][0], r["stats"][0], r["gp"][0], r["gn"][0])
 
 
@@ -71,7 +80,69 @@ def test_batch_items_are_independent():
         _check_item(cfg.N, cfg.sigma, pts[b], nrm[b], G[b], r["chi"][b], r["stats"][b], r["gp"][b], r["gn"][b])
 
 
-def test_points_on_lattice_planes_and_wrap():
+@pytest.mark.parametrize("path", PATHS)
+def test_latency_path_small_batches(path):
+    # several items per launch on the latency path (32^3: up to 4, 64^3: up to 2); item b == the oracle on item b alone
+    for N, B, P in ((32, 4, 1500), (64, 2, 2500)):
+        cfg, pts, nrm = inputs.make_config(3, batch=B, P=P)
+        G = inputs.upstream_grad(N, B, seed=2)
+        r = _gpu_run(N, 2.0, pts, nrm, G, path)
+        for b in range(B):
+            _check_item(N, 2.0, pts[b], nrm[b], G[b], r["chi"][b], r["stats"][b], r["gp"][b], r["gn"][b])
+
+
+def test_paths_can_be_mixed_and_latency_needs_an_eligible_handle():
+    import torch
+    from paper_2106_03452_b200.binding import Dpsr, SapError
+    N, P = 64, 3000
+    pts, nrm = inputs.make_cloud("torus", P, seed=5)
+    G = inputs.upstream_grad(N, 1, seed=6)
+    f = orc.forward(N, 2.0, pts, nrm)
+    b = orc.backward(N, 2.0, pts, nrm, f, G[0])
+    h = Dpsr(N, 2.0, 1, P)
+    assert h.path == "latency"            # SAP_PATH_AUTO at 64^3
+    tp, tn, tG = torch.from_numpy(pts[None].copy()).cuda(), torch.from_numpy(nrm[None].copy()).cuda(), torch.from_numpy(G).cuda()
+    for fwd_path, bwd_path in (("latency", "throughput"), ("throughput", "latency")):
+        h.set_path(fwd_path)
+        chi = h.forward(tp, tn)
+        h.set_path(bwd_path)
+        gp, gn = h.backward(tp, tn, chi, tG)
+        torch.cuda.synchronize()
+        assert np.abs(chi.cpu().numpy()[0] - f["chi"]).max() <= CHI_TOL * np.abs(f["chi"]).max()
+        assert np.linalg.norm(gp.cpu().numpy()[0] - b["grad_points"]) <= GRAD_TOL * np.linalg.norm(b["grad_points"])
+        assert np.linalg.norm(gn.cpu().numpy()[0] - b["grad_normals"]) <= GRAD_TOL * np.linalg.norm(b["grad_normals"])
+    assert len(h.fused_phases()) > 0
+    h.close()
+    big = Dpsr(128, 2.0, 2, 100)          # batch * N > #SMs: not eligible
+    assert big.path == "throughput"
+    with pytest.raises(SapError):
+        big.set_path("latency")
+    big.close()
+    h128 = Dpsr(128, 2.0, 1, 100)          # eligible, but AUTO keeps the throughput path at 128^3
+    assert h128.path == "throughput"
+    h128.set_path("latency")
+    assert h128.path == "latency"
+    h128.close()
+
+
+def test_splat_is_bit_reproducible_on_the_latency_path():
+    # the latency path rasterises with integer (fixed-point) atomics: chi' is independent of the order of the adds;
+    # only mu (double atomics over <= 148 partial sums) could differ in its last bits
+    import torch
+    from paper_2106_03452_b200.binding import Dpsr
+    cfg, pts, nrm = inputs.make_config(1)
+    h = Dpsr(cfg.N, cfg.sigma, 1, cfg.P)
+    h.set_path("latency")
+    tp, tn = torch.from_numpy(pts).cuda(), torch.from_numpy(nrm).cuda()
+    a = h.forward(tp, tn).clone()
+    for _ in range(3):
+        b = h.forward(tp, tn)
+        assert (a - b).abs().max().item() <= 2e-7 * a.abs().max().item()
+    h.close()
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_points_on_lattice_planes_and_wrap(path):
     # degenerate positions: exactly on vertices, in the last cell (periodic wrap), coincident pairs
     N, sigma = 32, 2.0
     pts, nrm = inputs.make_cloud("sphere", 500, seed=11)
@@ -80,8 +151,139 @@ def test_points_on_lattice_planes_and_wrap():
     pts[60:70, 2] = 0.0
     pts[70:80] = pts[80:90]
     nrm[70:80] = -nrm[80:90]
-    r = _gpu_run(N, sigma, pts[None], nrm[None], None)
+    r = _gpu_run(N, sigma, pts[None], nrm[None], None, path)
     _check_item(N, sigma, pts, nrm, None, r["chi"][0], r["stats"][0], None, None)
+
+
+def _wrap_cloud(N, P, shape, seed, tile=32):
+    """A cloud pushed against the faces of the cube: points in the first and last cell of every axis, points exactly
+    on y-tile boundaries (multiples of tile/N: the bins of the N >= 256 kernels) and a few just below 1.0."""
+    pts, nrm = inputs.make_cloud(shape, P, seed=seed)
+    rng = np.random.default_rng(seed + 100)
+    k = P // 10
+    for a in range(3):
+        pts[a * k:(a + 1) * k, a] = rng.uniform(0.0, 1.0 / N, k)                       # first cell
+        pts[(3 + a) * k:(4 + a) * k, a] = rng.uniform(1.0 - 1.0 / N, 1.0 - 1e-7, k)    # last cell: +1 corner wraps to 0
+    pts[6 * k:7 * k, 1] = (rng.integers(0, N // tile, k) * tile + rng.uniform(0.0, 1.0, k) * (rng.uniform(0, 1, k) < 0.5)) / N
+    pts[7 * k:8 * k, 1] = (rng.integers(1, N // tile + 1, k) * tile - rng.uniform(0.0, 1.0, k)) / N
+    pts = np.clip(pts, 0.0, np.float32(1.0 - 6e-8)).astype(np.float32)
+    # gradients are undefined ON lattice planes (SURVEY 8(c)): nudge coordinates that sit within 1e-3 cell of one
+    t = pts.astype(np.float64) * N
+    near = np.abs(t - np.round(t)) < 1e-3
+    pts = np.where(near, (np.round(t) + 0.37) / N, pts).astype(np.float32)
+    pts = np.clip(pts, 0.0, np.float32(1.0 - 6e-8)).astype(np.float32)
+    return pts, nrm
+
+
+def test_wrapping_points_forward_and_backward_batched_128():
+    # periodic wrap through the backward (re-rasterised W, gather) with batch > 1 (ADVICE r1)
+    N, P, B = 128, 3000, 2
+    pts = np.empty((B, P, 3), np.float32)
+    nrm = np.empty((B, P, 3), np.float32)
+    for b in range(B):
+        pts[b], nrm[b] = _wrap_cloud(N, P, "ellipsoids3", seed=20 + b)
+    G = inputs.upstream_grad(N, B, seed=9)
+    r = _gpu_run(N, 2.0, pts, nrm, G)
+    for b in range(B):
+        _check_item(N, 2.0, pts[b], nrm[b], G[b], r["chi"][b], r["stats"][b], r["gp"][b], r["gn"][b])
+
+
+@pytest.mark.slow
+def test_wrapping_points_forward_and_backward_256():
+    # N >= 256 paths: y-tile wrap (ty + NTY - 1) % NTY, x-slab wrap with NTY > 1, transposed Nyquist planes (ADVICE r1)
+    N, P = 256, 20000
+    pts, nrm = _wrap_cloud(N, P, "ellipsoids8", seed=31)
+    G = inputs.upstream_grad(N, 1, seed=10)
+    r = _gpu_run(N, 2.0, pts[None], nrm[None], G)
+    _check_item(N, 2.0, pts, nrm, G[0], r["chi"][0], r["stats"][0], r["gp"][0], r["gn"][0])
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_non_unit_and_near_zero_normals(path):
+    # normals are not normalised; a near-zero normal mutes its point (PAPER.md:L494)
+    N, P = 64, 4000
+    pts, nrm = inputs.make_cloud("ellipsoids3", P, seed=12)
+    rng = np.random.default_rng(5)
+    nrm = (nrm * rng.uniform(0.2, 5.0, (P, 1))).astype(np.float32)
+    nrm[:400] *= np.float32(1e-6)
+    nrm[400:420] = 0.0
+    G = inputs.upstream_grad(N, 1, seed=13)
+    r = _gpu_run(N, 3.0, pts[None], nrm[None], G, path)
+    _check_item(N, 3.0, pts, nrm, G[0], r["chi"][0], r["stats"][0], r["gp"][0], r["gn"][0])
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_backward_with_fewer_points_than_max_points(path):
+    import torch
+    from paper_2106_03452_b200.binding import Dpsr
+    N, Pmax, P = 64, 6000, 2500
+    pts, nrm = inputs.make_cloud("torus", P, seed=14)
+    G = inputs.upstream_grad(N, 1, seed=15)
+    h = Dpsr(N, 2.0, 1, Pmax)
+    h.set_path(path)
+    tp, tn = torch.from_numpy(pts[None].copy()).cuda(), torch.from_numpy(nrm[None].copy()).cuda()
+    chi = h.forward(tp, tn)
+    gp, gn = h.backward(tp, tn, chi, torch.from_numpy(G).cuda())
+    torch.cuda.synchronize()
+    _check_item(N, 2.0, pts, nrm, G[0], chi.cpu().numpy()[0], h.stats()[0], gp.cpu().numpy()[0], gn.cpu().numpy()[0])
+    h.close()
+
+
+def test_stale_forward_is_detected():
+    # ADVICE r1: two forwards through one handle before a backward must not silently use the other cloud's state
+    import torch
+    from paper_2106_03452_b200.binding import Dpsr, SapError, dpsr
+    N, P = 32, 1000
+    h = Dpsr(N, 2.0, 1, P)
+    clouds = [inputs.make_cloud(s, P, seed=3) for s in ("sphere", "torus")]
+    tp = [torch.from_numpy(c[0][None].copy()).cuda().requires_grad_(True) for c in clouds]
+    tn = [torch.from_numpy(c[1][None].copy()).cuda().requires_grad_(True) for c in clouds]
+    f = dpsr(h)
+    chi0 = f(tp[0], tn[0])
+    e0 = h.epoch
+    chi1 = f(tp[1], tn[1])                 # evaluation forward in between
+    assert h.epoch == e0 + 1
+    with pytest.raises(SapError):
+        chi0.sum().backward()              # bins and statistics now belong to cloud 1
+    chi1.sum().backward()                  # the latest forward is still differentiable
+    assert tp[1].grad is not None
+    # host forward followed by a device forward: backward_host must refuse
+    hp, hn = torch.from_numpy(clouds[0][0][None].copy()), torch.from_numpy(clouds[0][1][None].copy())
+    h.forward_host(hp, hn, None)
+    h.forward(tp[1].detach(), tn[1].detach())
+    with pytest.raises(SapError):
+        h.backward_host(torch.zeros((1, N, N, N)), torch.empty((1, P, 3)), torch.empty((1, P, 3)))
+    h.close()
+
+
+def test_reserve_makes_first_fused_loss_call_capturable():
+    # sap_dpsr_reserve: the optional buffers exist before the first call, so that call can be captured in a CUDA graph
+    import torch
+    from paper_2106_03452_b200.binding import Dpsr
+    cfg, pts, nrm = inputs.make_config(3, batch=1, P=2000)
+    N = cfg.N
+    h = Dpsr(N, cfg.sigma, 1, 2000)
+    ws0 = h.workspace_bytes
+    h.reserve(mse=True, host=True)
+    assert h.workspace_bytes > ws0
+    ws1 = h.workspace_bytes
+    tp, tn = torch.from_numpy(pts).cuda(), torch.from_numpy(nrm).cuda()
+    gt = torch.zeros((1, N, N, N), device="cuda")
+    chi = torch.empty((1, N, N, N), device="cuda")
+    loss = torch.empty((1,), device="cuda")
+    gp, gn = torch.empty_like(tp), torch.empty_like(tn)
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):          # very first forward_mse on this handle, inside capture
+        h.forward_mse(tp, tn, gt, chi, loss)
+        h.backward_mse(tp, tn, chi, gp, gn)
+    graph.replay()
+    torch.cuda.synchronize()
+    assert h.workspace_bytes == ws1
+    f = orc.forward(N, cfg.sigma, pts[0], nrm[0])
+    assert abs(loss.item() - (f["chi"] ** 2).sum()) <= 1e-4 * (f["chi"] ** 2).sum()
+    del graph
+    h.close()
 
 
 @pytest.mark.slow
@@ -193,6 +395,7 @@ def test_repeatable_and_handle_reuse():
     cfg, pts, nrm = inputs.make_config(1)
     h = Dpsr(cfg.N, cfg.sigma, 1, cfg.P)
     tp, tn = torch.from_numpy(pts).cuda(), torch.from_numpy(nrm).cuda()
+    h.set_path("throughput")
     a = h.forward(tp, tn).clone()
     b = h.forward(tp, tn)
     # only the atomics' summation order may differ between two runs
