@@ -1,0 +1,631 @@
+// sap_mesh.cu -- the mesh side of the optimisation-based pipeline (include/sap_mesh.h): Marching Cubes on the indicator
+// grid, the surrogate gradient of Eq.6 (L113-L117) and the bi-directional L2 Chamfer distance (L102),
+// all on the device with data-dependent sizes kept in device memory.  Readings M1-M6: DESIGN.md / sap_mesh.h.
+//
+//   Marching Cubes: classify (per node: which of its 3 owned edges cross, sign configuration and triangle count of its
+//   cell; per-block totals) -> exclusive scan of the block totals -> emit vertices (per-node offsets from an in-block
+//   scan; position, normal, t) -> emit triangles (vertex ids looked up through the per-node offsets).  No atomics, so
+//   vertex and triangle order are fixed: increasing (node, axis) and increasing cell.
+//   Eq.6: owner-computes gather per grid node over its <= 6 incident edges (no atomics, no memset, deterministic).
+//   Chamfer: counting sort of each set into a uniform cell grid, exact nearest neighbour by ring search, lowest index wins
+//   an exact tie.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdio.h>
+#include <new>
+#include <string>
+
+#include "../../include/sap_mesh.h"
+
+namespace sapm {
+
+// ---- cube triangulation by rule M3, built on the host --------------------------------------------------------------
+constexpr int MAX_TRI = 12;
+struct CubeTables {
+    unsigned char ntri[256];
+    signed char tri[256][MAX_TRI * 3];
+    int max_tri;
+};
+static int ins_bit(int v, int pos, int bit) { return (v & ((1 << pos) - 1)) | (bit << pos) | ((v >> pos) << (pos + 1)); }
+static int del_bit(int v, int pos) { return (v & ((1 << pos) - 1)) | ((v >> (pos + 1)) << pos); }
+static int edge_of(int ca, int cb) {   // cube edge joining two adjacent corners
+    const int d = ca ^ cb;
+    const int a = (d == 1) ? 0 : (d == 2) ? 1 : 2;
+    return 4 * a + del_bit(ca, a);
+}
+static void build_case(int cfg, CubeTables& T) {
+    int link[12][2], nlink[12];
+    bool cut[12];
+    for (int e = 0; e < 12; ++e) {
+        const int a = e >> 2, c0 = ins_bit(e & 3, a, 0), c1 = c0 | (1 << a);
+        cut[e] = (((cfg >> c0) ^ (cfg >> c1)) & 1) != 0;
+        nlink[e] = 0;
+    }
+    auto join = [&](int ea, int eb) { link[ea][nlink[ea]++] = eb; link[eb][nlink[eb]++] = ea; };
+    static const int gray[4] = {0, 1, 3, 2};   // (u, v) = (0,0), (1,0), (1,1), (0,1)
+    for (int a = 0; a < 3; ++a)
+        for (int side = 0; side < 2; ++side) {
+            int corner[4], fedge[4], inside[4], ncut = 0;
+            for (int i = 0; i < 4; ++i) {
+                corner[i] = ins_bit(gray[i], a, side);
+                inside[i] = (cfg >> corner[i]) & 1;
+            }
+            for (int i = 0; i < 4; ++i) {
+                fedge[i] = edge_of(corner[i], corner[(i + 1) & 3]);
+                ncut += inside[i] != inside[(i + 1) & 3];
+            }
+            if (ncut == 2) {
+                int first = -1;
+                for (int i = 0; i < 4; ++i)
+                    if (inside[i] != inside[(i + 1) & 3]) {
+                        if (first < 0) first = fedge[i];
+                        else join(first, fedge[i]);
+                    }
+            } else if (ncut == 4) {
+                for (int i = 0; i < 4; ++i)
+                    if (inside[i]) join(fedge[(i + 3) & 3], fedge[i]);   // cut each INSIDE corner off on its own
+            }
+        }
+    bool done[12] = {};
+    int nt = 0;
+    for (int start = 0; start < 12; ++start) {
+        if (!cut[start] || done[start]) continue;
+        int loop[12], n = 0;
+        for (int prev = -1, cur = start;;) {
+            loop[n++] = cur;
+            done[cur] = true;
+            const int next = (n == 1 || link[cur][0] != prev) ? link[cur][0] : link[cur][1];
+            prev = cur;
+            cur = next;
+            if (cur == start) break;
+        }
+        // orientation: loop normal (Newell, edge midpoints) must agree with the mean INSIDE -> OUTSIDE direction
+        double mid[12][3], out_dir[3] = {0, 0, 0}, nrm[3] = {0, 0, 0};
+        for (int i = 0; i < n; ++i) {
+            const int a = loop[i] >> 2, c0 = ins_bit(loop[i] & 3, a, 0);
+            for (int d = 0; d < 3; ++d) mid[i][d] = (d == a) ? 0.5 : (double)((c0 >> d) & 1);
+            out_dir[a] += ((cfg >> c0) & 1) ? 1.0 : -1.0;
+        }
+        for (int i = 0; i < n; ++i) {
+            const double* p = mid[i];
+            const double* q = mid[(i + 1) % n];
+            for (int d = 0; d < 3; ++d) {
+                const int d1 = (d + 1) % 3, d2 = (d + 2) % 3;
+                nrm[d] += (p[d1] - q[d1]) * (p[d2] + q[d2]);
+            }
+        }
+        const bool reverse = nrm[0] * out_dir[0] + nrm[1] * out_dir[1] + nrm[2] * out_dir[2] < 0.0;
+        for (int i = 1; i + 1 < n; ++i) {
+            const int v1 = reverse ? loop[n - i] : loop[i], v2 = reverse ? loop[n - i - 1] : loop[i + 1];
+            T.tri[cfg][3 * nt] = (signed char)loop[0];
+            T.tri[cfg][3 * nt + 1] = (signed char)v1;
+            T.tri[cfg][3 * nt + 2] = (signed char)v2;
+            ++nt;
+        }
+    }
+    T.ntri[cfg] = (unsigned char)nt;
+    for (int i = 3 * nt; i < 3 * MAX_TRI; ++i) T.tri[cfg][i] = -1;
+}
+static const CubeTables& cube_tables() {
+    static CubeTables T;
+    static bool built = false;
+    if (!built) {
+        T.max_tri = 0;
+        for (int cfg = 0; cfg < 256; ++cfg) {
+            build_case(cfg, T);
+            if (T.ntri[cfg] > T.max_tri) T.max_tri = T.ntri[cfg];
+        }
+        built = true;
+    }
+    return T;
+}
+
+__constant__ unsigned char c_ntri[256];
+__constant__ signed char c_tri[256 * MAX_TRI * 3];
+
+// ---- Marching Cubes kernels ----------------------------------------------------------------------------------------
+constexpr int MC_BLOCK = 256;
+struct Node { int x, y, z; };
+__device__ __forceinline__ Node node_xyz(unsigned n, int N, int lg) { return Node{(int)(n >> (2 * lg)), (int)((n >> lg) & (N - 1)), (int)(n & (N - 1))}; }
+__device__ __forceinline__ unsigned long long pack(unsigned nv, unsigned nt) { return ((unsigned long long)nt << 32) | nv; }
+
+// per node: code = crossing mask of its 3 owned edges (bit a: the edge towards +axis a) | triangle count of its cell << 3;
+// cfg = sign configuration of its cell; per block: (vertices, triangles) of its nodes
+__global__ void k_mc_classify(const float* __restrict__ chi, int N, int lg, unsigned char* __restrict__ code,
+                              unsigned char* __restrict__ cfg_out, unsigned long long* __restrict__ blocksum) {
+    __shared__ unsigned long long wsum[MC_BLOCK / 32];
+    const unsigned n = blockIdx.x * MC_BLOCK + threadIdx.x;   // N^3 is a multiple of MC_BLOCK
+    const Node j = node_xyz(n, N, lg);
+    const int sx = N * N, sy = N;
+    const bool hx = j.x + 1 < N, hy = j.y + 1 < N, hz = j.z + 1 < N;
+    const bool in0 = chi[n] < 0.f;
+    unsigned mask = 0, cfg = 0, nt = 0;
+    const bool i1 = hx && chi[n + sx] < 0.f, i2 = hy && chi[n + sy] < 0.f, i4 = hz && chi[n + 1] < 0.f;
+    if (hx && i1 != in0) mask |= 1u;
+    if (hy && i2 != in0) mask |= 2u;
+    if (hz && i4 != in0) mask |= 4u;
+    if (hx && hy && hz) {
+        cfg = (unsigned)in0 | ((unsigned)i1 << 1) | ((unsigned)i2 << 2) | ((unsigned)(chi[n + sx + sy] < 0.f) << 3) | ((unsigned)i4 << 4) |
+              ((unsigned)(chi[n + sx + 1] < 0.f) << 5) | ((unsigned)(chi[n + sy + 1] < 0.f) << 6) | ((unsigned)(chi[n + sx + sy + 1] < 0.f) << 7);
+        nt = c_ntri[cfg];
+    }
+    code[n] = (unsigned char)(mask | (nt << 3));
+    cfg_out[n] = (unsigned char)cfg;
+    unsigned long long s = pack(__popc(mask), nt);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned long long t = 0;
+        for (int w = 0; w < MC_BLOCK / 32; ++w) t += wsum[w];
+        blocksum[blockIdx.x] = t;
+    }
+}
+// one block: exclusive scan of the block totals in place; counts = {V, T}
+__global__ void k_mc_scan_blocks(unsigned long long* __restrict__ blocksum, int nb, int* __restrict__ counts) {
+    __shared__ unsigned long long part[1024];
+    const int tid = threadIdx.x, per = (nb + 1023) / 1024;
+    const int lo = tid * per, hi = min(lo + per, nb);
+    unsigned long long s = 0;
+    for (int i = lo; i < hi; ++i) s += blocksum[i];
+    part[tid] = s;
+    __syncthreads();
+    for (int d = 1; d < 1024; d <<= 1) {   // Hillis-Steele, inclusive
+        const unsigned long long v = (tid >= d) ? part[tid - d] : 0ull;
+        __syncthreads();
+        part[tid] += v;
+        __syncthreads();
+    }
+    unsigned long long run = part[tid] - s;
+    for (int i = lo; i < hi; ++i) {
+        const unsigned long long v = blocksum[i];
+        blocksum[i] = run;
+        run += v;
+    }
+    if (tid == 1023) {
+        counts[0] = (int)(part[1023] & 0xffffffffull);
+        counts[1] = (int)(part[1023] >> 32);
+    }
+}
+// exclusive scan of one packed value per thread over the block (MC_BLOCK threads)
+__device__ __forceinline__ unsigned long long block_excl_scan(unsigned long long v, unsigned long long* wsum) {
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    unsigned long long inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const unsigned long long t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) wsum[w] = inc;
+    __syncthreads();
+    unsigned long long base = 0;
+    for (int i = 0; i < w; ++i) base += wsum[i];
+    return base + inc - v;
+}
+__global__ void k_mc_emit_verts(const float* __restrict__ chi, int N, int lg, const unsigned char* __restrict__ code,
+                                const unsigned long long* __restrict__ blockoff, unsigned* __restrict__ vprefix,
+                                unsigned* __restrict__ tprefix, float* __restrict__ verts, float* __restrict__ normals,
+                                float* __restrict__ vt, int max_v) {
+    __shared__ unsigned long long wsum[MC_BLOCK / 32];
+    const unsigned n = blockIdx.x * MC_BLOCK + threadIdx.x;
+    const unsigned cd = code[n], mask = cd & 7u;
+    const unsigned long long off = blockoff[blockIdx.x] + block_excl_scan(pack(__popc(mask), cd >> 3), wsum);
+    unsigned v = (unsigned)(off & 0xffffffffull);
+    vprefix[n] = v;
+    tprefix[n] = (unsigned)(off >> 32);
+    if (!mask) return;
+    const Node j = node_xyz(n, N, lg);
+    const int M = N - 1;
+    const float c0 = chi[n], hN = 0.5f * (float)N, inv = 1.f / (float)N;
+    auto at = [&](int x, int y, int z) { return chi[((unsigned)(x & M) << (2 * lg)) | ((unsigned)(y & M) << lg) | (unsigned)(z & M)]; };
+    auto grad = [&](int x, int y, int z, float* g) {   // central differences, periodic like chi itself (M4)
+        g[0] = hN * (at(x + 1, y, z) - at(x - 1, y, z));
+        g[1] = hN * (at(x, y + 1, z) - at(x, y - 1, z));
+        g[2] = hN * (at(x, y, z + 1) - at(x, y, z - 1));
+    };
+    float g0[3];
+    grad(j.x, j.y, j.z, g0);
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        if (!(mask & (1u << a))) continue;
+        const int kx = j.x + (a == 0), ky = j.y + (a == 1), kz = j.z + (a == 2);
+        const float c1 = at(kx, ky, kz);
+        const float t = c0 / (c0 - c1);
+        if ((int)v < max_v) {
+            float g1[3], g[3];
+            grad(kx, ky, kz, g1);
+            float nn = 0.f;
+#pragma unroll
+            for (int d = 0; d < 3; ++d) { g[d] = (1.f - t) * g0[d] + t * g1[d]; nn += g[d] * g[d]; }
+            const float rn = nn > 0.f ? 1.f / sqrtf(nn) : 0.f;
+            const float p[3] = {(float)j.x, (float)j.y, (float)j.z};
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                verts[3 * (size_t)v + d] = (p[d] + (d == a ? t : 0.f)) * inv;
+                normals[3 * (size_t)v + d] = g[d] * rn;
+            }
+            vt[v] = t;
+        }
+        ++v;
+    }
+}
+__global__ void k_mc_emit_tris(int N, int lg, const unsigned char* __restrict__ code, const unsigned char* __restrict__ cfgs,
+                               const unsigned* __restrict__ vprefix, const unsigned* __restrict__ tprefix, int* __restrict__ tris,
+                               int max_t) {
+    const unsigned n = blockIdx.x * MC_BLOCK + threadIdx.x;
+    const unsigned nt = code[n] >> 3;
+    if (!nt) return;
+    const unsigned cfg = cfgs[n], t0 = tprefix[n];
+    // vertex id on cube edge e of this cell: owned by node n + offset, axis a
+    auto vid = [&](int e) {
+        const int a = e >> 2, k = e & 3;
+        const int lo = k & 1, hi = k >> 1;
+        const int ox = (a == 0) ? 0 : lo, oy = (a == 1) ? 0 : (a == 0 ? lo : hi), oz = (a == 2) ? 0 : hi;
+        const unsigned m = n + ((unsigned)ox << (2 * lg)) + ((unsigned)oy << lg) + (unsigned)oz;
+        return (int)(vprefix[m] + __popc(code[m] & ((1u << a) - 1u)));
+    };
+    for (unsigned i = 0; i < nt; ++i) {
+        if ((int)(t0 + i) >= max_t) break;
+        const signed char* tr = c_tri + (cfg * MAX_TRI + i) * 3;
+        int* o = tris + 3 * (size_t)(t0 + i);
+        o[0] = vid(tr[0]); o[1] = vid(tr[1]); o[2] = vid(tr[2]);
+    }
+}
+// Eq.6 (M5), owner computes: node n gathers from its 3 owned edges (weight 1 - t) and the 3 edges that end in it (t)
+__global__ void k_mc_eq6(int N, int lg, const unsigned char* __restrict__ code, const unsigned* __restrict__ vprefix,
+                         const float* __restrict__ vt, const float* __restrict__ gv, const float* __restrict__ nrm,
+                         float* __restrict__ G, int max_v) {
+    const unsigned n = blockIdx.x * MC_BLOCK + threadIdx.x;
+    const Node j = node_xyz(n, N, lg);
+    const int jj[3] = {j.x, j.y, j.z};
+    const unsigned stride[3] = {1u << (2 * lg), 1u << lg, 1u};
+    float acc = 0.f;
+    auto contrib = [&](unsigned m, int a, bool head) {
+        const unsigned cm = code[m];
+        if (!(cm & (1u << a))) return;
+        const unsigned v = vprefix[m] + __popc(cm & ((1u << a) - 1u));
+        if ((int)v >= max_v) return;
+        const float g = -(gv[3 * (size_t)v] * nrm[3 * (size_t)v] + gv[3 * (size_t)v + 1] * nrm[3 * (size_t)v + 1] + gv[3 * (size_t)v + 2] * nrm[3 * (size_t)v + 2]);
+        const float t = vt[v];
+        acc += (head ? 1.f - t : t) * g;
+    };
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        contrib(n, a, true);
+        if (jj[a] >= 1) contrib(n - stride[a], a, false);
+    }
+    G[n] = acc;
+}
+
+// ---- Chamfer kernels -------------------------------------------------------------------------------------------------
+__device__ __forceinline__ int count_of(int n, const int* n_dev) { return n_dev ? min(*n_dev, n) : n; }
+__device__ __forceinline__ int cell_coord(float c, int Gc) { return min(max((int)floorf(c * (float)Gc), 0), Gc - 1); }
+__global__ void k_cell_count(const float* __restrict__ pts, int n, const int* n_dev, int Gc, int* __restrict__ cnt) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= count_of(n, n_dev)) return;
+    const int c = (cell_coord(pts[3 * i], Gc) * Gc + cell_coord(pts[3 * i + 1], Gc)) * Gc + cell_coord(pts[3 * i + 2], Gc);
+    atomicAdd(cnt + c, 1);
+}
+// one block: start = exclusive scan of cnt over ncell entries (+ total at [ncell]); cursor = start
+__global__ void k_cell_scan(const int* __restrict__ cnt, int ncell, int* __restrict__ start, int* __restrict__ cursor) {
+    __shared__ int part[1024];
+    const int tid = threadIdx.x, per = (ncell + 1023) / 1024;
+    const int lo = tid * per, hi = min(lo + per, ncell);
+    int s = 0;
+    for (int i = lo; i < hi; ++i) s += cnt[i];
+    part[tid] = s;
+    __syncthreads();
+    for (int d = 1; d < 1024; d <<= 1) {
+        const int v = (tid >= d) ? part[tid - d] : 0;
+        __syncthreads();
+        part[tid] += v;
+        __syncthreads();
+    }
+    int run = part[tid] - s;
+    for (int i = lo; i < hi; ++i) {
+        start[i] = run;
+        cursor[i] = run;
+        run += cnt[i];
+    }
+    if (tid == 1023) start[ncell] = part[1023];
+}
+__global__ void k_cell_scatter(const float* __restrict__ pts, int n, const int* n_dev, int Gc, int* __restrict__ cursor,
+                               float4* __restrict__ sorted) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= count_of(n, n_dev)) return;
+    const float x = pts[3 * i], y = pts[3 * i + 1], z = pts[3 * i + 2];
+    const int c = (cell_coord(x, Gc) * Gc + cell_coord(y, Gc)) * Gc + cell_coord(z, Gc);
+    sorted[atomicAdd(cursor + c, 1)] = make_float4(x, y, z, __int_as_float(i));
+}
+// exact nearest neighbour of every query in the binned set: rings of cells of growing Chebyshev radius r around the
+// query's cell; every point not yet visited after ring r is at least r / Gc away, so the search stops once best <= (r/Gc)^2
+__global__ void k_nn_query(const float* __restrict__ q, int nq, const int* nq_dev, int Gc, const int* __restrict__ start,
+                           const float4* __restrict__ sorted, int ntarget, const int* ntarget_dev, int* __restrict__ nn,
+                           float* __restrict__ d2out) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= count_of(nq, nq_dev)) return;
+    if (count_of(ntarget, ntarget_dev) <= 0) { nn[i] = -1; d2out[i] = 0.f; return; }
+    const float px = q[3 * i], py = q[3 * i + 1], pz = q[3 * i + 2];
+    const int cx = cell_coord(px, Gc), cy = cell_coord(py, Gc), cz = cell_coord(pz, Gc);
+    const float h = 1.f / (float)Gc;
+    float best = INFINITY;
+    int bi = 0x7fffffff;
+    for (int r = 0; r < Gc; ++r) {
+        const int x0 = max(cx - r, 0), x1 = min(cx + r, Gc - 1), y0 = max(cy - r, 0), y1 = min(cy + r, Gc - 1);
+        const int z0 = max(cz - r, 0), z1 = min(cz + r, Gc - 1);
+        for (int x = x0; x <= x1; ++x)
+            for (int y = y0; y <= y1; ++y) {
+                const bool shell_xy = (abs(x - cx) == r) || (abs(y - cy) == r);
+                for (int z = z0; z <= z1; z += (shell_xy || r == 0) ? 1 : max(z1 - z0, 1)) {
+                    if (!shell_xy && abs(z - cz) != r) continue;   // interior of the cube of radius r: visited by earlier rings
+                    const int c = (x * Gc + y) * Gc + z;
+                    for (int k = start[c]; k < start[c + 1]; ++k) {
+                        const float4 t = sorted[k];
+                        const float dx = px - t.x, dy = py - t.y, dz = pz - t.z;
+                        const float d = dx * dx + dy * dy + dz * dz;
+                        const int ti = __float_as_int(t.w);
+                        if (d < best || (d == best && ti < bi)) { best = d; bi = ti; }
+                    }
+                }
+            }
+        const float reach = (float)r * h;
+        if (best <= reach * reach) break;
+    }
+    nn[i] = bi;
+    d2out[i] = best;
+}
+__device__ __forceinline__ float block_sum_f(float x, float* sh) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = x;
+    __syncthreads();
+    float r = 0.f;
+    if (threadIdx.x < 32) {
+        r = (threadIdx.x < (blockDim.x >> 5)) ? sh[threadIdx.x] : 0.f;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) r += __shfl_xor_sync(0xffffffffu, r, o);
+    }
+    return r;
+}
+// a side: loss += d2 / na, grad_a[i] = (2 / na) (a_i - b_nn(i))
+__global__ void k_chamfer_a(const float* __restrict__ a, int na, const int* na_dev, const float* __restrict__ b, const int* __restrict__ nn_a,
+                            const float* __restrict__ d2, float* __restrict__ grad_a, double* __restrict__ lacc) {
+    __shared__ float sh[32];
+    const int n = count_of(na, na_dev), i = blockIdx.x * blockDim.x + threadIdx.x;
+    float l = 0.f;
+    if (i < n) {
+        const int k = nn_a[i];
+        l = d2[i] / (float)n;
+        if (grad_a) {
+            const float s = 2.f / (float)n;
+#pragma unroll
+            for (int d = 0; d < 3; ++d) grad_a[3 * i + d] = (k >= 0) ? s * (a[3 * i + d] - b[3 * k + d]) : 0.f;
+        }
+    }
+    const float t = block_sum_f(l, sh);
+    if (threadIdx.x == 0 && t != 0.f) atomicAdd(lacc, (double)t);
+}
+// b side: loss += d2 / nb, grad_a[nn_b(k)] += (2 / nb) (a_nn - b_k)
+__global__ void k_chamfer_b(const float* __restrict__ a, int na, const int* na_dev, const float* __restrict__ b, int nb,
+                            const int* __restrict__ nn_b, const float* __restrict__ d2, float* __restrict__ grad_a, double* __restrict__ lacc) {
+    __shared__ float sh[32];
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    float l = 0.f;
+    if (k < nb && count_of(na, na_dev) > 0) {
+        const int i = nn_b[k];
+        l = d2[k] / (float)nb;
+        if (grad_a && i >= 0) {
+            const float s = 2.f / (float)nb;
+#pragma unroll
+            for (int d = 0; d < 3; ++d) atomicAdd(grad_a + 3 * i + d, s * (a[3 * i + d] - b[3 * k + d]));
+        }
+    }
+    const float t = block_sum_f(l, sh);
+    if (threadIdx.x == 0 && t != 0.f) atomicAdd(lacc, (double)t);
+}
+__global__ void k_loss_store(double* __restrict__ lacc, float* __restrict__ loss) {
+    *loss = (float)*lacc;
+    *lacc = 0.0;
+}
+
+}  // namespace sapm
+
+// ================================================================================================
+struct sap_mesh {
+    int N = 0, lg = 0, max_v = 0, max_t = 0, max_p = 0, device = 0, Gc = 0, launches = 0;
+    unsigned char* code = nullptr;       // [N^3]
+    unsigned char* cfg = nullptr;        // [N^3]
+    unsigned long long* blocksum = nullptr;  // [N^3 / MC_BLOCK]
+    unsigned* vprefix = nullptr;         // [N^3]
+    unsigned* tprefix = nullptr;         // [N^3]
+    float* vt = nullptr;                 // [max_v]
+    int* counts_dev = nullptr;           // [2] of the last extract (device copy kept for the backward)
+    // Chamfer
+    int* cell_cnt = nullptr;             // [Gc^3]
+    int* cell_start = nullptr;           // [Gc^3 + 1]
+    int* cell_cursor = nullptr;          // [Gc^3]
+    float4* sorted = nullptr;            // [max_p]
+    int* nn_tmp_a = nullptr;             // [max_p]
+    int* nn_tmp_b = nullptr;             // [max_p]
+    float* d2_a = nullptr;               // [max_p]
+    float* d2_b = nullptr;               // [max_p]
+    double* lacc = nullptr;              // [1]
+    bool extracted = false;
+    size_t ws_bytes = 0;
+    std::string err;
+};
+
+namespace sapm {
+static thread_local std::string g_err;
+static bool ok(sap_mesh* h, cudaError_t e, const char* what) {
+    if (e == cudaSuccess) return true;
+    char buf[384];
+    snprintf(buf, sizeof buf, "%s: %s", what, cudaGetErrorString(e));
+    if (h) h->err = buf; else g_err = buf;
+    return false;
+}
+template <class T> static cudaError_t alloc(sap_mesh* h, T** p, size_t n) {
+    const cudaError_t e = cudaMalloc((void**)p, n * sizeof(T));
+    if (e == cudaSuccess) h->ws_bytes += n * sizeof(T);
+    return e;
+}
+static void free_all(sap_mesh* h) {
+    cudaFree(h->code); cudaFree(h->cfg); cudaFree(h->blocksum); cudaFree(h->vprefix); cudaFree(h->tprefix); cudaFree(h->vt);
+    cudaFree(h->counts_dev); cudaFree(h->cell_cnt); cudaFree(h->cell_start); cudaFree(h->cell_cursor); cudaFree(h->sorted);
+    cudaFree(h->nn_tmp_a); cudaFree(h->nn_tmp_b); cudaFree(h->d2_a); cudaFree(h->d2_b); cudaFree(h->lacc);
+}
+static sap_status_t check(sap_mesh* h) {
+    if (!h) return SAP_ERR_INVALID_ARG;
+    h->err.clear();
+    h->launches = 0;
+    int dev = -1;
+    if (!ok(h, cudaGetDevice(&dev), "cudaGetDevice")) return SAP_ERR_CUDA;
+    if (dev != h->device) { h->err = "current CUDA device is not the one the handle was created on"; return SAP_ERR_INVALID_ARG; }
+    return SAP_OK;
+}
+#define MESH_LAUNCH_CHECK(h, name)                                   \
+    do {                                                             \
+        ++(h)->launches;                                             \
+        if (!ok((h), cudaGetLastError(), name)) return SAP_ERR_CUDA; \
+    } while (0)
+}  // namespace sapm
+using namespace sapm;
+
+extern "C" int sap_mc_table(int* ntri, int* tris) {
+    const CubeTables& T = cube_tables();
+    for (int c = 0; c < 256; ++c) {
+        if (ntri) ntri[c] = T.ntri[c];
+        if (tris) for (int i = 0; i < MAX_TRI * 3; ++i) tris[c * MAX_TRI * 3 + i] = T.tri[c][i];
+    }
+    return T.max_tri;
+}
+
+extern "C" sap_status_t sap_mesh_create(int N, int max_vertices, int max_triangles, int max_points, sap_mesh_t** out) {
+    g_err.clear();
+    if (!out) { g_err = "out is NULL"; return SAP_ERR_INVALID_ARG; }
+    if (N <= 0 || max_vertices <= 0 || max_triangles <= 0 || max_points <= 0) { g_err = "sizes must be positive"; return SAP_ERR_INVALID_ARG; }
+    int lg = 0;
+    while ((1 << lg) < N) ++lg;
+    if ((1 << lg) != N || N < 8 || N > 512) { g_err = "N must be a power of two in [8, 512]"; return SAP_ERR_UNSUPPORTED; }
+    int dev = 0;
+    if (!ok(nullptr, cudaGetDevice(&dev), "cudaGetDevice")) return SAP_ERR_CUDA;
+    cudaDeviceProp prop;
+    if (!ok(nullptr, cudaGetDeviceProperties(&prop, dev), "cudaGetDeviceProperties")) return SAP_ERR_CUDA;
+    if (prop.major != 10) { g_err = "device is not sm_100 (Blackwell B200); this library has no other code path"; return SAP_ERR_UNSUPPORTED; }
+    sap_mesh* h = new (std::nothrow) sap_mesh;
+    if (!h) { g_err = "host allocation failed"; return SAP_ERR_OOM; }
+    h->N = N; h->lg = lg; h->max_v = max_vertices; h->max_t = max_triangles; h->max_p = max_points; h->device = dev;
+    int gc = (int)lround(cbrt((double)max_points / 2.0));
+    h->Gc = gc < 4 ? 4 : gc > 128 ? 128 : gc;
+    const size_t V = (size_t)N * N * N, C = (size_t)h->Gc * h->Gc * h->Gc;
+    cudaError_t e = cudaSuccess;
+    auto upd = [&](cudaError_t x) { if (e == cudaSuccess) e = x; };
+    upd(alloc(h, &h->code, V)); upd(alloc(h, &h->cfg, V)); upd(alloc(h, &h->blocksum, V / MC_BLOCK));
+    upd(alloc(h, &h->vprefix, V)); upd(alloc(h, &h->tprefix, V)); upd(alloc(h, &h->vt, (size_t)max_vertices));
+    upd(alloc(h, &h->counts_dev, (size_t)2));
+    upd(alloc(h, &h->cell_cnt, C)); upd(alloc(h, &h->cell_start, C + 1)); upd(alloc(h, &h->cell_cursor, C));
+    upd(alloc(h, &h->sorted, (size_t)max_points));
+    upd(alloc(h, &h->nn_tmp_a, (size_t)max_points)); upd(alloc(h, &h->nn_tmp_b, (size_t)max_points));
+    upd(alloc(h, &h->d2_a, (size_t)max_points)); upd(alloc(h, &h->d2_b, (size_t)max_points));
+    upd(alloc(h, &h->lacc, (size_t)1));
+    if (e == cudaSuccess) upd(cudaMemset(h->lacc, 0, sizeof(double)));
+    if (e == cudaSuccess) upd(cudaMemset(h->counts_dev, 0, 2 * sizeof(int)));
+    if (e == cudaSuccess) {
+        const CubeTables& T = cube_tables();
+        upd(cudaMemcpyToSymbol(c_ntri, T.ntri, sizeof(T.ntri)));
+        upd(cudaMemcpyToSymbol(c_tri, T.tri, sizeof(T.tri)));
+    }
+    if (e != cudaSuccess) {
+        ok(nullptr, e, "sap_mesh_create");
+        const bool oom = e == cudaErrorMemoryAllocation;
+        free_all(h); delete h; cudaGetLastError();
+        return oom ? SAP_ERR_OOM : SAP_ERR_CUDA;
+    }
+    *out = h;
+    return SAP_OK;
+}
+
+extern "C" sap_status_t sap_mc_extract(sap_mesh_t* h, const float* chi, float* verts, float* normals, int* tris, int* counts,
+                                       void* stream) {
+    sap_status_t st = check(h);
+    if (st != SAP_OK) return st;
+    if (!chi || !verts || !normals || !tris || !counts) { h->err = "null pointer argument"; return SAP_ERR_INVALID_ARG; }
+    cudaStream_t s = (cudaStream_t)stream;
+    const int N = h->N, nb = (int)(((size_t)N * N * N) / MC_BLOCK);
+    k_mc_classify<<<nb, MC_BLOCK, 0, s>>>(chi, N, h->lg, h->code, h->cfg, h->blocksum);
+    MESH_LAUNCH_CHECK(h, "k_mc_classify");
+    k_mc_scan_blocks<<<1, 1024, 0, s>>>(h->blocksum, nb, h->counts_dev);
+    MESH_LAUNCH_CHECK(h, "k_mc_scan_blocks");
+    k_mc_emit_verts<<<nb, MC_BLOCK, 0, s>>>(chi, N, h->lg, h->code, h->blocksum, h->vprefix, h->tprefix, verts, normals, h->vt, h->max_v);
+    MESH_LAUNCH_CHECK(h, "k_mc_emit_verts");
+    k_mc_emit_tris<<<nb, MC_BLOCK, 0, s>>>(N, h->lg, h->code, h->cfg, h->vprefix, h->tprefix, tris, h->max_t);
+    MESH_LAUNCH_CHECK(h, "k_mc_emit_tris");
+    if (!ok(h, cudaMemcpyAsync(counts, h->counts_dev, 2 * sizeof(int), cudaMemcpyDeviceToDevice, s), "copy counts")) return SAP_ERR_CUDA;
+    h->extracted = true;
+    return SAP_OK;
+}
+
+extern "C" sap_status_t sap_mc_backward(sap_mesh_t* h, const float* grad_verts, const float* normals, float* grad_chi, void* stream) {
+    sap_status_t st = check(h);
+    if (st != SAP_OK) return st;
+    if (!grad_verts || !normals || !grad_chi) { h->err = "null pointer argument"; return SAP_ERR_INVALID_ARG; }
+    if (!h->extracted) { h->err = "sap_mc_backward must follow sap_mc_extract on this handle"; return SAP_ERR_INVALID_ARG; }
+    const int N = h->N, nb = (int)(((size_t)N * N * N) / MC_BLOCK);
+    k_mc_eq6<<<nb, MC_BLOCK, 0, (cudaStream_t)stream>>>(N, h->lg, h->code, h->vprefix, h->vt, grad_verts, normals, grad_chi, h->max_v);
+    MESH_LAUNCH_CHECK(h, "k_mc_eq6");
+    return SAP_OK;
+}
+
+extern "C" sap_status_t sap_chamfer(sap_mesh_t* h, const float* a, int na, const int* na_dev, const float* b, int nb, float* loss,
+                                    float* grad_a, int* nn_a, int* nn_b, void* stream) {
+    sap_status_t st = check(h);
+    if (st != SAP_OK) return st;
+    if (!a || !b || !loss) { h->err = "null pointer argument"; return SAP_ERR_INVALID_ARG; }
+    if (na < 0 || nb < 1 || na > h->max_p || nb > h->max_p) { h->err = "point counts out of range (0 <= na <= max_points, 1 <= nb <= max_points)"; return SAP_ERR_INVALID_ARG; }
+    cudaStream_t s = (cudaStream_t)stream;
+    const int Gc = h->Gc, ncell = Gc * Gc * Gc;
+    int* nna = nn_a ? nn_a : h->nn_tmp_a;
+    int* nnb = nn_b ? nn_b : h->nn_tmp_b;
+    if (na == 0) {
+        if (!ok(h, cudaMemsetAsync(loss, 0, sizeof(float), s), "memset loss")) return SAP_ERR_CUDA;
+        return SAP_OK;
+    }
+    const int ga = (na + 255) / 256, gb = (nb + 255) / 256;
+    // grid over b, queries a
+    if (!ok(h, cudaMemsetAsync(h->cell_cnt, 0, sizeof(int) * ncell, s), "memset cells")) return SAP_ERR_CUDA;
+    k_cell_count<<<gb, 256, 0, s>>>(b, nb, nullptr, Gc, h->cell_cnt);
+    MESH_LAUNCH_CHECK(h, "k_cell_count");
+    k_cell_scan<<<1, 1024, 0, s>>>(h->cell_cnt, ncell, h->cell_start, h->cell_cursor);
+    MESH_LAUNCH_CHECK(h, "k_cell_scan");
+    k_cell_scatter<<<gb, 256, 0, s>>>(b, nb, nullptr, Gc, h->cell_cursor, h->sorted);
+    MESH_LAUNCH_CHECK(h, "k_cell_scatter");
+    k_nn_query<<<ga, 256, 0, s>>>(a, na, na_dev, Gc, h->cell_start, h->sorted, nb, nullptr, nna, h->d2_a);
+    MESH_LAUNCH_CHECK(h, "k_nn_query");
+    k_chamfer_a<<<ga, 256, 0, s>>>(a, na, na_dev, b, nna, h->d2_a, grad_a, h->lacc);
+    MESH_LAUNCH_CHECK(h, "k_chamfer_a");
+    // grid over a, queries b
+    if (!ok(h, cudaMemsetAsync(h->cell_cnt, 0, sizeof(int) * ncell, s), "memset cells")) return SAP_ERR_CUDA;
+    k_cell_count<<<ga, 256, 0, s>>>(a, na, na_dev, Gc, h->cell_cnt);
+    MESH_LAUNCH_CHECK(h, "k_cell_count");
+    k_cell_scan<<<1, 1024, 0, s>>>(h->cell_cnt, ncell, h->cell_start, h->cell_cursor);
+    MESH_LAUNCH_CHECK(h, "k_cell_scan");
+    k_cell_scatter<<<ga, 256, 0, s>>>(a, na, na_dev, Gc, h->cell_cursor, h->sorted);
+    MESH_LAUNCH_CHECK(h, "k_cell_scatter");
+    k_nn_query<<<gb, 256, 0, s>>>(b, nb, nullptr, Gc, h->cell_start, h->sorted, na, na_dev, nnb, h->d2_b);
+    MESH_LAUNCH_CHECK(h, "k_nn_query");
+    k_chamfer_b<<<gb, 256, 0, s>>>(a, na, na_dev, b, nb, nnb, h->d2_b, grad_a, h->lacc);
+    MESH_LAUNCH_CHECK(h, "k_chamfer_b");
+    k_loss_store<<<1, 1, 0, s>>>(h->lacc, loss);
+    MESH_LAUNCH_CHECK(h, "k_loss_store");
+    return SAP_OK;
+}
+
+extern "C" void sap_mesh_destroy(sap_mesh_t* h) {
+    if (!h) return;
+    free_all(h);
+    delete h;
+}
+extern "C" const char* sap_mesh_last_error(const sap_mesh_t* h) { return h ? h->err.c_str() : g_err.c_str(); }
+extern "C" size_t sap_mesh_workspace_bytes(const sap_mesh_t* h) { return h ? h->ws_bytes : 0; }
+extern "C" int sap_mesh_last_launch_count(const sap_mesh_t* h) { return h ? h->launches : 0; }

@@ -1,0 +1,159 @@
+"""GPU parity of the mesh entry points (include/sap_mesh.h) against the float64 mesh oracle: Marching Cubes
+(PAPER.md:L100), Eq.6 (L113-L117), Chamfer (L102).  Integer topology is compared bit-exactly; positions, normals,
+gradients within float32 bounds.  The sign test chi < 0 is taken on the same float32 values by both sides."""
+import numpy as np
+import pytest
+
+from oracle import dpsr_oracle as orc
+from oracle import mesh_oracle as mo
+from paper_2106_03452_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+
+def _chi_from_cloud(N, shape, P, seed, sigma=2.0):
+    pts, nrm = inputs.make_cloud(shape, P, seed=seed)
+    return orc.forward(N, sigma, pts, nrm)["chi"].astype(np.float32), pts
+
+
+def _extract(N, chi32, cap_v=None, cap_t=None):
+    import torch
+    from paper_2106_03452_b200.mesh import Mesh
+    ref = mo.marching_cubes(chi32)
+    V, T = ref["verts"].shape[0], ref["tris"].shape[0]
+    h = Mesh(N, cap_v or V + 7, cap_t or T + 5, max(V + 7, 1000))
+    out = h.extract(torch.from_numpy(chi32).cuda())
+    torch.cuda.synchronize()
+    return h, ref, out
+
+
+@pytest.mark.parametrize("N,shape,P", [(32, "sphere", 3000), (64, "torus", 8000), (64, "ellipsoids3", 6000), (128, "bumpy", 20000)])
+def test_marching_cubes_matches_the_oracle(N, shape, P):
+    chi32, _ = _chi_from_cloud(N, shape, P, seed=1)
+    h, ref, (verts, normals, tris, counts) = _extract(N, chi32)
+    V, T = ref["verts"].shape[0], ref["tris"].shape[0]
+    assert counts.cpu().tolist() == [V, T] and V > 100
+    assert np.array_equal(tris[:T].cpu().numpy(), ref["tris"].astype(np.int32))          # topology: bit-exact, same order
+    assert np.abs(verts[:V].cpu().numpy() - ref["verts"]).max() <= 1e-6
+    # normals: float32 central differences of chi; compare where the gradient is not tiny
+    assert np.abs(normals[:V].cpu().numpy() - ref["normals"]).max() <= 2e-3
+    assert np.abs(np.linalg.norm(normals[:V].cpu().numpy(), axis=1) - 1).max() <= 1e-5
+    assert h.last_launch_count == 4
+    h.close()
+
+
+def test_marching_cubes_edge_cases():
+    import torch
+    from paper_2106_03452_b200.mesh import Mesh
+    N = 16
+    g = np.arange(N) / N
+    X, Y, Z = np.meshgrid(g, g, g, indexing="ij")
+    # empty mesh
+    h = Mesh(N, 100, 100, 1000)
+    v, n, t, c = h.extract(torch.ones((N, N, N), device="cuda"))
+    assert c.cpu().tolist() == [0, 0]
+    # surface through the grid boundary (open mesh) and exact zeros on nodes (chi == 0 counts as OUTSIDE)
+    chi = (X - 0.5).astype(np.float32)
+    ref = mo.marching_cubes(chi)
+    h2 = Mesh(N, ref["verts"].shape[0], ref["tris"].shape[0], 1000)
+    v, n, t, c = h2.extract(torch.from_numpy(chi).cuda())
+    assert c.cpu().tolist() == [ref["verts"].shape[0], ref["tris"].shape[0]]
+    assert np.array_equal(t.cpu().numpy(), ref["tris"].astype(np.int32))
+    assert np.abs(v.cpu().numpy() - ref["verts"]).max() <= 1e-7
+    # capacity overflow: arrays filled up to capacity, counts report the sizes needed
+    chi = (np.sqrt((X - 0.5) ** 2 + (Y - 0.5) ** 2 + (Z - 0.5) ** 2) - 0.3).astype(np.float32)
+    ref = mo.marching_cubes(chi)
+    V, T = ref["verts"].shape[0], ref["tris"].shape[0]
+    h3 = Mesh(N, V // 2, T // 3, 1000)
+    v, n, t, c = h3.extract(torch.from_numpy(chi).cuda())
+    assert c.cpu().tolist() == [V, T]
+    assert np.abs(v.cpu().numpy() - ref["verts"][:V // 2]).max() <= 1e-6
+    assert np.array_equal(t.cpu().numpy(), ref["tris"][:T // 3].astype(np.int32))
+    for x in (h, h2, h3):
+        x.close()
+
+
+def test_eq6_backward_matches_the_oracle():
+    import torch
+    N = 64
+    chi32, _ = _chi_from_cloud(N, "torus", 8000, seed=2)
+    h, ref, (verts, normals, tris, counts) = _extract(N, chi32)
+    V = ref["verts"].shape[0]
+    rng = np.random.default_rng(0)
+    d = rng.standard_normal((h.max_v, 3)).astype(np.float32)
+    G = h.backward(torch.from_numpy(d).cuda(), normals)
+    torch.cuda.synchronize()
+    want = mo.eq6_backward(N, ref, d[:V].astype(np.float64))
+    got = G.cpu().numpy()
+    assert np.linalg.norm(got - want) <= 2e-3 * np.linalg.norm(want)       # normals differ at the 1e-3 level (float32 gradients)
+    # with the oracle's normals handed in the kernel itself is exact to float32 rounding
+    nref = np.zeros((h.max_v, 3), np.float32)
+    nref[:V] = ref["normals"]
+    got2 = h.backward(torch.from_numpy(d).cuda(), torch.from_numpy(nref).cuda()).cpu().numpy()
+    assert np.linalg.norm(got2 - want) <= 1e-6 * np.linalg.norm(want)
+    assert (got2[want == 0] == 0).all()
+    h.close()
+
+
+@pytest.mark.parametrize("na,nb", [(5000, 3000), (1, 1), (37, 4000), (20000, 20000)])
+def test_chamfer_matches_brute_force(na, nb):
+    import torch
+    from paper_2106_03452_b200.mesh import Mesh
+    rng = np.random.default_rng(na + nb)
+    if na >= 1000:
+        a, _ = inputs.make_cloud("torus", na, seed=3)
+        b, _ = inputs.make_cloud("ellipsoids3", nb, seed=4)      # two different surfaces: neighbours several cells apart
+    else:
+        a = rng.uniform(0, 1, (na, 3)).astype(np.float32)
+        b = rng.uniform(0, 1, (nb, 3)).astype(np.float32)
+    ref = mo.chamfer(a, b)
+    h = Mesh(8, 8, 8, max(na, nb))
+    loss, ga, nn_a, nn_b = h.chamfer(torch.from_numpy(a).cuda(), torch.from_numpy(b).cuda(), want_nn=True)
+    torch.cuda.synchronize()
+    assert abs(loss.item() - ref["loss"]) <= 1e-5 * ref["loss"]
+    # indices: exact wherever the nearest neighbour is unique at float32 resolution
+    for got, want, q, t in ((nn_a.cpu().numpy(), ref["nn_a"], a, b), (nn_b.cpu().numpy(), ref["nn_b"], b, a)):
+        diff = got != want
+        if diff.any():
+            dg = ((q[diff].astype(np.float64) - t[got[diff]]) ** 2).sum(1)
+            dw = ((q[diff].astype(np.float64) - t[want[diff]]) ** 2).sum(1)
+            assert np.all(np.abs(dg - dw) <= 1e-6 * dw + 1e-12)      # only float32 near-ties may differ
+        assert diff.mean() <= 1e-3
+    assert np.linalg.norm(ga.cpu().numpy() - ref["grad_a"]) <= 1e-4 * np.linalg.norm(ref["grad_a"]) + 1e-12
+    h.close()
+
+
+def test_optimisation_step_on_the_device_without_host_round_trips():
+    # one iteration of the loop of Sec.3.2 enqueued back to back: DPSR forward -> MC -> Chamfer (device-side vertex count)
+    # -> Eq.6 -> DPSR backward; the oracle does the same in float64
+    import torch
+    from paper_2106_03452_b200.binding import Dpsr
+    from paper_2106_03452_b200.mesh import Mesh
+    N, P, sigma = 32, 3000, 2.0
+    src, nrm = inputs.make_cloud("sphere", P, seed=0)
+    target, _ = inputs.make_cloud("ellipsoids3", 4000, seed=5)
+    d = Dpsr(N, sigma, 1, P)
+    m = Mesh(N, 20000, 40000, 20000)
+    tp, tn = torch.from_numpy(src[None].copy()).cuda(), torch.from_numpy(nrm[None].copy()).cuda()
+    tb = torch.from_numpy(target).cuda()
+    chi = d.forward(tp, tn)
+    verts, normals, tris, counts = m.extract(chi[0])
+    loss, gv, _, _ = m.chamfer(verts, tb, na_dev=counts)
+    G = m.backward(gv, normals)
+    gp, gn = d.backward(tp, tn, chi, G[None])
+    torch.cuda.synchronize()
+    # oracle chain on the GPU's float32 chi for the mesh (sign decisions in the same precision), float64 elsewhere
+    f = orc.forward(N, sigma, src, nrm)
+    assert np.abs(chi.cpu().numpy()[0] - f["chi"]).max() <= 1e-4 * np.abs(f["chi"]).max()
+    ref = mo.marching_cubes(chi.cpu().numpy()[0])
+    V = ref["verts"].shape[0]
+    assert counts.cpu().tolist() == [V, ref["tris"].shape[0]]
+    c = mo.chamfer(ref["verts"], target)
+    assert abs(loss.item() - c["loss"]) <= 1e-4 * c["loss"]
+    Gref = mo.eq6_backward(N, ref, c["grad_a"])
+    assert np.linalg.norm(G.cpu().numpy() - Gref) <= 5e-3 * np.linalg.norm(Gref)
+    b = orc.backward(N, sigma, src, nrm, f, Gref)
+    assert np.linalg.norm(gp.cpu().numpy()[0] - b["grad_points"]) <= 1e-2 * np.linalg.norm(b["grad_points"])
+    assert np.linalg.norm(gn.cpu().numpy()[0] - b["grad_normals"]) <= 1e-2 * np.linalg.norm(b["grad_normals"])
+    d.close()
+    m.close()
