@@ -29,44 +29,48 @@ import numpy as np  # noqa: E402
 METRIC = "dpsr_fwd_bwd_ms_per_grid"
 UNIT = "ms/grid"
 
-# Algorithmic bytes per grid in units of V = 4 N^3 (SURVEY.md 8(d) per-axis-pass model): which table
-# rows each of our kernels covers, and the bytes that kernel must itself read once + write once.
-#   label: (yardstick V fused (N<=128), yardstick V unfused, compulsory V)   -- per channel-set launch
+# Bytes a kernel must itself read once + write once ("compulsory"), in units of V = 4 N^3 per batch item: what
+# roofline.achieved / roofline.frac are computed on (DESIGN.md 7 has the table).  The 52V per-axis-pass
+# model of SURVEY 8(d) is a DIFFERENT quantity -- bytes an unfused one-pass-per-axis design would move -- and is only
+# reported as `fusion_gain_vs_52V_model` (how many times fewer bytes than that model would need at the measured speed),
+# never as a fraction of HBM peak.
 YARD_FWD_BWD_V = 52.0
 KERNEL_BYTES_V = {
-    # label: (yardstick V fused (N<=128), yardstick V unfused (N>=256), compulsory V fused, compulsory V unfused)
-    # forward
-    "F:k_bin_count": (0.0, 0.0, 0.0, 0.0),               # counting sort of the points (bytes ~ 72 B/point, ignored)
-    "F:k_bin_scan": (0.0, 0.0, 0.0, 0.0),
-    "F:k_bin_scatter": (0.0, 0.0, 0.0, 0.0),
-    # splat fused in: rows "splat" (3V) + z r2c x3 (6V) [+ y x3 (6V) when fused]; it only WRITES 3V itself
-    "F:k_zy_fwd": (15.0, 9.0, 3.0, 3.0),
-    "F:k_ring<FWD,y>": (0.0, 6.0, 0.0, 5.0),             # row y sweep x3; writes 2 spectra (x, u = h_y y + h_z z)
-    "F:k_ring<SOLVE>": (4.0, 4.0, 4.0, 3.0),             # row x sweep + solve + x inverse (3V or 2V in, 1V out)
-    "F:k_ring<INV,y>": (0.0, 2.0, 0.0, 2.0),             # row inverse y
-    "F:k_zl_inv": (4.0, 2.0, 2.0, 2.0),                  # rows [inverse y (2V) +] inverse z c2r (2V)
-    "F:k_sample_mean": (0.0, 0.0, 0.0, 0.0),
-    "F:k_scale_shift": (2.0, 2.0, 2.0, 2.0),             # row normalise
-    # backward
-    "B:k_reduce_g": (2.0, 2.0, 2.0, 2.0),                # row reductions
-    "B:k_zl_gbar": (5.0, 3.0, 2.0, 2.0),                 # rows z r2c (G+W in, 1 out = 3V) + y (2V); W is re-rasterised, not read
-    "B:k_zy_fwd<GBAR>": (5.0, 3.0, 2.0, 2.0),            # the same pass, one tile per CTA (N >= 256)
-    "B:k_ring<FWD,y>": (0.0, 2.0, 0.0, 2.0),
-    "B:k_ring<ADJ>": (4.0, 4.0, 4.0, 3.0),               # row x sweep + conj(M) fan-out + x inverses (1V in, 3V or 2V out)
-    "B:k_ring<INV,y>": (0.0, 6.0, 0.0, 5.0),             # reads 2 spectra (x, B), writes 3
-    "B:k_zl_inv": (12.0, 6.0, 6.0, 6.0),                 # rows inverse y x3 + inverse z x3
-    "B:k_gather_grads": (4.0, 4.0, 0.0, 0.0),            # row gather (<= 4V, sparse)
+    # label: (compulsory V for N <= 128 (y fused with z), compulsory V for N >= 256)
+    "F:k_bin_count": (0.0, 0.0), "F:k_bin_scan": (0.0, 0.0), "F:k_bin_scatter": (0.0, 0.0),   # 72 B/point, no grid traffic
+    "F:k_zy_fwd": (3.0, 3.0),            # writes 3 spectra; the splatted field never exists in HBM
+    "F:k_ring<FWD,y>": (0.0, 5.0),       # N >= 256 only: reads 3 spectra, writes 2 (x, u = h_y y + h_z z)
+    "F:k_ring<SOLVE>": (4.0, 3.0),       # reads 3 (2) spectra, writes 1
+    "F:k_ring<INV,y>": (0.0, 2.0),
+    "F:k_zl_inv": (2.0, 2.0),            # reads 1 spectrum, writes chi'
+    "F:k_sample_mean": (0.0, 0.0),       # gathers 8 values per point
+    "F:k_scale_shift": (2.0, 2.0),
+    "F:k_scale_shift_mse": (4.0, 4.0),
+    "B:k_reduce_g": (2.0, 2.0),          # reads G and chi
+    "B:k_zl_gbar": (2.0, 2.0),           # reads G, writes 1 spectrum (W is re-rasterised, not read)
+    "B:k_zy_fwd<GBAR>": (2.0, 2.0),
+    "B:k_ring<FWD,y>": (0.0, 2.0),
+    "B:k_ring<ADJ>": (3.0, 3.0),         # reads 1 spectrum, writes 2 (x, B)
+    "B:k_ring<INV,y>": (0.0, 5.0),       # reads 2 spectra, writes 3
+    "B:k_zl_inv": (5.0, 6.0),            # N <= 128: reads 2 spectra (B twice, the second time from L2), writes 3 grids
+    "B:k_gather_grads": (0.0, 0.0),      # gathers 32 values per point
+    # latency path: only chi (forward) / G and chi (backward) must cross HBM; the spectra live in L2 between the phases
+    "F:k_fused_fwd": (1.0, 1.0), "B:k_fused_bwd": (2.0, 2.0),
 }
+TRAFFIC_JSON = os.path.join(ROOT, "profiles", "r02_traffic.json")
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the `ncu --set full` captures summarised under
-# profiles/r01_full_cfg{2,3,4}.md (one forward+backward each, kernels in launch order).  At 128^3 batch 1 the working
-# set (~50 MB) lives in the 126 MB L2, so DRAM traffic is far BELOW the algorithmic bytes there.
-NCU_TRAFFIC = {
-    "cfg2_torus_128": {"F:k_bin_count": 244480, "F:k_bin_scan": 8704, "F:k_bin_scatter": 484864, "F:k_zy_fwd": 667648, "F:k_ring<SOLVE>": 25604096, "F:k_zl_inv": 8542976, "F:k_sample_mean": 2118400, "F:k_scale_shift": 8392192, "B:k_reduce_g": 16787968, "B:k_zl_gbar": 8739328, "B:k_ring<ADJ>": 8562944, "B:k_zl_inv": 25624832, "B:k_gather_grads": 7804160},
-    "cfg3_ellipsoids_128_b32": {"F:k_zy_fwd": 773939712, "F:k_ring<SOLVE>": 1066452480, "F:k_zl_inv": 491010304, "F:k_scale_shift": 479487232, "B:k_reduce_g": 540808448, "B:k_zl_gbar": 495542528, "B:k_ring<ADJ>": 1032498688, "B:k_zl_inv": 1574035200},
-    "cfg4_ellipsoids_256": {"F:k_zy_fwd": 147610880, "F:k_ring<FWD,y>": 284943616, "F:k_ring<SOLVE>": 166544896, "F:k_ring<INV,y>": 78128896, "F:k_zl_inv": 82979328, "F:k_scale_shift": 78618880, "B:k_reduce_g": 137347328, "B:k_zy_fwd<GBAR>": 92718336, "B:k_ring<FWD,y>": 78034432, "B:k_ring<ADJ>": 144984832, "B:k_ring<INV,y>": 280314112, "B:k_zl_inv": 350683648},
-}
+def load_traffic():
+    """profiles/r02_traffic.json (written by paper_2106_03452_b200.profiling from an `ncu --set full` capture): per-launch
+    dram bytes, valid only for the kernel sources it was captured at."""
+    try:
+        from paper_2106_03452_b200.profiling import kernel_tree_hash
+        doc = json.load(open(TRAFFIC_JSON))
+        if doc.get("kernel_sources") != kernel_tree_hash():
+            return {}, f"stale (captured at kernel sources {doc.get('kernel_sources')}, running {kernel_tree_hash()})"
+        return {k: v["bytes"] for k, v in doc["workloads"].items()}, f"profiles/r02_traffic.json @ {doc['kernel_sources']}"
+    except Exception as e:   # no capture committed yet
+        return {}, f"unavailable ({type(e).__name__})"
 
 
 def read_peaks():
@@ -183,27 +187,24 @@ def make_device_inputs(cfg_id, rank, torch):
     return cfg, pts, nrm, G
 
 
-def time_config(cfg_id, steps, warmup, rank, torch, flush, with_e2e=True, with_profile=True):
-    """Times `steps` forward+backward passes of BASELINE.json config cfg_id on the current device."""
+def time_config(cfg_id, steps, warmup, rank, torch, flush, with_e2e=True, with_profile=True, path="auto", custom=None):
+    """Times `steps` forward+backward passes of BASELINE.json config cfg_id (or custom = (Config, pts, nrm, G)) on the
+    current device: CUDA events on the launching stream, L2 flushed (256 MB write) before every step, outside the interval."""
     from paper_2106_03452_b200.binding import Dpsr
-    cfg, pts, nrm, G = make_device_inputs(cfg_id, rank, torch)
+    cfg, pts, nrm, G = make_device_inputs(cfg_id, rank, torch) if custom is None else custom
     B, N, P = cfg.batch, cfg.N, cfg.P
     h = Dpsr(N, cfg.sigma, B, P)
+    h.set_path(path)
     d_pts, d_nrm, d_G = torch.from_numpy(pts).cuda(), torch.from_numpy(nrm).cuda(), torch.from_numpy(G).cuda()
     chi = torch.empty((B, N, N, N), dtype=torch.float32, device="cuda")
     gp, gn = torch.empty_like(d_pts), torch.empty_like(d_nrm)
     stream = torch.cuda.current_stream()
 
-    def step():
-        h.forward(d_pts, d_nrm, chi, stream)
-        nf = h.last_launch_count
-        h.backward(d_pts, d_nrm, chi, d_G, gp, gn, stream)
-        return nf + h.last_launch_count
-
     launches = 0
     for _ in range(warmup):
         flush.zero_()
-        step()
+        h.forward(d_pts, d_nrm, chi, stream)
+        h.backward(d_pts, d_nrm, chi, d_G, gp, gn, stream)
     torch.cuda.synchronize()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
           for _ in range(steps)]
@@ -220,7 +221,7 @@ def time_config(cfg_id, steps, warmup, rank, torch, flush, with_e2e=True, with_p
     t_fwd = sum(a.elapsed_time(m) for a, m, b in ev)
     t_all = sum(a.elapsed_time(b) for a, m, b in ev)
     res = {"cfg": cfg, "ms_total": t_all, "ms_fwd": t_fwd / steps, "ms_bwd": (t_all - t_fwd) / steps,
-           "ms_step": t_all / steps, "launches": launches, "workspace_bytes": h.workspace_bytes}
+           "ms_step": t_all / steps, "launches": launches, "workspace_bytes": h.workspace_bytes, "path": h.path}
 
     if with_profile:   # second pass with per-kernel events (their gaps would perturb the headline timing)
         h.set_profiling(True)
@@ -235,8 +236,11 @@ def time_config(cfg_id, steps, warmup, rank, torch, flush, with_e2e=True, with_p
                 acc.setdefault(name, []).append(ms)
         h.set_profiling(False)
         res["kernels_ms"] = {k: float(np.mean(v)) for k, v in acc.items()}
+        if h.path == "latency":
+            res["fused_phases_us"] = dict(h.fused_phases())
 
     if with_e2e:       # host buffers through the C ABI: H2D points, normals, dL/dchi; D2H chi, gradients
+        h.reserve(host=True)
         hp, hn, hG = (torch.from_numpy(x).pin_memory() for x in (pts, nrm, G))
         hchi = torch.empty((B, N, N, N), dtype=torch.float32).pin_memory()
         hgp, hgn = torch.empty((B, P, 3)).pin_memory(), torch.empty((B, P, 3)).pin_memory()
@@ -265,6 +269,7 @@ def time_fused_mse(cfg_id, steps, warmup, torch, flush):
     cfg, pts, nrm, G = make_device_inputs(cfg_id, 0, torch)
     B, N, P = cfg.batch, cfg.N, cfg.P
     h = Dpsr(N, cfg.sigma, B, P)
+    h.reserve(mse=True)
     d_pts, d_nrm = torch.from_numpy(pts).cuda(), torch.from_numpy(nrm).cuda()
     d_gt = torch.from_numpy(np.tanh(G).astype(np.float32) * 0.5).cuda()
     chi = torch.empty((B, N, N, N), dtype=torch.float32, device="cuda")
@@ -286,86 +291,224 @@ def time_fused_mse(cfg_id, steps, warmup, torch, flush):
     return {"ms_per_grid": tot / steps / B, "steps": steps, "what": "forward_mse + backward_mse (loss and dL/dchi never leave the handle)"}
 
 
-def time_coarse_to_fine(iters, torch, flush):
-    """The optimisation-based schedule of the paper (L121, L396): 32^3 -> 64^3 -> 128^3 (1000 iterations each, sigma
-    2, 2, 3) -> 256^3 (200 iterations, sigma 3) on 20,000 points, one handle per level.  An iteration here = DPSR
-    forward + backward + a gradient step on the points and normals (torch, on the device); Marching Cubes and the
-    Chamfer loss of the paper's loop are out of scope, the upstream gradient is a fixed seeded grid.  `iters`
-    iterations per level are timed and scaled to the paper's counts."""
-    from paper_2106_03452_b200 import inputs
-    from paper_2106_03452_b200.binding import Dpsr
-    P = 20000
-    pts, nrm = inputs.make_cloud("torus", P, seed=0)
-    d_pts, d_nrm = torch.from_numpy(pts[None].copy()).cuda(), torch.from_numpy(nrm[None].copy()).cuda()
+def _timed_loop(torch, fn, iters, warm=3):
     stream = torch.cuda.current_stream()
-    out, total = {}, 0.0
-    for N, sigma, n_it in ((32, 2.0, 1000), (64, 2.0, 1000), (128, 3.0, 1000), (256, 3.0, 200)):
-        h = Dpsr(N, sigma, 1, P)
-        G = torch.from_numpy(inputs.upstream_grad(N, 1, seed=N)).cuda()
-        chi = torch.empty((1, N, N, N), dtype=torch.float32, device="cuda")
-        gp, gn = torch.empty_like(d_pts), torch.empty_like(d_nrm)
-        c, n = d_pts.clone(), d_nrm.clone()
+    for _ in range(warm):
+        fn()
+    torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(stream)
+    for _ in range(iters):
+        fn()
+    b.record(stream)
+    torch.cuda.synchronize()
+    return a.elapsed_time(b) / iters
 
-        def it():
-            h.forward(c, n, chi)
-            h.backward(c, n, chi, G, gp, gn)
-            step = 0.25 / N / gp.abs().max().clamp_min(1e-20)   # largest move: a quarter of a cell
-            c.sub_(step * gp).clamp_(0.0, 1.0 - 1e-6)
-            n.sub_(step * gn)
 
-        def timed(fn):
-            for _ in range(3):
-                fn()
-            torch.cuda.synchronize()
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record(stream)
-            for _ in range(iters):
-                fn()
-            b.record(stream)
-            torch.cuda.synchronize()
-            return a.elapsed_time(b) / iters
-
-        ms = timed(it)
-        entry = {"ms_per_iteration": ms, "paper_iterations": n_it}
-        try:   # the same iteration replayed as a CUDA graph: the library allocates nothing and never synchronises
-            side = torch.cuda.Stream()
-            side.wait_stream(stream)
-            with torch.cuda.stream(side):
-                it()
-            stream.wait_stream(side)
-            graph = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(graph):
-                it()
-            entry["ms_per_iteration_cuda_graph"] = timed(graph.replay)
-            ms = min(ms, entry["ms_per_iteration_cuda_graph"])
-            del graph
-        except Exception as e:   # capture not supported in this environment: keep the eager number
-            entry["cuda_graph_error"] = str(e)[:200]
-            torch.cuda.synchronize()
-        out[f"{N}^3"] = entry
-        total += ms * n_it
-        h.close()
-    out["dpsr_ms_for_the_paper_schedule"] = total
-    out["what"] = ("forward+backward+point update per iteration, 20,000 points; total = sum over levels of ms x the paper's "
-                   "iteration counts (the paper's whole loop incl. Marching Cubes and Chamfer: 326-380 s per object on a 1080 Ti)")
+def _eager_and_graph(torch, it, iters):
+    """ms per call of `it`, back to back from the host and replayed as a CUDA graph (the library allocates nothing and never
+    synchronises, so an iteration can be captured)."""
+    out = {"ms_per_iteration": _timed_loop(torch, it, iters)}
+    try:
+        stream = torch.cuda.current_stream()
+        side = torch.cuda.Stream()
+        side.wait_stream(stream)
+        with torch.cuda.stream(side):
+            it()
+        stream.wait_stream(side)
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph):
+            it()
+        out["ms_per_iteration_cuda_graph"] = _timed_loop(torch, graph.replay, iters)
+        del graph
+    except Exception as e:   # capture not supported in this environment: keep the eager number
+        out["cuda_graph_error"] = str(e)[:200]
+        torch.cuda.synchronize()
     return out
 
 
-def roofline_of(res, peak_gbs):
-    """Dominant kernel of the step and its achieved bandwidth on the SURVEY 8(d) yardstick bytes."""
+def time_config4_loop(torch, iters=100):
+    """BASELINE.json configs[3] as stated: 100 CONSECUTIVE forward+backward iterations on the 100,000-point cloud at 256^3
+    with a point update between them (points move by up to a quarter cell per iteration, so nothing about the binning can
+    be cached).  Timed end to end with one pair of events around all iterations."""
+    from paper_2106_03452_b200 import inputs
+    from paper_2106_03452_b200.schedule import CoarseToFine, Level
+    cfg, pts, nrm = inputs.make_config(4)
+    sched = CoarseToFine(cfg.P, levels=(Level(cfg.N, cfg.sigma, iters),), with_mesh=False)
+    c, n = torch.from_numpy(pts).cuda(), torch.from_numpy(nrm).cuda()
+    G = torch.from_numpy(inputs.upstream_grad(cfg.N, 1)).cuda()
+
+    def it():
+        sched.run_level(0, c, n, iterations=1, grad_chi=G)
+    out = _eager_and_graph(torch, it, iters)
+    out["iterations"] = iters
+    out["what"] = "forward + backward + point update per iteration, 100,000 points at 256^3, all iterations inside one timed interval (no L2 flush: consecutive iterations)"
+    sched.close()
+    return out
+
+
+def time_coarse_to_fine(iters, torch):
+    """The optimisation-based schedule of the paper (L121, L396) through paper_2106_03452_b200.schedule: 32^3 -> 64^3 ->
+    128^3 (1000 iterations each, sigma 2, 2, 3) -> 256^3 (200 iterations, sigma 3) on 20,000 points.  Two legs per level:
+    `dpsr` = forward + backward with a fixed upstream gradient + point update; `full` = the whole loop of Sec.3.2 on the
+    device (DPSR forward, Marching Cubes, Chamfer to a 20,000-point target, Eq.6, DPSR backward, Adam step)."""
+    from paper_2106_03452_b200 import inputs
+    from paper_2106_03452_b200.schedule import CoarseToFine, paper_levels
+    P = 20000
+    pts, nrm = inputs.make_cloud("torus", P, seed=0)
+    tgt, _ = inputs.make_cloud("ellipsoids3", P, seed=1)
+    levels = paper_levels(3.0)
+    out, total, total_full = {}, 0.0, 0.0
+    for li, lv in enumerate(levels):
+        entry = {"paper_iterations": lv.iterations, "sigma": lv.sigma}
+        sched = CoarseToFine(P, levels=(lv,), with_mesh=True, max_target_points=P)
+        c, n = torch.from_numpy(pts[None].copy()).cuda(), torch.from_numpy(nrm[None].copy()).cuda()
+        G = torch.from_numpy(inputs.upstream_grad(lv.N, 1, seed=lv.N)).cuda()
+        entry["path"] = sched.dpsr[0].path
+        e = _eager_and_graph(torch, lambda: sched.run_level(0, c, n, iterations=1, grad_chi=G), iters)
+        entry["dpsr"] = e
+        total += min(e.values() if "cuda_graph_error" not in e else [e["ms_per_iteration"]]) * lv.iterations
+        c2 = torch.from_numpy(pts[None].copy()).cuda().requires_grad_(True)
+        n2 = torch.from_numpy(nrm[None].copy()).cuda().requires_grad_(True)
+        t = torch.from_numpy(tgt).cuda()
+        opt = torch.optim.Adam([c2, n2], lr=2e-3 * 0.7 ** li)
+        with torch.no_grad():
+            ms = _timed_loop(torch, lambda: sched.run_level(0, c2, n2, iterations=1, target=t, optimizer=opt), iters)
+            b = sched._buffers(0, c2.device)
+            entry["full"] = {"ms_per_iteration": ms, "mesh_vertices": int(b["counts"][0].item()), "mesh_triangles": int(b["counts"][1].item()),
+                             "chamfer_loss": float(b["loss"].item())}
+        total_full += ms * lv.iterations
+        out[f"{lv.N}^3"] = entry
+        sched.close()
+    out["dpsr_ms_for_the_paper_schedule"] = total
+    out["full_loop_ms_for_the_paper_schedule"] = total_full
+    out["what"] = ("per level: ms per iteration on 20,000 points; totals = sum over levels of ms x the paper's iteration counts "
+                   "(dpsr: best of eager / CUDA graph).  The paper's whole loop took 326-380 s per object on a 1080 Ti with "
+                   "Marching Cubes on the CPU (Table 2, L166-L176)")
+    return out
+
+
+def time_cufft_comparison(cfg_ids, steps, torch, flush):
+    """BENCH-ONLY yardstick (the product links no cuFFT): the library pipeline the paper describes (L84) for the
+    same sizes -- torch.fft (cuFFT) 3 x rfftn + pointwise solve + 1 x irfftn forward, 1 x rfftn + pointwise + 3 x irfftn
+    backward -- WITHOUT splat, normalisation or gather.  Same L2 flush and event protocol as the headline."""
+    out = {}
+    for cid in cfg_ids:
+        from paper_2106_03452_b200 import inputs
+        cfg = inputs.CONFIGS[cid]
+        N, B = cfg.N, cfg.batch
+        v = torch.randn((B, 3, N, N, N), device="cuda")
+        g = torch.randn((B, N, N, N), device="cuda")
+        k = torch.fft.fftfreq(N, 1.0 / N, device="cuda")
+        kz = torch.fft.rfftfreq(N, 1.0 / N, device="cuda")
+        KX, KY, KZ = torch.meshgrid(k, k, kz, indexing="ij")
+        q = KX * KX + KY * KY + KZ * KZ
+        f = torch.exp(-2.0 * cfg.sigma ** 2 * q / N ** 2) / (-2.0 * np.pi * q.clamp_min(1.0))
+        f[0, 0, 0] = 0.0
+        M = torch.stack([KX * f, KY * f, KZ * f]).to(torch.complex64) * 1j       # [3, N, N, N/2+1]
+
+        def step():
+            vh = torch.fft.rfftn(v, dim=(-3, -2, -1))
+            chi = torch.fft.irfftn((vh * M).sum(1), s=(N, N, N), dim=(-3, -2, -1))
+            gh = torch.fft.rfftn(g, dim=(-3, -2, -1))
+            vb = torch.fft.irfftn(gh[:, None] * M.conj(), s=(N, N, N), dim=(-3, -2, -1))
+            return chi, vb
+        for _ in range(3):
+            step()
+        torch.cuda.synchronize()
+        tot = 0.0
+        for _ in range(steps):
+            flush.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            step()
+            b.record()
+            torch.cuda.synchronize()
+            tot += a.elapsed_time(b)
+        out[cfg.name] = {"ms_per_grid": tot / steps / B, "what": "cuFFT via torch.fft: 4 rfftn + 4 irfftn + 2 pointwise multiplies; no splat / normalise / gather"}
+        del v, g, M, q, f, KX, KY, KZ
+        torch.cuda.empty_cache()
+    return out
+
+
+def time_mesh_steps(torch, flush, N=128, P=20000, steps=10):
+    """Marching Cubes / Chamfer / Eq.6 kernels alone (sap_mesh.h) on the indicator grid of a 20,000-point torus."""
+    from paper_2106_03452_b200 import inputs
+    from paper_2106_03452_b200.binding import Dpsr
+    from paper_2106_03452_b200.mesh import Mesh
+    pts, nrm = inputs.make_cloud("torus", P, seed=0)
+    tgt, _ = inputs.make_cloud("torus", P, seed=1)
+    d = Dpsr(N, 3.0, 1, P)
+    m = Mesh(N, 12 * N * N, 24 * N * N, 12 * N * N)
+    chi = d.forward(torch.from_numpy(pts[None].copy()).cuda(), torch.from_numpy(nrm[None].copy()).cuda())
+    t = torch.from_numpy(tgt).cuda()
+    verts, normals, tris, counts = m.extract(chi[0])
+    loss, gv, _, _ = m.chamfer(verts, t, na_dev=counts)
+    G = m.backward(gv, normals)
+    torch.cuda.synchronize()
+    out = {"N": N, "mesh_vertices": int(counts[0].item()), "mesh_triangles": int(counts[1].item()), "target_points": P}
+
+    def timed(fn):
+        tot = 0.0
+        for _ in range(steps):
+            flush.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); fn(); b.record()
+            torch.cuda.synchronize()
+            tot += a.elapsed_time(b)
+        return tot / steps
+    out["marching_cubes_ms"] = timed(lambda: m.extract(chi[0], verts, normals, tris, counts))
+    out["chamfer_ms"] = timed(lambda: m.chamfer(verts, t, na_dev=counts, loss=loss, grad_a=gv))
+    out["eq6_backward_ms"] = timed(lambda: m.backward(gv, normals, G))
+    out["paper_context"] = "PAPER.md Table 4: Marching Cubes (CPU library) 0.039 s at 128^3, 0.374 s at 256^3"
+    d.close(); m.close()
+    return out
+
+
+def roofline_of(res, peak_gbs, traffic):
+    """Dominant kernel of the step (longest average launch) and its achieved bandwidth on the bytes the kernel itself must
+    read once + write once (KERNEL_BYTES_V).  At 128^3 batch 1 the working set lives in the 126 MB L2, so the fraction says how
+    far the launch is from streaming its compulsory bytes at HBM speed, not that it is HBM-bound."""
     cfg = res["cfg"]
     V = 4.0 * cfg.N ** 3 * cfg.batch
-    fused = cfg.N <= 128
     km = res["kernels_ms"]
     name = max(km, key=km.get)
-    yard_v, comp_v = (KERNEL_BYTES_V[name][0], KERNEL_BYTES_V[name][2]) if fused else (KERNEL_BYTES_V[name][1], KERNEL_BYTES_V[name][3])
-    ach = yard_v * V / (km[name] * 1e-3) / 1e9
-    comp = comp_v * V / (km[name] * 1e-3) / 1e9
+    comp_v = KERNEL_BYTES_V[name][0 if cfg.N <= 128 else 1]
+    ach = comp_v * V / (km[name] * 1e-3) / 1e9
+    t = traffic.get(cfg.name, {}).get(name)
     return {"bound": "hbm", "kernel": name, "kernel_ms": km[name], "share_of_step": km[name] / sum(km.values()),
-            "achieved": ach, "peak": peak_gbs, "unit": "GB/s", "frac": ach / peak_gbs,
-            "traffic": NCU_TRAFFIC.get(cfg.name, {}).get(name),
-            "algorithmic_bytes": yard_v * V, "achieved_compulsory": comp, "frac_compulsory": comp / peak_gbs,
-            "compulsory_bytes": comp_v * V}
+            "achieved": ach, "peak": peak_gbs, "unit": "GB/s", "frac": ach / peak_gbs, "traffic": t,
+            "algorithmic_bytes": comp_v * V, "algorithmic_bytes_in_V": comp_v}
+
+
+def kernel_fracs(res, peak_gbs):
+    """compulsory bytes / time / measured peak for every grid kernel of the step"""
+    cfg = res["cfg"]
+    V = 4.0 * cfg.N ** 3 * cfg.batch
+    out = {}
+    for k, ms in res["kernels_ms"].items():
+        cv = KERNEL_BYTES_V.get(k, (0.0, 0.0))[0 if cfg.N <= 128 else 1]
+        if cv > 0:
+            out[k] = round(cv * V / (ms * 1e-3) / 1e9 / peak_gbs, 3)
+    return out
+
+
+def oracle_baseline(cfg_id, reps):
+    """The float64 oracle as it stands on ONE grid of config cfg_id (512^3: a bounded sample, see `sample`)."""
+    from oracle import dpsr_oracle as orc
+    from paper_2106_03452_b200 import inputs
+    cfg = inputs.CONFIGS[cfg_id]
+    scale, N, P = 1.0, cfg.N, cfg.P
+    if cfg.N > 256:    # 512^3 costs the oracle ~3.5 minutes: time the same shape at 256^3 with P/8 points, scale by the O(N^4) law
+        N, P, scale = 256, cfg.P // 8, (cfg.N / 256.0) ** 4
+    pts, nrm = inputs.make_cloud(cfg.shape, P, seed=0)
+    G = inputs.upstream_grad(N, 1)[0]
+    c = inputs.Config(cfg.name, N, 1, P, cfg.sigma, cfg.shape)
+    t = min(oracle_step(c, pts, nrm, G) for _ in range(reps))
+    sample = f"1 grid (N={N}, P={P}), forward+backward, best of {reps}"
+    if scale != 1.0:
+        sample += f"; x{scale:g} = (N_workload/N_sample)^4, the cost law of the oracle's naive separable DFT"
+    return {"value": 1e3 * t * scale, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle", "sample": sample}
 
 
 def main():
@@ -375,6 +518,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (1-based); default configs[1]")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--path", default="auto", choices=["auto", "throughput", "latency"], help="SAP_PATH_* of the headline handle")
     ap.add_argument("--also", default="3,4,5", help="other configs to report under 'also' (rank 0, N=1 only); '' = none")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -395,6 +539,7 @@ def main():
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     peak, peak_src = read_peaks()
+    traffic, traffic_src = load_traffic()
     flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device="cuda")
 
     def barrier():
@@ -405,7 +550,7 @@ def main():
     # headline: device-resident timing, barrier + synchronize on both sides, clocks sampled meanwhile
     barrier()
     with ClockSampler(local) as cs:
-        res = time_config(args.config, args.steps, args.warmup, rank, torch, flush, with_e2e=False, with_profile=False)
+        res = time_config(args.config, args.steps, args.warmup, rank, torch, flush, with_e2e=False, with_profile=False, path=args.path)
         barrier()
     clocks = cs.summary()
     t_ms = torch.tensor([res["ms_total"]], dtype=torch.float64, device="cuda")
@@ -413,7 +558,7 @@ def main():
         dist.all_reduce(t_ms, op=dist.ReduceOp.MAX)
     t_total = float(t_ms.item())
     # per-kernel pass + end-to-end pass (separate so that their events/copies do not perturb `value`)
-    res2 = time_config(args.config, args.steps, args.warmup, rank, torch, flush, with_e2e=True, with_profile=True)
+    res2 = time_config(args.config, args.steps, args.warmup, rank, torch, flush, with_e2e=True, with_profile=True, path=args.path)
     e2e = torch.tensor([res2["e2e_ms_step"]], dtype=torch.float64, device="cuda")
     if dist is not None:
         dist.all_reduce(e2e, op=dist.ReduceOp.MAX)
@@ -427,19 +572,23 @@ def main():
         "ms_per_step": ms_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic",
         "config": {"workload": cfg.name, "N": cfg.N, "batch": cfg.batch, "points": cfg.P, "sigma": cfg.sigma,
-                   "parallelism": f"replicas x{world} (no collective)", "l2": "flushed between steps (256 MB write)"},
+                   "parallelism": f"replicas x{world} (no collective)", "l2": "flushed between steps (256 MB write)",
+                   "path": res["path"]},
         "ms_fwd": res["ms_fwd"], "ms_bwd": res["ms_bwd"], "grids_per_s": 1e3 / value,
-        "path_GBps_52V": YARD_FWD_BWD_V * V / (value * 1e-3) / 1e9,
-        "path_frac_52V": YARD_FWD_BWD_V * V / (value * 1e-3) / 1e9 / (peak * world),
+        "fusion_gain_vs_52V_model": {"what": "bytes the unfused per-axis-pass model of SURVEY 8(d) would move (52 V) / (time x measured HBM peak): "
+                                             ">1 means the path is faster than that model could be at full HBM speed; NOT a fraction of peak",
+                                     "value": YARD_FWD_BWD_V * V / (value * 1e-3) / 1e9 / (peak * world)},
         "clocks": clocks,
         "e2e": {"value": float(e2e.item()) / grids, "unit": UNIT, "h2d_bytes_per_step": res2["h2d"],
                 "d2h_bytes_per_step": res2["d2h"]},
         "gpu_launches": res["launches"],
-        "roofline": dict(roofline_of(res2, peak), peak_source=peak_src),
+        "roofline": dict(roofline_of(res2, peak, traffic), peak_source=peak_src, traffic_source=traffic_src),
         "kernels_ms": res2["kernels_ms"],
+        "kernel_frac_of_hbm_peak": kernel_fracs(res2, peak),
         "paper_context": "PAPER.md Table 4: 12 ms forward only at 128^3, 140 ms at 256^3, on a GTX 1080 Ti (not the target)",
     }
-    if rank == 0 and world == 1 and args.also:
+    solo = rank == 0 and world == 1
+    if solo and args.also:
         also = {}
         for cid in [int(x) for x in args.also.split(",") if x.strip()]:
             if cid == args.config:
@@ -449,24 +598,43 @@ def main():
             c = r["cfg"]
             Vc = 4.0 * c.N ** 3
             per_grid = r["ms_step"] / c.batch
-            also[c.name] = {"ms_per_grid": per_grid, "ms_fwd": r["ms_fwd"], "ms_bwd": r["ms_bwd"], "steps": k,
+            km = r["kernels_ms"]
+            actual = sum(traffic.get(c.name, {}).values())
+            also[c.name] = {"ms_per_grid": per_grid, "ms_fwd": r["ms_fwd"], "ms_bwd": r["ms_bwd"], "steps": k, "path": r["path"],
                             "grids_per_s": 1e3 / per_grid,
-                            "path_frac_52V": YARD_FWD_BWD_V * Vc / (per_grid * 1e-3) / 1e9 / peak,
-                            "roofline": roofline_of(r, peak), "kernels_ms": r["kernels_ms"]}
-        line["also"] = also
-    if rank == 0 and world == 1 and args.also:
-        line["also"]["coarse_to_fine_schedule"] = time_coarse_to_fine(20, torch, flush)
-    if rank == 0 and world == 1 and args.also and "3" in args.also.split(","):
-        line["also"]["cfg3_fused_mse_loss"] = time_fused_mse(3, 10, 3, torch, flush)
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        from oracle import dpsr_oracle as orc
+                            "fusion_gain_vs_52V_model": YARD_FWD_BWD_V * Vc / (per_grid * 1e-3) / 1e9 / peak,
+                            "dram_bytes_per_fwd_bwd_in_V": (actual / (Vc * c.batch)) if actual else None,
+                            "dram_GBps_actual": (actual / c.batch / (per_grid * 1e-3) / 1e9) if actual else None,
+                            "roofline": roofline_of(r, peak, traffic), "kernels_ms": km,
+                            "kernel_frac_of_hbm_peak": kernel_fracs(r, peak)}
+            if not args.no_cpu_baseline:
+                also[c.name]["cpu_baseline"] = oracle_baseline(cid, 1)
+        # both implementations of the path where the latency path applies
         from paper_2106_03452_b200 import inputs
-        c, pts, nrm = inputs.make_config(args.config, batch=1)
-        G = inputs.upstream_grad(c.N, 1)[0]
-        reps = 3 if c.N <= 128 else 1
-        t = min(oracle_step(c, pts[0], nrm[0], G) for _ in range(reps))
-        line["cpu_baseline"] = {"value": 1e3 * t, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
-                                "sample": f"1 grid of the workload (N={c.N}, P={c.P}), forward+backward, best of {reps}"}
+        paths = {}
+        for name, N, P, shape in (("32^3", 32, 3000, "sphere"), ("64^3", 64, 20000, "torus"), ("128^3", 128, 20000, "torus")):
+            pts, nrm = inputs.make_cloud(shape, P, seed=0)
+            custom = (inputs.Config(name, N, 1, P, 2.0, shape), pts[None].copy(), nrm[None].copy(), inputs.upstream_grad(N, 1))
+            e = {}
+            for path in ("throughput", "latency"):
+                r = time_config(0, 20, 3, rank, torch, flush, with_e2e=False, with_profile=(path == "latency"), path=path, custom=custom)
+                e[path + "_ms"] = r["ms_step"]
+                if path == "latency":
+                    e["latency_phases_us"] = r.get("fused_phases_us")
+            paths[name] = e
+        also["paths_throughput_vs_latency"] = paths
+        if "4" in args.also.split(","):
+            also["cfg4_100_iterations_with_point_updates"] = time_config4_loop(torch)
+        also["cufft_comparison"] = time_cufft_comparison([c for c in (2, 3, 4, 5) if str(c) in args.also.split(",") or c == args.config], 5, torch, flush)
+        also["coarse_to_fine_schedule"] = time_coarse_to_fine(20, torch)
+        also["mesh_kernels_128"] = time_mesh_steps(torch, flush, 128)
+        if "4" in args.also.split(","):
+            also["mesh_kernels_256"] = time_mesh_steps(torch, flush, 256)
+        if "3" in args.also.split(","):
+            also["cfg3_fused_mse_loss"] = time_fused_mse(3, 10, 3, torch, flush)
+        line["also"] = also
+    if solo and not args.no_cpu_baseline:
+        line["cpu_baseline"] = oracle_baseline(args.config, 3 if cfg.N <= 128 else 1)
     if dist is not None:
         dist.barrier()
         dist.destroy_process_group()

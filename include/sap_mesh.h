@@ -75,6 +75,16 @@ sap_status_t sap_mc_backward(sap_mesh_t* h, const float* grad_verts, const float
 sap_status_t sap_chamfer(sap_mesh_t* h, const float* a, int na, const int* na_dev, const float* b, int nb, float* loss,
                          float* grad_a, int* nn_a, int* nn_b, void* stream);
 
+/*
+ * The plain point update of BASELINE.json configs[3] ("iterations with a point update between them") and of the
+ * fixed-gradient mode of the coarse-to-fine driver, as two small kernels instead of a dozen framework ops:
+ *   eta = move / (N max |grad_points|);  points <- clip(points - eta grad_points, 0, 1 - 1e-6);  normals <- normals - eta grad_normals
+ * i.e. the largest point step is `move` cells of an N^3 grid.  All arrays dev float [count] (count = batch * P * 3),
+ * scratch dev [1] unsigned.  (The paper's own loop uses Adam, L396: that stays with the host framework.)
+ */
+sap_status_t sap_points_sgd_step(float* points, float* normals, const float* grad_points, const float* grad_normals,
+                                 int count, int N, float move, unsigned* scratch, void* stream);
+
 /* The cube triangulation built at load (M3), for tests: ntri[256], tris[256][12][3] cube-edge ids (-1 padded).
  * Cube corner c has offsets (c & 1, (c >> 1) & 1, (c >> 2) & 1); cube edge 4 a + k runs along axis a, k = u + 2 v with
  * (u, v) the offsets along the two other axes in increasing order.  Returns the largest triangle count of a cube. */

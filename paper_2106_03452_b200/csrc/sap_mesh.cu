@@ -299,17 +299,24 @@ __global__ void k_mc_eq6(int N, int lg, const unsigned char* __restrict__ code, 
 }
 
 // ---- Chamfer kernels -------------------------------------------------------------------------------------------------
+constexpr int GC_MAX = 64;   // cells per axis of the largest grid (the workspace is sized for it)
 __device__ __forceinline__ int count_of(int n, const int* n_dev) { return n_dev ? min(*n_dev, n) : n; }
+// Cells per axis for a set of n points: about 2 points per cell on average (a surface fills O(Gc^2) of the Gc^3 cells
+// with ~2 Gc / 3 points each).  Computed ON THE DEVICE from the actual count -- the size of a mesh is only known there --
+// identically in every kernel that touches the grid, so a small set gets a coarse grid and a far query few rings.
+__device__ __forceinline__ int grid_cells(int n) { return min(max((int)cbrtf(0.5f * (float)n), 2), GC_MAX); }
 __device__ __forceinline__ int cell_coord(float c, int Gc) { return min(max((int)floorf(c * (float)Gc), 0), Gc - 1); }
-__global__ void k_cell_count(const float* __restrict__ pts, int n, const int* n_dev, int Gc, int* __restrict__ cnt) {
+__global__ void k_cell_count(const float* __restrict__ pts, int n, const int* n_dev, int* __restrict__ cnt) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int Gc = grid_cells(count_of(n, n_dev));
     if (i >= count_of(n, n_dev)) return;
     const int c = (cell_coord(pts[3 * i], Gc) * Gc + cell_coord(pts[3 * i + 1], Gc)) * Gc + cell_coord(pts[3 * i + 2], Gc);
     atomicAdd(cnt + c, 1);
 }
 // one block: start = exclusive scan of cnt over ncell entries (+ total at [ncell]); cursor = start
-__global__ void k_cell_scan(const int* __restrict__ cnt, int ncell, int* __restrict__ start, int* __restrict__ cursor) {
+__global__ void k_cell_scan(int* __restrict__ cnt, int n, const int* n_dev, int* __restrict__ start, int* __restrict__ cursor) {
     __shared__ int part[1024];
+    const int Gc = grid_cells(count_of(n, n_dev)), ncell = Gc * Gc * Gc;
     const int tid = threadIdx.x, per = (ncell + 1023) / 1024;
     const int lo = tid * per, hi = min(lo + per, ncell);
     int s = 0;
@@ -324,15 +331,18 @@ __global__ void k_cell_scan(const int* __restrict__ cnt, int ncell, int* __restr
     }
     int run = part[tid] - s;
     for (int i = lo; i < hi; ++i) {
+        const int c = cnt[i];
         start[i] = run;
         cursor[i] = run;
-        run += cnt[i];
+        cnt[i] = 0;              // the counters are zero again for the next grid
+        run += c;
     }
     if (tid == 1023) start[ncell] = part[1023];
 }
-__global__ void k_cell_scatter(const float* __restrict__ pts, int n, const int* n_dev, int Gc, int* __restrict__ cursor,
+__global__ void k_cell_scatter(const float* __restrict__ pts, int n, const int* n_dev, int* __restrict__ cursor,
                                float4* __restrict__ sorted) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int Gc = grid_cells(count_of(n, n_dev));
     if (i >= count_of(n, n_dev)) return;
     const float x = pts[3 * i], y = pts[3 * i + 1], z = pts[3 * i + 2];
     const int c = (cell_coord(x, Gc) * Gc + cell_coord(y, Gc)) * Gc + cell_coord(z, Gc);
@@ -340,12 +350,13 @@ __global__ void k_cell_scatter(const float* __restrict__ pts, int n, const int* 
 }
 // exact nearest neighbour of every query in the binned set: rings of cells of growing Chebyshev radius r around the
 // query's cell; every point not yet visited after ring r is at least r / Gc away, so the search stops once best <= (r/Gc)^2
-__global__ void k_nn_query(const float* __restrict__ q, int nq, const int* nq_dev, int Gc, const int* __restrict__ start,
+__global__ void k_nn_query(const float* __restrict__ q, int nq, const int* nq_dev, const int* __restrict__ start,
                            const float4* __restrict__ sorted, int ntarget, const int* ntarget_dev, int* __restrict__ nn,
                            float* __restrict__ d2out) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= count_of(nq, nq_dev)) return;
     if (count_of(ntarget, ntarget_dev) <= 0) { nn[i] = -1; d2out[i] = 0.f; return; }
+    const int Gc = grid_cells(count_of(ntarget, ntarget_dev));
     const float px = q[3 * i], py = q[3 * i + 1], pz = q[3 * i + 2];
     const int cx = cell_coord(px, Gc), cy = cell_coord(py, Gc), cz = cell_coord(pz, Gc);
     const float h = 1.f / (float)Gc;
@@ -433,7 +444,7 @@ __global__ void k_loss_store(double* __restrict__ lacc, float* __restrict__ loss
 
 // ================================================================================================
 struct sap_mesh {
-    int N = 0, lg = 0, max_v = 0, max_t = 0, max_p = 0, device = 0, Gc = 0, launches = 0;
+    int N = 0, lg = 0, max_v = 0, max_t = 0, max_p = 0, device = 0, launches = 0;
     unsigned char* code = nullptr;       // [N^3]
     unsigned char* cfg = nullptr;        // [N^3]
     unsigned long long* blocksum = nullptr;  // [N^3 / MC_BLOCK]
@@ -442,9 +453,9 @@ struct sap_mesh {
     float* vt = nullptr;                 // [max_v]
     int* counts_dev = nullptr;           // [2] of the last extract (device copy kept for the backward)
     // Chamfer
-    int* cell_cnt = nullptr;             // [Gc^3]
-    int* cell_start = nullptr;           // [Gc^3 + 1]
-    int* cell_cursor = nullptr;          // [Gc^3]
+    int* cell_cnt = nullptr;             // [GC_MAX^3], zero between uses
+    int* cell_start = nullptr;           // [GC_MAX^3 + 1]
+    int* cell_cursor = nullptr;          // [GC_MAX^3]
     float4* sorted = nullptr;            // [max_p]
     int* nn_tmp_a = nullptr;             // [max_p]
     int* nn_tmp_b = nullptr;             // [max_p]
@@ -516,9 +527,7 @@ extern "C" sap_status_t sap_mesh_create(int N, int max_vertices, int max_triangl
     sap_mesh* h = new (std::nothrow) sap_mesh;
     if (!h) { g_err = "host allocation failed"; return SAP_ERR_OOM; }
     h->N = N; h->lg = lg; h->max_v = max_vertices; h->max_t = max_triangles; h->max_p = max_points; h->device = dev;
-    int gc = (int)lround(cbrt((double)max_points / 2.0));
-    h->Gc = gc < 4 ? 4 : gc > 128 ? 128 : gc;
-    const size_t V = (size_t)N * N * N, C = (size_t)h->Gc * h->Gc * h->Gc;
+    const size_t V = (size_t)N * N * N, C = (size_t)GC_MAX * GC_MAX * GC_MAX;
     cudaError_t e = cudaSuccess;
     auto upd = [&](cudaError_t x) { if (e == cudaSuccess) e = x; };
     upd(alloc(h, &h->code, V)); upd(alloc(h, &h->cfg, V)); upd(alloc(h, &h->blocksum, V / MC_BLOCK));
@@ -530,6 +539,7 @@ extern "C" sap_status_t sap_mesh_create(int N, int max_vertices, int max_triangl
     upd(alloc(h, &h->d2_a, (size_t)max_points)); upd(alloc(h, &h->d2_b, (size_t)max_points));
     upd(alloc(h, &h->lacc, (size_t)1));
     if (e == cudaSuccess) upd(cudaMemset(h->lacc, 0, sizeof(double)));
+    if (e == cudaSuccess) upd(cudaMemset(h->cell_cnt, 0, sizeof(int) * C));
     if (e == cudaSuccess) upd(cudaMemset(h->counts_dev, 0, 2 * sizeof(int)));
     if (e == cudaSuccess) {
         const CubeTables& T = cube_tables();
@@ -584,7 +594,6 @@ extern "C" sap_status_t sap_chamfer(sap_mesh_t* h, const float* a, int na, const
     if (!a || !b || !loss) { h->err = "null pointer argument"; return SAP_ERR_INVALID_ARG; }
     if (na < 0 || nb < 1 || na > h->max_p || nb > h->max_p) { h->err = "point counts out of range (0 <= na <= max_points, 1 <= nb <= max_points)"; return SAP_ERR_INVALID_ARG; }
     cudaStream_t s = (cudaStream_t)stream;
-    const int Gc = h->Gc, ncell = Gc * Gc * Gc;
     int* nna = nn_a ? nn_a : h->nn_tmp_a;
     int* nnb = nn_b ? nn_b : h->nn_tmp_b;
     if (na == 0) {
@@ -593,32 +602,67 @@ extern "C" sap_status_t sap_chamfer(sap_mesh_t* h, const float* a, int na, const
     }
     const int ga = (na + 255) / 256, gb = (nb + 255) / 256;
     // grid over b, queries a
-    if (!ok(h, cudaMemsetAsync(h->cell_cnt, 0, sizeof(int) * ncell, s), "memset cells")) return SAP_ERR_CUDA;
-    k_cell_count<<<gb, 256, 0, s>>>(b, nb, nullptr, Gc, h->cell_cnt);
+    k_cell_count<<<gb, 256, 0, s>>>(b, nb, nullptr, h->cell_cnt);
     MESH_LAUNCH_CHECK(h, "k_cell_count");
-    k_cell_scan<<<1, 1024, 0, s>>>(h->cell_cnt, ncell, h->cell_start, h->cell_cursor);
+    k_cell_scan<<<1, 1024, 0, s>>>(h->cell_cnt, nb, nullptr, h->cell_start, h->cell_cursor);
     MESH_LAUNCH_CHECK(h, "k_cell_scan");
-    k_cell_scatter<<<gb, 256, 0, s>>>(b, nb, nullptr, Gc, h->cell_cursor, h->sorted);
+    k_cell_scatter<<<gb, 256, 0, s>>>(b, nb, nullptr, h->cell_cursor, h->sorted);
     MESH_LAUNCH_CHECK(h, "k_cell_scatter");
-    k_nn_query<<<ga, 256, 0, s>>>(a, na, na_dev, Gc, h->cell_start, h->sorted, nb, nullptr, nna, h->d2_a);
+    k_nn_query<<<ga, 256, 0, s>>>(a, na, na_dev, h->cell_start, h->sorted, nb, nullptr, nna, h->d2_a);
     MESH_LAUNCH_CHECK(h, "k_nn_query");
     k_chamfer_a<<<ga, 256, 0, s>>>(a, na, na_dev, b, nna, h->d2_a, grad_a, h->lacc);
     MESH_LAUNCH_CHECK(h, "k_chamfer_a");
     // grid over a, queries b
-    if (!ok(h, cudaMemsetAsync(h->cell_cnt, 0, sizeof(int) * ncell, s), "memset cells")) return SAP_ERR_CUDA;
-    k_cell_count<<<ga, 256, 0, s>>>(a, na, na_dev, Gc, h->cell_cnt);
+    k_cell_count<<<ga, 256, 0, s>>>(a, na, na_dev, h->cell_cnt);
     MESH_LAUNCH_CHECK(h, "k_cell_count");
-    k_cell_scan<<<1, 1024, 0, s>>>(h->cell_cnt, ncell, h->cell_start, h->cell_cursor);
+    k_cell_scan<<<1, 1024, 0, s>>>(h->cell_cnt, na, na_dev, h->cell_start, h->cell_cursor);
     MESH_LAUNCH_CHECK(h, "k_cell_scan");
-    k_cell_scatter<<<ga, 256, 0, s>>>(a, na, na_dev, Gc, h->cell_cursor, h->sorted);
+    k_cell_scatter<<<ga, 256, 0, s>>>(a, na, na_dev, h->cell_cursor, h->sorted);
     MESH_LAUNCH_CHECK(h, "k_cell_scatter");
-    k_nn_query<<<gb, 256, 0, s>>>(b, nb, nullptr, Gc, h->cell_start, h->sorted, na, na_dev, nnb, h->d2_b);
+    k_nn_query<<<gb, 256, 0, s>>>(b, nb, nullptr, h->cell_start, h->sorted, na, na_dev, nnb, h->d2_b);
     MESH_LAUNCH_CHECK(h, "k_nn_query");
     k_chamfer_b<<<gb, 256, 0, s>>>(a, na, na_dev, b, nb, nnb, h->d2_b, grad_a, h->lacc);
     MESH_LAUNCH_CHECK(h, "k_chamfer_b");
     k_loss_store<<<1, 1, 0, s>>>(h->lacc, loss);
     MESH_LAUNCH_CHECK(h, "k_loss_store");
     return SAP_OK;
+}
+
+// eta = move / (N max|gp|);  points <- clip(points - eta gp, 0, 1 - 1e-6);  normals <- normals - eta gn
+namespace sapm {
+__global__ void k_absmax(const float* __restrict__ g, int n, unsigned* __restrict__ out) {
+    __shared__ float sh[32];
+    float m = 0.f;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) m = fmaxf(m, fabsf(g[i]));
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = m;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < (int)(blockDim.x >> 5); ++w) m = fmaxf(m, sh[w]);
+        atomicMax(out, __float_as_uint(m));   // non-negative floats order like their bit patterns
+    }
+}
+__global__ void k_sgd_apply(float* __restrict__ pts, float* __restrict__ nrm, const float* __restrict__ gp, const float* __restrict__ gn,
+                            int n, float move_over_N, unsigned* __restrict__ gmax) {
+    const float eta = move_over_N / fmaxf(__uint_as_float(*gmax), 1e-20f);
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) {
+        pts[i] = fminf(fmaxf(pts[i] - eta * gp[i], 0.f), 1.f - 1e-6f);
+        nrm[i] -= eta * gn[i];
+    }
+}
+__global__ void k_zero_u32(unsigned* p) { *p = 0u; }
+}  // namespace sapm
+extern "C" sap_status_t sap_points_sgd_step(float* points, float* normals, const float* grad_points, const float* grad_normals,
+                                            int count, int N, float move, unsigned* scratch, void* stream) {
+    if (!points || !normals || !grad_points || !grad_normals || !scratch || count < 1 || N < 1) return SAP_ERR_INVALID_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    const int nb = (count + 255) / 256;
+    k_zero_u32<<<1, 1, 0, s>>>(scratch);
+    k_absmax<<<nb < 296 ? nb : 296, 256, 0, s>>>(grad_points, count, scratch);
+    k_sgd_apply<<<nb, 256, 0, s>>>(points, normals, grad_points, grad_normals, count, move / (float)N, scratch);
+    return cudaGetLastError() == cudaSuccess ? SAP_OK : SAP_ERR_CUDA;
 }
 
 extern "C" void sap_mesh_destroy(sap_mesh_t* h) {

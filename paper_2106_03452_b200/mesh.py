@@ -8,7 +8,7 @@ import ctypes
 from .binding import SAP_OK, SapError, _stream_ptr, lib as _dpsr_lib
 
 EXPORTS = ["sap_mesh_create", "sap_mc_extract", "sap_mc_backward", "sap_chamfer", "sap_mc_table", "sap_mesh_destroy",
-           "sap_mesh_last_error", "sap_mesh_workspace_bytes", "sap_mesh_last_launch_count"]
+           "sap_mesh_last_error", "sap_mesh_workspace_bytes", "sap_mesh_last_launch_count", "sap_points_sgd_step"]
 MC_MAX_TRI = 12
 _ready = False
 
@@ -28,6 +28,8 @@ def lib():
         L.sap_chamfer.restype = ci
         L.sap_mc_table.argtypes = [vp, vp]
         L.sap_mc_table.restype = ci
+        L.sap_points_sgd_step.argtypes = [vp, vp, vp, vp, ci, ci, ctypes.c_float, vp, vp]
+        L.sap_points_sgd_step.restype = ci
         L.sap_mesh_destroy.argtypes = [vp]
         L.sap_mesh_destroy.restype = None
         L.sap_mesh_last_error.argtypes = [vp]
@@ -47,6 +49,15 @@ def mc_table():
     tris = np.zeros((256, MC_MAX_TRI, 3), np.int32)
     lib().sap_mc_table(ntri.ctypes.data_as(ctypes.c_void_p), tris.ctypes.data_as(ctypes.c_void_p))
     return ntri, tris
+
+
+def sgd_step(points, normals, grad_points, grad_normals, N, move, scratch, stream=None):
+    """sap_points_sgd_step on CUDA float32 tensors of equal size (in place); scratch: CUDA int32/uint32 tensor [1]."""
+    st = lib().sap_points_sgd_step(ctypes.c_void_p(points.data_ptr()), ctypes.c_void_p(normals.data_ptr()),
+                                   ctypes.c_void_p(grad_points.data_ptr()), ctypes.c_void_p(grad_normals.data_ptr()),
+                                   int(points.numel()), int(N), float(move), ctypes.c_void_p(scratch.data_ptr()), _stream_ptr(stream))
+    if st != SAP_OK:
+        raise SapError(st, "sap_points_sgd_step")
 
 
 class Mesh:

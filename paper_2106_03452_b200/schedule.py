@@ -34,11 +34,18 @@ def paper_levels(sigma_final: float = 3.0):
     return (Level(32, 2.0, 1000), Level(64, 2.0, 1000), Level(128, 3.0, 1000), Level(256, float(sigma_final), 200))
 
 
+_scratch = {}
+
+
 def sgd_update(points, normals, gp, gn, N, move=0.25):
-    """The plain update of the fixed-gradient mode, in place, on the device (elementwise torch ops; no host sync)."""
-    eta = move / N / gp.abs().max().clamp_min(1e-20)
-    points.sub_(eta * gp).clamp_(0.0, 1.0 - 1e-6)
-    normals.sub_(eta * gn)
+    """The plain update of the fixed-gradient mode, in place, on the device, no host sync (sap_points_sgd_step: two small
+    kernels): eta = move / (N max|gp|); points <- clip(points - eta gp, 0, 1 - 1e-6); normals <- normals - eta gn."""
+    import torch
+    from .mesh import sgd_step
+    key = points.device
+    if key not in _scratch:
+        _scratch[key] = torch.zeros((1,), dtype=torch.int32, device=points.device)
+    sgd_step(points, normals, gp, gn, N, move, _scratch[key])
 
 
 class CoarseToFine:

@@ -35,7 +35,7 @@ def test_mesh_header_symbols_are_exported_and_table_matches_the_oracle(lib):
     from paper_2106_03452_b200 import mesh
     text = (ROOT / "include" / "sap_mesh.h").read_text()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    names = sorted(set(re.findall(r"\b(sap_(?:mesh|mc|chamfer)[a-z_]*)\s*\(", text)))
+    names = sorted(set(re.findall(r"\b(sap_(?:mesh|mc|chamfer|points)[a-z_]*)\s*\(", text)))
     assert len(names) >= 8 and sorted(mesh.EXPORTS) == names
     L = mesh.lib()
     for n in names:
