@@ -148,7 +148,7 @@ sap_status_t sap_dpsr_reserve(sap_dpsr_t* h, int what);
  *                        the 32^3 / 64^3 / 128^3 levels of the coarse-to-fine schedule, at batch 1).
  * SAP_PATH_AUTO (default) takes the latency path where it measured faster (eligible handles with N <= 64), else the
  * throughput path; SAP_PATH_LATENCY forces it on any eligible handle (else SAP_ERR_UNSUPPORTED).  Both leave the same state in the
- * handle, so a forward on one path may be followed by the backward on the other.  sap_dpsr_get_path returns the path
+ handle, so a forward on one path may be followed by the backward on the other.  sap_dpsr_get_path returns the path
  * the next call will take.  The fused-loss entry points always use the throughput path.
  */
 enum { SAP_PATH_AUTO = 0, SAP_PATH_THROUGHPUT = 1, SAP_PATH_LATENCY = 2 };

@@ -138,35 +138,6 @@ SAP_HD int bits_f2i(float f) {
     union { int i; float f; } u; u.f = f; return u.i;
 #endif
 }
-// ---- fixed-point rasterisation ---------------------------------------------------------------------------------------
-// The trilinear splat accumulates into shared memory with NATIVE 32-bit integer atomics (a float atomicAdd on shared
-// memory is a compare-and-swap loop, measured at ~400 cycles per add here: 12 of them per point were the straggler
-// of the whole forward).  Each contribution w * n_c is rounded once to a multiple of the quantum 1/S; S is a power of
-// two chosen per tile from bound = sum over the tile's points of max_c |n_ic|  >=  |any cell sum|, so that
-// bound * S < 2^30: overflow is impossible, whatever the point distribution.  Integer addition is associative, so the
-// rasterised field is bit-identical from run to run (the float atomics were not).  Error: <= quantum / 2 per
-// contribution, quantum <= bound / 2^29 (for 650 unit normals on a plane: 1.2e-6, about 10 fp32 ulps of 1; the
-// tolerance of the path is 1e-4 max|chi|).
-struct FixScale { float S, invS; };
-SAP_HD FixScale fix_scale(float bound) {
-    FixScale f;
-    if (!(bound > 0.f) || !(bound < 3.0e38f)) { f.S = 1.f; f.invS = 1.f; return f; }
-    int e;
-    (void)frexpf(bound, &e);          // bound = m 2^e, m in [0.5, 1)  =>  bound < 2^e
-    int k = 30 - e;                   // S = 2^k: bound S < 2^30
-    if (k > 120) k = 120;
-    if (k < -120) k = -120;
-    f.S = ldexpf(1.f, k);
-    f.invS = ldexpf(1.f, -k);
-    return f;
-}
-SAP_HD int fix_round(float v) {
-#ifdef __CUDA_ARCH__
-    return __float2int_rn(v);
-#else
-    return (int)lrintf(v);
-#endif
-}
 // index of (line l, z slot pz) in a dense plane (column swizzle of the HBM layout, see kz_swz)
 template <int H> SAP_HD int dzi(int l, int pz) { return l * H + (pz ^ (l & 15)); }
 
@@ -650,6 +621,7 @@ SAP_HD void fwd_x_solve(Ctx& ctx, const FusedParams& p, const FusedSmem<N>& sm, 
         const int blk = t / W, c = t - blk * W, e0 = blk * RL * W + c;
         float4 ey, ez;
         xt.col_freq(p.ftab, c, ey, ez);
+        const MultCol mc = mult_col(ey, ez, p.cs);
         float2 v[RL], a[RL];
 #pragma unroll
         for (int r = 0; r < RL; ++r) v[r] = b0[e0 + r * W];
@@ -661,7 +633,7 @@ SAP_HD void fwd_x_solve(Ctx& ctx, const FusedParams& p, const FusedSmem<N>& sm, 
         dft_fwd<RL>(v);
 #pragma unroll
         for (int r = 0; r < RL; ++r) {
-            const float f = mult_f(sm.fx[blk * RL + r], ey, ez, p.cs);
+            const float f = mult_fc(sm.fx[blk * RL + r], mc);
             const float2 dv = cscale(f, cadd(a[r], v[r]));
             a[r] = make_float2(-dv.y, dv.x);  // chi~ = i (div)
         }
@@ -888,13 +860,14 @@ SAP_HD void bwd_x_adj(Ctx& ctx, const FusedParams& p, const FusedSmem<N>& sm, fl
         const int blk = t / W, c = t - blk * W, e0 = blk * RL * W + c;
         float4 ey, ez;
         xt.col_freq(p.ftab, c, ey, ez);
+        const MultCol mc = mult_col(ey, ez, p.cs);
         float2 v[RL], a[RL];
 #pragma unroll
         for (int r = 0; r < RL; ++r) v[r] = b0[e0 + r * W];
         dft_fwd<RL>(v);
 #pragma unroll
         for (int r = 0; r < RL; ++r) {
-            const float f = mult_f(sm.fx[blk * RL + r], ey, ez, p.cs);
+            const float f = mult_fc(sm.fx[blk * RL + r], mc);
             a[r] = make_float2(f * v[r].y, -f * v[r].x);          // A = -i f Gbar'~
             v[r] = cscale(sm.fx[blk * RL + r].x, a[r]);            // h_x A
         }

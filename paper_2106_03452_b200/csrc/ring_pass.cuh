@@ -463,6 +463,7 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
             // first inverse stage happen on the registers of the last forward stage (same slots, no barrier).
             float4 ey, ez;
             col_freq(tid % W, ey, ez);  // NTC % W == 0: every task of this thread is in column tid % W
+            const MultCol mc = mult_col(ey, ez, p.cs);
             float2 acc[TPT][RL];
             (void)acc;
             constexpr bool SIDE = NSTAGE >= 2 * 3;  // the ring can hold whole tiles and still prefetch
@@ -521,7 +522,7 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
                 dft_fwd<RL>(v);
 #pragma unroll
                 for (int r = 0; r < RL; ++r) {
-                    const float f = mult_f(fx[blk * RL + r], ey, ez, p.cs);
+                    const float f = mult_fc(fx[blk * RL + r], mc);
                     const float2 dv = cscale(f, cadd(a[r], v[r]));
                     a[r] = make_float2(-dv.y, dv.x);  // chi~ = i (div)
                 }
@@ -542,6 +543,7 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
             // x transform B of A, so a tile needs two inverse x transforms, not three, and writes two spectra.
             float4 ey, ez;
             col_freq(tid % W, ey, ez);
+            const MultCol mc = mult_col(ey, ez, p.cs);
             float2* buf = acquire(it);
             ring_stage<N, 0, W, NTC, false>(buf, tabF, tid);
             consumer_sync<NTC>(group);
@@ -559,7 +561,7 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
                 dft_fwd<RL>(v);
 #pragma unroll
                 for (int r = 0; r < RL; ++r) {
-                    const float f = mult_f(fx[blk * RL + r], ey, ez, p.cs);
+                    const float f = mult_fc(fx[blk * RL + r], mc);
                     acc[i][r] = make_float2(f * v[r].y, -f * v[r].x);
                 }
             }

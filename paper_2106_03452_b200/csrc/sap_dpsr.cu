@@ -20,6 +20,7 @@ struct DevCtx {
     int tid, nthr;
     __device__ __forceinline__ void sync() const { __syncthreads(); }
     __device__ __forceinline__ void atomic_add(float* p, float v) const { atomicAdd(p, v); }
+    __device__ __forceinline__ void atomic_add(int* p, int v) const { atomicAdd(p, v); }
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -29,7 +30,7 @@ struct DevCtx {
 template <int N> constexpr int zy_min_blocks() { return (N == 128 || N == 512) ? 3 : 4; }
 template <int N, int NL, bool DO_Y, int SRC, int NT>
 __global__ void __launch_bounds__(NT, zy_min_blocks<N>()) k_zy_fwd(ZyFwdParams p) {
-    extern __shared__ float2 smem[];
+    extern __shared__ __align__(16) float2 smem[];
     DevCtx ctx{(int)threadIdx.x, NT};
     pdl_wait();
     zy_fwd_body<N, NL, DO_Y, SRC>(ctx, p, smem, (int)blockIdx.x, (int)blockIdx.y);
@@ -75,8 +76,10 @@ __global__ void k_bin_count(const float* __restrict__ pts, int P, int N, int NL,
     atomicAdd(cnt + (size_t)b * nbins + bin_key(pts + ((size_t)b * P + i) * 3, N, NL), 1);
 }
 // one block per item: exclusive scan of the counts -> start[nbins+1]; cursor = start; counts reset to 0
-__global__ void k_bin_scan(int* __restrict__ cnt, int nbins, int P, int* __restrict__ start, int* __restrict__ cursor) {
+__global__ void k_bin_scan(int* __restrict__ cnt, int nbins, int P, int* __restrict__ start, int* __restrict__ cursor,
+                           unsigned* __restrict__ nmax) {
     pdl_wait();
+    if (threadIdx.x == 0) nmax[blockIdx.x] = 0u;   // k_bin_scatter (the next launch) takes the max of |n| into it
     __shared__ int wsum[32];
     const int b = blockIdx.x, tid = threadIdx.x, nt = blockDim.x;
     int* c = cnt + (size_t)b * nbins;
@@ -116,15 +119,20 @@ __global__ void k_bin_scan(int* __restrict__ cnt, int nbins, int P, int* __restr
 }
 __global__ void k_bin_scatter(const float* __restrict__ pts, const float* __restrict__ nrm, int P, int N, int NL,
                               int nbins, int* __restrict__ cursor, float4* __restrict__ spts,
-                              float4* __restrict__ snrm) {
+                              float4* __restrict__ snrm, unsigned* __restrict__ nmax) {
     pdl_wait();
     const int i = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y;
-    if (i >= P) return;
-    const float* c = pts + ((size_t)b * P + i) * 3;
-    const float* n = nrm + ((size_t)b * P + i) * 3;
-    const int pos = atomicAdd(cursor + (size_t)b * nbins + bin_key(c, N, NL), 1);
-    spts[(size_t)b * P + pos] = make_float4(c[0], c[1], c[2], __int_as_float(i));  // .w: index in the caller's order
-    snrm[(size_t)b * P + pos] = make_float4(n[0], n[1], n[2], 0.f);
+    unsigned amax = 0u;   // bit pattern of max_c |n_c| (non-negative floats order like their bits): scale of the fixed-point splat
+    if (i < P) {
+        const float* c = pts + ((size_t)b * P + i) * 3;
+        const float* n = nrm + ((size_t)b * P + i) * 3;
+        const int pos = atomicAdd(cursor + (size_t)b * nbins + bin_key(c, N, NL), 1);
+        spts[(size_t)b * P + pos] = make_float4(c[0], c[1], c[2], __int_as_float(i));  // .w: index in the caller's order
+        snrm[(size_t)b * P + pos] = make_float4(n[0], n[1], n[2], 0.f);
+        amax = __float_as_uint(fmaxf(fmaxf(fabsf(n[0]), fabsf(n[1])), fabsf(n[2])));
+    }
+    amax = __reduce_max_sync(0xffffffffu, amax);
+    if ((threadIdx.x & 31) == 0 && amax) atomicMax(nmax + b, amax);
 }
 
 __device__ __forceinline__ float warp_sum(float x) {
@@ -382,6 +390,7 @@ struct sap_dpsr {
     unsigned* ticket = nullptr;  // [B][2]
     float* stats = nullptr;    // [B][4] {mu, a, s, -}
     float* bw = nullptr;       // [B][4] {s, beta/P, S1/a, beta/(P s)}
+    unsigned* nmax = nullptr;  // [B] bit pattern of the largest |normal component| of the item (fixed-point scale of the splat)
     // staging for the *_host entry points (allocated on first use)
     float *h_pts = nullptr, *h_nrm = nullptr, *h_chi = nullptr, *h_gchi = nullptr, *h_gp = nullptr, *h_gn = nullptr;
     int host_P = 0;
@@ -649,15 +658,15 @@ template <int N> struct Runner {
             const dim3 gp((P + 255) / 256, B);
             launch_pdl(k_bin_count, dim3(gp), dim3(256), 0, st, pts, P, N, C::NL, h->nbins, h->bin_cnt);
             SAP_LAUNCH_CHECK(h, "k_bin_count");
-            launch_pdl(k_bin_scan, dim3(B), dim3(1024), 0, st, h->bin_cnt, h->nbins, P, h->bin_start, h->bin_cursor);
+            launch_pdl(k_bin_scan, dim3(B), dim3(1024), 0, st, h->bin_cnt, h->nbins, P, h->bin_start, h->bin_cursor, h->nmax);
             SAP_LAUNCH_CHECK(h, "k_bin_scan");
-            launch_pdl(k_bin_scatter, dim3(gp), dim3(256), 0, st, pts, nrm, P, N, C::NL, h->nbins, h->bin_cursor, h->spts, h->snrm);
+            launch_pdl(k_bin_scatter, dim3(gp), dim3(256), 0, st, pts, nrm, P, N, C::NL, h->nbins, h->bin_cursor, h->spts, h->snrm, h->nmax);
             SAP_LAUNCH_CHECK(h, "k_bin_scatter");
             h->binned_P = P;
         }
         // F2 z (+y) forward, 3 channels
         {
-            ZyFwdParams p{h->spts, h->snrm, h->bin_start, P, nullptr, nullptr, h->S3, C::FUSED_ZY ? h->Q3 : h->QT3, h->tw, 3};
+            ZyFwdParams p{h->spts, h->snrm, h->bin_start, P, nullptr, nullptr, h->S3, C::FUSED_ZY ? h->Q3 : h->QT3, h->tw, 3, h->nmax};
             launch_pdl(k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_SPLAT, C::NT_ZY>, dim3(N * N / C::NL, B * 3), dim3(C::NT_ZY), zy_smem_bytes<N, C::NL>(), st, p);
             SAP_LAUNCH_CHECK(h, "k_zy_fwd");
         }
@@ -719,7 +728,7 @@ template <int N> struct Runner {
         }
         // B2 + B3: Gbar' assembled on load, z (+y) forward
         {
-            ZyFwdParams p{h->spts, h->snrm, h->bin_start, P, gchi, h->bw, h->S1, C::FUSED_ZY ? h->Q1 : h->QT1, h->tw, 1};
+            ZyFwdParams p{h->spts, h->snrm, h->bin_start, P, gchi, h->bw, h->S1, C::FUSED_ZY ? h->Q1 : h->QT1, h->tw, 1, h->nmax};
             if constexpr (C::FUSED_ZY) launch_zl_gbar(h, st, p, B);
             else launch_pdl(k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_GBAR, C::NT_ZY>, dim3(N * N / C::NL, B), dim3(C::NT_ZY), zy_smem_bytes<N, C::NL>(), st, p);
             SAP_LAUNCH_CHECK(h, C::FUSED_ZY ? "k_zl_gbar" : "k_zy_fwd<GBAR>");
@@ -771,7 +780,7 @@ static void free_all(sap_dpsr* h) {
     for (int i = 0; i < sap_dpsr::MAX_EV; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
     cudaFree(h->v); cudaFree(h->spts); cudaFree(h->snrm); cudaFree(h->bin_cnt); cudaFree(h->bin_cursor); cudaFree(h->bin_start); cudaFree(h->S3); cudaFree(h->Q3); cudaFree(h->S1); cudaFree(h->Q1); cudaFree(h->QT3); cudaFree(h->QT1); cudaFree(h->tw); cudaFree(h->ftab);
     cudaFree(h->fhist); cudaFree(h->facc); cudaFree(h->fsync); cudaFree(h->fstamps);
-    cudaFree(h->gmse); cudaFree(h->acc_mse); cudaFree(h->acc); cudaFree(h->ticket); cudaFree(h->stats); cudaFree(h->bw);
+    cudaFree(h->gmse); cudaFree(h->acc_mse); cudaFree(h->acc); cudaFree(h->ticket); cudaFree(h->stats); cudaFree(h->bw); cudaFree(h->nmax);
     cudaFree(h->h_pts); cudaFree(h->h_nrm); cudaFree(h->h_chi); cudaFree(h->h_gchi); cudaFree(h->h_gp); cudaFree(h->h_gn);
 }
 
@@ -812,6 +821,7 @@ extern "C" sap_status_t sap_dpsr_create(int N, float sigma, int batch, int max_p
     upd(dev_alloc(h, &h->ticket, B * 2));
     upd(dev_alloc(h, &h->stats, B * 4));
     upd(dev_alloc(h, &h->bw, B * 4));
+    upd(dev_alloc(h, &h->nmax, B));
     h->fused_ok = (N <= 128) && ((long long)batch * N <= h->num_sms) && batch <= (N == 32 ? 4 : N == 64 ? 2 : 1);
     if (h->fused_ok) {
         upd(dev_alloc(h, &h->fhist, B * (size_t)h->num_sms * N));
@@ -839,6 +849,7 @@ extern "C" sap_status_t sap_dpsr_create(int N, float sigma, int batch, int max_p
     upd(cudaMemset(h->ticket, 0, sizeof(unsigned) * B * 2));
     upd(cudaMemset(h->stats, 0, sizeof(float) * B * 4));
     upd(cudaMemset(h->bw, 0, sizeof(float) * B * 4));
+    upd(cudaMemset(h->nmax, 0, sizeof(unsigned) * B));
     if (h->fused_ok) {
         upd(cudaMemset(h->facc, 0, sizeof(double) * B * 2));
         upd(cudaMemset(h->fsync, 0, sizeof(unsigned) * 4));

@@ -25,17 +25,32 @@ template <int N> SAP_HD float4 freq_entry_z(int slot, float cg) {
     const int k = (slot == H) ? H : pos2freq<H>(slot);
     return make_float4((k == H) ? 0.f : (float)k, (float)(k * k), expf(-cg * (float)(k * k)), 0.f);
 }
+// 1 / x for x = |u|^2, an exact integer >= 1: the approximate reciprocal (one MUFU, 1 ulp) -- __frcp_rn brings a
+// Newton step and a denormal slow path whose branches cost 8% of the solve kernel's instructions
 SAP_HD float fast_rcp(float x) {
 #ifdef __CUDA_ARCH__
-    return __frcp_rn(x);
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
 #else
     return 1.f / x;
 #endif
 }
-// f = cs g / q from three table entries (0 at DC)
+// f = cs g / q from three table entries (0 at DC); branch-free
 SAP_HD float mult_f(const float4& ex, const float4& ey, const float4& ez, float cs) {
     const float q = ex.y + ey.y + ez.y;
-    return (q == 0.f) ? 0.f : cs * (ex.z * ey.z) * ez.z * fast_rcp(q);
+    const float f = cs * (ex.z * ey.z) * ez.z * fast_rcp(q);
+    return (q > 0.f) ? f : 0.f;
+}
+// the same with the column part (y and z slots: fixed for all butterflies of a thread) folded once per tile
+struct MultCol {
+    float qyz, gyz;   // |u_y|^2 + |u_z|^2,  cs g_y g_z
+};
+SAP_HD MultCol mult_col(const float4& ey, const float4& ez, float cs) { return MultCol{ey.y + ez.y, cs * ey.z * ez.z}; }
+SAP_HD float mult_fc(const float4& ex, const MultCol& c) {
+    const float q = ex.y + c.qyz;
+    const float f = c.gyz * ex.z * fast_rcp(q);
+    return (q > 0.f) ? f : 0.f;
 }
 
 // MODE_FWD3 / MODE_INV3: the y pass of the three field channels when it is a kernel of its own (N >= 256).  The y and z

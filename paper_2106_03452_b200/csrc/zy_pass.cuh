@@ -8,6 +8,7 @@
 // global.
 // smem: (H+1) rows (kz slots + Nyquist) x PITCH = NL+1 columns (lines); PITCH == 1 (mod 16).
 #pragma once
+#include <math.h>
 #include "fft_core.cuh"
 
 namespace sap {
@@ -29,6 +30,7 @@ struct ZyFwdParams {
     float2* Q;             // [planes][N*N]  ([x][y] when the plane is fused (N <= 128), transposed [y][x] otherwise)
     const float2* tw;      // exp(-2 pi i t / N), t < N
     int nch;               // planes per batch item (3 for SPLAT, 1 for GBAR)
+    const unsigned* nmax;  // SPLAT: [batch] bit pattern of max_i max_c |n_ic| (k_bin_scatter), for the fixed-point scale
 };
 
 // Column swizzle of the main spectrum in HBM: the value of z slot pz of line (x, y) is stored in column
@@ -37,6 +39,42 @@ struct ZyFwdParams {
 // conflicts.  An involution: the same function maps a stored column back to its slot.
 SAP_HD int kz_swz(int pz, int y) { return pz ^ (y & 15); }
 
+// ---- fixed-point rasterisation ---------------------------------------------------------------------------------------
+// The trilinear splat accumulates into shared memory with NATIVE 32-bit integer atomics (a float atomicAdd on shared
+// memory is a compare-and-swap loop, measured at ~400 cycles per add here: 12 of them per point were the straggler
+// of the whole forward).  Each contribution w * n_c is rounded once to a multiple of the quantum 1/S; S is a power of
+// two chosen per tile from bound = sum over the tile's points of max_c |n_ic|  >=  |any cell sum|, so that
+// bound * S < 2^30: overflow is impossible, whatever the point distribution.  Integer addition is associative, so the
+// rasterised field is bit-identical from run to run (the float atomics were not).  Error: <= quantum / 2 per
+// contribution, quantum <= bound / 2^29 (for 650 unit normals on a plane: 1.2e-6, about 10 fp32 ulps of 1; the
+// tolerance of the path is 1e-4 max|chi|).
+SAP_HD float bits_u2f(unsigned u) {
+#ifdef __CUDA_ARCH__
+    return __uint_as_float(u);
+#else
+    union { unsigned u; float f; } v; v.u = u; return v.f;
+#endif
+}
+struct FixScale { float S, invS; };
+SAP_HD FixScale fix_scale(float bound) {
+    FixScale f;
+    if (!(bound > 0.f) || !(bound < 3.0e38f)) { f.S = 1.f; f.invS = 1.f; return f; }
+    int e;
+    (void)frexpf(bound, &e);          // bound = m 2^e, m in [0.5, 1)  =>  bound < 2^e
+    int k = 30 - e;                   // S = 2^k: bound S < 2^30
+    if (k > 120) k = 120;
+    if (k < -120) k = -120;
+    f.S = ldexpf(1.f, k);
+    f.invS = ldexpf(1.f, -k);
+    return f;
+}
+SAP_HD int fix_round(float v) {
+#ifdef __CUDA_ARCH__
+    return __float2int_rn(v);
+#else
+    return (int)lrintf(v);
+#endif
+}
 template <int N, int NL> constexpr size_t zy_smem_bytes() { return ((size_t)(N / 2 + 1) * (NL + 1) + N) * sizeof(float2); }
 
 // task t -> (line, q) for the global<->smem z stage: q (ST0 consecutive complex of one line) fastest,
@@ -80,12 +118,9 @@ SAP_HD void zy_fwd_body(Ctx& ctx, const ZyFwdParams& p, float2* smem, int bx, in
         b_n[k] = use ? bs[bin + 1] - b_lo[k] : 0;
         total += b_n[k];
     }
-    // A1: zero the plane, rasterise the points into it (shared-memory atomics), z = 2m + parity
-    // (the bin offsets above are in flight while the twiddles are fetched and the plane is cleared)
-    for (int i = ctx.tid; i < N; i += ctx.nthr) tw[i] = p.tw[i];
-    for (int i = ctx.tid; i < H * PITCH; i += ctx.nthr) s[i] = make_float2(0.f, 0.f);
-    if (SRC == SRC_SPLAT && total == 0) {  // nothing lands here: the spectrum of zeros is zeros
-        for (int i = ctx.tid; i < NL * H; i += ctx.nthr) So[i] = make_float2(0.f, 0.f);
+    if (SRC == SRC_SPLAT && total == 0) {  // nothing lands here: the spectrum of zeros is zeros (before any other work)
+        float4* So4 = reinterpret_cast<float4*>(So);
+        for (int i = ctx.tid; i < NL * H / 2; i += ctx.nthr) So4[i] = make_float4(0.f, 0.f, 0.f, 0.f);
         if constexpr (DO_Y) {
             for (int l = ctx.tid; l < NL; l += ctx.nthr) Qo[l] = make_float2(0.f, 0.f);
         } else {
@@ -94,19 +129,29 @@ SAP_HD void zy_fwd_body(Ctx& ctx, const ZyFwdParams& p, float2* smem, int bx, in
         }
         return;
     }
+    // A1: zero the plane, rasterise the points into it, z = 2m + parity.  The plane holds 32-bit FIXED-POINT sums while it
+    // is rasterised (native integer shared-memory atomics; a float atomicAdd on shared memory is a compare-and-swap loop):
+    // scale 2^k with (number of points that can touch the tile) x (largest normal component of the item) x 2^k < 2^30.
+    for (int i = ctx.tid; i < N; i += ctx.nthr) tw[i] = p.tw[i];
+    {
+        float4* s4 = reinterpret_cast<float4*>(s);
+        for (int i = ctx.tid; i < (H * PITCH + 1) / 2; i += ctx.nthr) s4[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+    const float amax = (SRC == SRC_SPLAT) ? bits_u2f(p.nmax[item]) : 1.f;
+    const FixScale fs = fix_scale((float)total * amax);
     ctx.sync();
     {
-        float* sf = reinterpret_cast<float*>(s);
+        int* si = reinterpret_cast<int*>(s);
         const float4* sp = p.spts + (size_t)item * p.P;
         const float4* sn = p.snrm + (size_t)item * p.P;
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
             for (int i = b_lo[k] + ctx.tid; i < b_lo[k] + b_n[k]; i += ctx.nthr) {
                 const float4 c = sp[i];
-                float val = 1.f;
+                float val = fs.S;
                 if (SRC == SRC_SPLAT) {
                     const float4 n = sn[i];
-                    val = (ch == 0) ? n.x : (ch == 1) ? n.y : n.z;
+                    val *= (ch == 0) ? n.x : (ch == 1) ? n.y : n.z;
                 }
                 const float tx = c.x * (float)N, tyf = c.y * (float)N, tz = c.z * (float)N;
                 const float fx0 = floorf(tx), fy0 = floorf(tyf), fz0 = floorf(tz);
@@ -124,7 +169,7 @@ SAP_HD void zy_fwd_body(Ctx& ctx, const ZyFwdParams& p, float2* smem, int bx, in
 #pragma unroll
                         for (int dz = 0; dz < 2; ++dz) {
                             const int z = (jz + dz) & M;
-                            ctx.atomic_add(sf + ((z >> 1) * PITCH + ly) * 2 + (z & 1), wxy * (dz ? fz : 1.f - fz));
+                            ctx.atomic_add(si + ((z >> 1) * PITCH + ly) * 2 + (z & 1), fix_round(wxy * (dz ? fz : 1.f - fz)));
                         }
                     }
                 }
@@ -146,7 +191,8 @@ SAP_HD void zy_fwd_body(Ctx& ctx, const ZyFwdParams& p, float2* smem, int bx, in
             float2 v[R0];
 #pragma unroll
             for (int r = 0; r < R0; ++r) {
-                float2 xv = s[(q + ST0 * r) * PITCH + l];
+                const int2 iv = reinterpret_cast<const int2*>(s)[(q + ST0 * r) * PITCH + l];   // fixed-point sums
+                float2 xv = make_float2(fs.invS * (float)iv.x, fs.invS * (float)iv.y);
                 if (SRC == SRC_GBAR) {
                     const int e = l * H + q + ST0 * r;
                     const float2 g = g2[e];
@@ -165,7 +211,7 @@ SAP_HD void zy_fwd_body(Ctx& ctx, const ZyFwdParams& p, float2* smem, int bx, in
     static_assert(Plan<H>::NS <= 2, "z plans have at most two stages");
     // (the fused variant holds a block pair = 2 R1 complex values per thread: worth it where the kernel has the
     // registers, i.e. at 3 CTAs per SM (N = 512); at N = 256 the kernel runs 4 CTAs per SM on 64 registers)
-    constexpr bool FUSE_SPLIT = !DO_Y && N >= 512;
+    constexpr bool FUSE_SPLIT = !DO_Y && N >= 512;   // at 256 it spills at 4 CTAs/SM and is no faster at 3 (r2: 67.6 vs 66.0 us)
     if constexpr (Plan<H>::NS > 1 && !FUSE_SPLIT) {
         fft_stage<H, 1, false, N, true>(s, PITCH, 1, NL, tw, ctx.tid, ctx.nthr);
         ctx.sync();
@@ -223,10 +269,12 @@ SAP_HD void zy_fwd_body(Ctx& ctx, const ZyFwdParams& p, float2* smem, int bx, in
         ctx.sync();
     }
     if constexpr (!DO_Y) {
-        // copy out (slot-major rows are contiguous in HBM)
-        for (int i = ctx.tid; i < NL * H; i += ctx.nthr) {
-            const int l = i / H, pc = i - l * H;
-            So[i] = s[kz_swz(pc, y0 + l) * PITCH + l];
+        // copy out (slot-major rows are contiguous in HBM), two columns = 16 bytes per store
+        float4* So4 = reinterpret_cast<float4*>(So);
+        for (int i = ctx.tid; i < NL * H / 2; i += ctx.nthr) {
+            const int l = i / (H / 2), pc = 2 * (i - l * (H / 2));
+            const float2 a = s[kz_swz(pc, y0 + l) * PITCH + l], b = s[kz_swz(pc + 1, y0 + l) * PITCH + l];
+            So4[i] = make_float4(a.x, a.y, b.x, b.y);
         }
         // Nyquist plane: written transposed ([y][x]) so that the y pass can fetch it with TMA tiles
         float2* Qt = p.Q + (size_t)by * ((size_t)N * N);
