@@ -8,7 +8,7 @@ import ctypes
 from .binding import SAP_OK, SapError, _stream_ptr, lib as _dpsr_lib
 
 EXPORTS = ["sap_mesh_create", "sap_mc_extract", "sap_mc_backward", "sap_chamfer", "sap_mc_table", "sap_mesh_destroy",
-           "sap_mesh_last_error", "sap_mesh_workspace_bytes", "sap_mesh_last_launch_count", "sap_points_sgd_step"]
+           "sap_mesh_last_error", "sap_mesh_workspace_bytes", "sap_mesh_last_launch_count", "sap_points_sgd_step", "sap_chamfer_set_search"]
 MC_MAX_TRI = 12
 _ready = False
 
@@ -30,6 +30,8 @@ def lib():
         L.sap_mc_table.restype = ci
         L.sap_points_sgd_step.argtypes = [vp, vp, vp, vp, ci, ci, ctypes.c_float, vp, vp]
         L.sap_points_sgd_step.restype = ci
+        L.sap_chamfer_set_search.argtypes = [vp, ci]
+        L.sap_chamfer_set_search.restype = ci
         L.sap_mesh_destroy.argtypes = [vp]
         L.sap_mesh_destroy.restype = None
         L.sap_mesh_last_error.argtypes = [vp]
@@ -130,6 +132,10 @@ class Mesh:
             null if nn_a is None else ctypes.c_void_p(nn_a.data_ptr()),
             null if nn_b is None else ctypes.c_void_p(nn_b.data_ptr()), _stream_ptr(stream)))
         return loss, grad_a, nn_a, nn_b
+
+    def set_search(self, mode):
+        """'auto' | 'brute' | 'grid': nearest-neighbour search of chamfer (include/sap_mesh.h, SAP_NN_*)."""
+        self._check(lib().sap_chamfer_set_search(self._h, {"auto": 0, "brute": 1, "grid": 2}[mode]))
 
     @property
     def workspace_bytes(self):

@@ -95,8 +95,9 @@ def test_eq6_backward_matches_the_oracle():
     h.close()
 
 
+@pytest.mark.parametrize("search", ["brute", "grid"])
 @pytest.mark.parametrize("na,nb", [(5000, 3000), (1, 1), (37, 4000), (20000, 20000)])
-def test_chamfer_matches_brute_force(na, nb):
+def test_chamfer_matches_brute_force(na, nb, search):
     import torch
     from paper_2106_03452_b200.mesh import Mesh
     rng = np.random.default_rng(na + nb)
@@ -108,6 +109,7 @@ def test_chamfer_matches_brute_force(na, nb):
         b = rng.uniform(0, 1, (nb, 3)).astype(np.float32)
     ref = mo.chamfer(a, b)
     h = Mesh(8, 8, 8, max(na, nb))
+    h.set_search(search)
     loss, ga, nn_a, nn_b = h.chamfer(torch.from_numpy(a).cuda(), torch.from_numpy(b).cuda(), want_nn=True)
     torch.cuda.synchronize()
     assert abs(loss.item() - ref["loss"]) <= 1e-5 * ref["loss"]
