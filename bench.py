@@ -37,7 +37,7 @@ UNIT = "ms/grid"
 YARD_FWD_BWD_V = 52.0
 KERNEL_BYTES_V = {
     # label: (compulsory V for N <= 128 (y fused with z), compulsory V for N >= 256)
-    "F:k_bin_count": (0.0, 0.0), "F:k_bin_scan": (0.0, 0.0), "F:k_bin_scatter": (0.0, 0.0),   # 72 B/point, no grid traffic
+    "F:k_bin_sort": (0.0, 0.0), "F:k_bin_count": (0.0, 0.0), "F:k_bin_scan": (0.0, 0.0), "F:k_bin_scatter": (0.0, 0.0),   # 72 B/point, no grid traffic
     "F:k_zy_fwd": (3.0, 3.0),            # writes 3 spectra; the splatted field never exists in HBM
     "F:k_ring<FWD,y>": (0.0, 5.0),       # N >= 256 only: reads 3 spectra, writes 2 (x, u = h_y y + h_z z)
     "F:k_ring<SOLVE>": (4.0, 3.0),       # reads 3 (2) spectra, writes 1

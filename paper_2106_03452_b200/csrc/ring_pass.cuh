@@ -43,7 +43,8 @@ template <int N> constexpr int ring_tw_entries() {
 template <int N, int MODE> constexpr size_t ring_smem_bytes() {
     using C = RingCfgM<N, MODE>;
     return (size_t)C::NSTAGE * N * C::W * sizeof(float2) + 2 * (size_t)ring_tw_entries<N>() * sizeof(float4) +
-           (size_t)N * sizeof(float4) + 3 * C::NSTAGE * sizeof(uint64_t) + 128;
+           (size_t)N * sizeof(float4) + 3 * C::NSTAGE * sizeof(uint64_t) + 128 +
+           (size_t)ring_threads<N, MODE>() * sizeof(int);   // tile ids of this CTA (listed mode)
 }
 constexpr size_t SMEM_PER_CTA_MAX = 227 * 1024;  // sm_100a opt-in limit per CTA
 static_assert(ring_smem_bytes<32, MODE_SOLVE>() * 4 <= SMEM_PER_CTA_MAX + 4096 && ring_smem_bytes<64, MODE_SOLVE>() * 3 <= SMEM_PER_CTA_MAX &&
@@ -61,6 +62,11 @@ struct RingParams {
     int units;           // planes (FWD / INV) or batch items (SOLVE / ADJ)
     int nyq_out_t;       // x pass: Nyquist-plane output is written transposed ([y][x]); the y pass always reads [y][x], writes [x][y]
     float cs;
+    // listed mode of the 3-channel y passes (MODE_FWD3 / MODE_INV3; see ActLists in sap_dpsr.cu), nullptr = every tile:
+    const int* ylist;    // global tile ids (unit * tiles_per_unit + T) of the tiles of the active planes + all Nyquist tiles.
+                         // MODE_FWD3 runs in place: the rows of an inactive plane in the output planes 0 and 1 are the zeros
+                         // the splat pass wrote there; MODE_INV3's output there is never read
+    const int* nact;     // {-, |ylist|, -, -}
 };
 
 // ---- PTX wrappers ---------------------------------------------------------------------------------------
@@ -267,6 +273,9 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
     uint64_t* full = reinterpret_cast<uint64_t*>(fx + N);
     uint64_t* empty = full + NSTAGE;
     volatile int* issued = reinterpret_cast<volatile int*>(empty + NSTAGE);  // fills issued into each buffer so far
+    int* tcache = const_cast<int*>(reinterpret_cast<volatile int*>(issued + NSTAGE + (NSTAGE & 1)));  // listed mode: this CTA's tile ids
+    constexpr int TCAP = ring_threads<N, MODE>();
+    constexpr bool CAN_LIST = (MODE == MODE_FWD3 || MODE == MODE_INV3);
     const int group = threadIdx.x / NTC, tid = threadIdx.x - group * NTC;
 
     for (int i = threadIdx.x; i < TWE; i += ring_threads<N, MODE>()) {
@@ -284,15 +293,28 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
     }
     __syncthreads();
     pdl_wait();  // the tables above are constants of the handle; the spectra below are the predecessor's output
-    const long long total = (long long)p.units * tiles_per_unit;
+    const bool listed = CAN_LIST && p.ylist != nullptr;
+    const long long total = listed ? (long long)p.nact[1] : (long long)p.units * tiles_per_unit;
+    if (CAN_LIST && listed) {
+        const long long idx = (long long)blockIdx.x + (long long)threadIdx.x * gridDim.x;
+        tcache[threadIdx.x] = idx < total ? p.ylist[idx] : -1;
+        __syncthreads();
+    }
+    // j-th tile of this CTA (global tile id), -1 past the end
+    auto tile_at = [&](int j) -> long long {
+        const long long idx = (long long)blockIdx.x + (long long)j * gridDim.x;
+        if (idx >= total) return -1;
+        if (CAN_LIST && listed) return j < TCAP ? (long long)tcache[j] : (long long)p.ylist[idx];
+        return idx;
+    };
 
     // One item = one (tile, input channel) = one ring buffer fill.  Item `it` of this CTA lives in buffer it % NSTAGE;
     // the thread that sees the last consumer warp release item `it` immediately refills the buffer with item
     // it + NSTAGE, so there is no producer warp (a 17th warp would cost every thread 1/5 of its registers).
     auto issue_load = [&](int it) {
         const int j = it / IT_PER_TILE, ch = it - j * IT_PER_TILE;
-        const long long g = (long long)blockIdx.x + (long long)j * gridDim.x;
-        if (g >= total) return;
+        const long long g = tile_at(j);
+        if (g < 0) return;
         const int unit = (int)(g / tiles_per_unit), T = (int)(g - (long long)unit * tiles_per_unit);
         const int s = it % NSTAGE;
         mbar_expect_tx(full + s, TILE_BYTES);
@@ -337,9 +359,11 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
 #pragma unroll 1
         for (int it = 0; it < NSTAGE; ++it) issue_load(it);
     }
-
     // ---------------- per-tile work of a consumer group ----------------
-    for (int j = group, g = blockIdx.x + group * gridDim.x; g < total; j += NG, g += NG * gridDim.x) {
+    for (int j = group;; j += NG) {
+        const long long gl = tile_at(j);
+        if (gl < 0) break;
+        const int g = (int)gl;
         const int it = j * IT_PER_TILE;  // ring position of this tile's first item
         const int unit = g / tiles_per_unit, T = g - unit * tiles_per_unit;
         TileDesc d = tile_desc<N, W>(AXIS, T);

@@ -69,13 +69,113 @@ __device__ __forceinline__ int bin_key(const float* __restrict__ c, int N, int N
     const int jx = (int)floorf(c[0] * (float)N) & M, jy = (int)floorf(c[1] * (float)N) & M;
     return jx * (N / NL) + jy / NL;
 }
-__global__ void k_bin_count(const float* __restrict__ pts, int P, int N, int NL, int nbins, int* __restrict__ cnt) {
+__global__ void k_bin_count(const float* __restrict__ pts, int P, int N, int NL, int nbins, int* __restrict__ cnt,
+                            int* __restrict__ nact) {
     pdl_wait();
     const int i = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y;
+    if (i == 0 && b == 0) { nact[0] = 0; nact[1] = 0; nact[2] = 0; nact[3] = 0; }  // lengths of the active-tile lists (k_bin_scan appends)
     if (i >= P) return;
     atomicAdd(cnt + (size_t)b * nbins + bin_key(pts + ((size_t)b * P + i) * 3, N, NL), 1);
 }
 // one block per item: exclusive scan of the counts -> start[nbins+1]; cursor = start; counts reset to 0
+// Activity lists ("nobody computes what nobody reads").  A tile (x, ty) = the NL z-lines y in [ty NL, (ty+1) NL) of plane x is
+// ACTIVE when a point can touch it: one of the bins (x, ty), (x-1, ty), (x, ty-1), (x-1, ty-1) is non-empty -- the test the
+// splat pass uses for its own tile.  A plane is active when one of its tiles is.  The splatted field is identically zero
+// on inactive tiles and the gather (B6) never reads vbar there, so
+//   - the forward y pass (N >= 256) neither loads nor transforms inactive planes (it writes their zeros),
+//   - the inverse y pass of the adjoint skips inactive planes and the inverse z pass of the adjoint inactive tiles.
+// zlist: ids item * nbins + bin of the active tiles; ylist: global tile ids of the y-pass tiles of the active planes and of
+// all Nyquist-plane tiles; nact = {|zlist|, |ylist|, number of active planes, -} (reset by the binning kernel).  Items append their segments with one atomicAdd each: the order of the items in the lists is arbitrary,
+// the results do not depend on it (tiles are independent).
+struct ActLists {
+    int* plane_act;   // [B][N] 1 = active
+    int* zlist;       // [B * nbins]
+    int* ylist;       // [B * (N * KT + NYQT)]  (N >= 256)
+    int* nact;        // [4]
+    int N, NTY, KT, NYQT;  // KT = y-pass tiles per plane (0: no y pass), NYQT = Nyquist tiles per item
+};
+__device__ __forceinline__ int block_excl_scan_1024(int v, int* wsum, int& total) {
+    const int tid = threadIdx.x, nt = blockDim.x;
+    int incl = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(0xffffffffu, incl, o);
+        if ((tid & 31) >= o) incl += t;
+    }
+    __syncthreads();
+    if ((tid & 31) == 31) wsum[tid >> 5] = incl;
+    __syncthreads();
+    if (tid < 32) {
+        int w = (tid < (nt >> 5)) ? wsum[tid] : 0;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, w, o);
+            if (tid >= o) w += t;
+        }
+        wsum[tid] = w;
+    }
+    __syncthreads();
+    total = wsum[31];
+    return incl - v + ((tid >> 5) ? wsum[(tid >> 5) - 1] : 0);
+}
+// Builds the lists of one item from its exclusive bin offsets start_at(0..nbins) (whole block, blockDim.x a multiple of 32
+// and >= nbins / 32; wsum = 32 ints of shared memory).  Bins are visited lanes-over-bins (conflict-free reads of the
+// offsets), the activity flags are packed with warp ballots and the lists are the set bits in increasing order.
+template <class F>
+__device__ __forceinline__ void build_act_lists(const ActLists& al, int b, int nbins, int* wsum, F start_at) {
+    __shared__ int s_base[2];
+    __shared__ int s_planes[512];
+    __shared__ unsigned s_bits[256];   // nbins <= 8192
+    const int tid = threadIdx.x, nt = blockDim.x;
+    const int N = al.N, NTY = al.NTY, lg = 31 - __clz(NTY);   // N and NTY are powers of two
+    auto bin_n = [&](int x, int t) { const int i = ((x & (N - 1)) << lg) + (t & (NTY - 1)); return start_at(i + 1) - start_at(i); };
+    for (int i = tid; i < nbins; i += nt) {   // nbins and nt are multiples of 32: whole warps
+        const int x = i >> lg, t = i & (NTY - 1);
+        int n = bin_n(x, t) + bin_n(x - 1, t);
+        if (NTY > 1) n += bin_n(x, t - 1) + bin_n(x - 1, t - 1);
+        const unsigned word = __ballot_sync(0xffffffffu, n > 0);
+        if ((tid & 31) == 0) s_bits[i >> 5] = word;
+    }
+    __syncthreads();
+    // active tiles: word w -> its set bits
+    const int nwords = nbins >> 5;
+    const unsigned myw = tid < nwords ? s_bits[tid] : 0u;
+    int ztot;
+    int zoff = block_excl_scan_1024(__popc(myw), wsum, ztot);
+    if (tid == 0) s_base[0] = atomicAdd(al.nact + 0, ztot);
+    // active planes: one of the NTY tiles of the plane is active (NTY <= 16 divides 32: the bits sit in one word)
+    int ptot = 0;
+    for (int x0 = 0; x0 < N; x0 += nt) {   // one round unless the block has fewer threads than planes
+        const int x = x0 + tid;
+        int pact = 0;
+        if (x < N) {
+            const int bit0 = x << lg;
+            pact = ((s_bits[bit0 >> 5] >> (bit0 & 31)) & ((NTY >= 32) ? 0xffffffffu : ((1u << NTY) - 1u))) ? 1 : 0;
+            al.plane_act[(size_t)b * N + x] = pact;
+        }
+        int tot;
+        const int poff = ptot + block_excl_scan_1024(pact, wsum, tot);
+        if (x < N && pact) s_planes[poff] = x;
+        ptot += tot;
+    }
+    if (tid == 0) {
+        s_base[1] = al.KT ? atomicAdd(al.nact + 1, ptot * al.KT + al.NYQT) : 0;
+        atomicAdd(al.nact + 2, ptot);
+    }
+    __syncthreads();
+    {
+        int* zl = al.zlist + s_base[0];
+        unsigned w = myw;
+        while (w) { const int bit = __ffs(w) - 1; w &= w - 1; zl[zoff++] = b * nbins + (tid << 5) + bit; }
+    }
+    if (al.KT) {
+        const int tpu = N * al.KT + al.NYQT;   // y-pass tiles per item (dense numbering)
+        const int lk = 31 - __clz(al.KT);      // KT is a power of two
+        int* yl = al.ylist + s_base[1];
+        for (int e = tid; e < ptot * al.KT; e += nt) yl[e] = b * tpu + (s_planes[e >> lk] << lk) + (e & (al.KT - 1));
+        for (int e = tid; e < al.NYQT; e += nt) yl[ptot * al.KT + e] = b * tpu + N * al.KT + e;
+    }
+}
 __global__ void k_bin_scan(int* __restrict__ cnt, int nbins, int P, int* __restrict__ start, int* __restrict__ cursor,
                            unsigned* __restrict__ nmax) {
     pdl_wait();
@@ -117,11 +217,136 @@ __global__ void k_bin_scan(int* __restrict__ cnt, int nbins, int P, int* __restr
     }
     if (tid == 0) st[nbins] = P;
 }
+// ---- F1a in ONE launch (the default): count + rank | per-item barrier | offsets (every block, in shared memory) + scatter ----
+// Phase 1 takes each point's rank inside its bin from the return value of the counting atomicAdd; after the barrier every
+// block of the item scans the item's counts itself (nbins <= 8192: 32 per thread) and places its points at
+// start[bin] + rank -- no second round of atomics, no second barrier, and the launch and drain latencies of two kernels
+// less (the three-kernel version below stays as the fall-back for batches too large to be co-resident).  The splat pass that
+// follows clears the counts and re-arms the barrier, so a forward leaves the state it found (replayable in a CUDA graph).
+struct BinSortParams {
+    const float* pts; const float* nrm;
+    int P, N, NL, nbins;
+    int* cnt;        // [B][nbins] zero on entry and on exit
+    int* start;      // [B][nbins + 1]
+    float4* spts; float4* snrm;
+    unsigned* nmax;  // [B]
+    unsigned* bsync; // [3] arrivals, -, time-out flag
+    ActLists al;
+};
+constexpr int BIN_PPT = 8;   // points per thread of k_bin_sort; bin and rank stay in registers across the barrier
+__global__ void __launch_bounds__(256, 6) k_bin_sort(const BinSortParams p) {
+    extern __shared__ int s_start[];   // [nbins + 1]
+    __shared__ int wsum[32];
+    pdl_wait();
+    // blocks 0 .. gx-1 of an item own its points (point i of block x, thread t, round k: i = (k gx + x) 256 + t); block gx
+    // owns none: it publishes the offsets and builds the activity lists while the others scatter
+    const int b = blockIdx.y, gx = gridDim.x - 1, tid = threadIdx.x, B = gridDim.y;
+    const bool publisher = (int)blockIdx.x == gx;
+    const unsigned nblk = gridDim.x * gridDim.y;
+    const int nbins = p.nbins, P = p.P;
+    int* cnt = p.cnt + (size_t)b * nbins;
+    const float* pts = p.pts + (size_t)b * P * 3;
+    const float* nrm = p.nrm + (size_t)b * P * 3;
+    int key[BIN_PPT], rank[BIN_PPT];
+    if (publisher) {
+        if (tid == 0) {
+            p.nmax[b] = 0u;
+            if (b == 0 && p.al.nact) { p.al.nact[0] = 0; p.al.nact[1] = 0; p.al.nact[2] = 0; p.al.nact[3] = 0; }
+        }
+    } else {
+        // phase 1: count; the value the atomic returns is the point's rank in its bin.  All loads first, then all atomics;
+        // the normals (read in phase 3) are pulled into L2 meanwhile.
+#pragma unroll
+        for (int k = 0; k < BIN_PPT; ++k) {
+            const int i = (k * gx + blockIdx.x) * 256 + tid;
+            key[k] = 0;
+            if (i < P) {
+                key[k] = bin_key(pts + (size_t)i * 3, p.N, p.NL);
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(nrm + (size_t)i * 3));
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < BIN_PPT; ++k) {
+            const int i = (k * gx + blockIdx.x) * 256 + tid;
+            rank[k] = 0;
+            if (i < P) rank[k] = atomicAdd(cnt + key[k], 1);
+        }
+    }
+    // barrier over all blocks of the launch (co-resident: cooperative launch); bounded spin, sticky time-out flag
+    __syncthreads();
+    if (tid == 0) {
+        asm volatile("fence.acq_rel.gpu;" ::: "memory");
+        atomicAdd(p.bsync, 1u);
+        unsigned seen, spins = 0;
+        unsigned long long t0 = 0;
+        do {
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(p.bsync) : "memory");
+            if (seen < nblk && (++spins & 1023u) == 0) {
+                unsigned long long t;
+                asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+                if (t0 == 0) t0 = t;
+                else if (t - t0 > 2000000000ull) { atomicExch(p.bsync + 2, 1u); break; }
+            }
+        } while (seen < nblk);
+        asm volatile("fence.acq_rel.gpu;" ::: "memory");
+    }
+    __syncthreads();
+    // phase 2: exclusive scan of the item's counts into shared memory (every block)
+    for (int i = tid; i < nbins; i += 256) s_start[i] = __ldcg(cnt + i);   // independent, coalesced loads (L2: written by atomics)
+    __syncthreads();
+    const int per = (nbins + 255) / 256;
+    const int lo = min(tid * per, nbins), hi = min(lo + per, nbins);
+    int local = 0;
+    for (int i = lo; i < hi; ++i) local += s_start[i];
+    int tot;
+    int run = block_excl_scan_1024(local, wsum, tot);
+    for (int i = lo; i < hi; ++i) { const int n = s_start[i]; s_start[i] = run; run += n; }
+    if (tid == 0) s_start[nbins] = P;
+    __syncthreads();
+    if (publisher) {
+        int* st = p.start + (size_t)b * (nbins + 1);
+        for (int i = tid; i <= nbins; i += 256) st[i] = s_start[i];
+        if (p.al.zlist) build_act_lists(p.al, b, nbins, wsum, [&](int i) { return s_start[i]; });
+    } else {
+        // phase 3: scatter
+        unsigned amax = 0u;
+#pragma unroll
+        for (int k = 0; k < BIN_PPT; ++k) {
+            const int i = (k * gx + blockIdx.x) * 256 + tid;
+            if (i < P) {
+                const float* c = pts + (size_t)i * 3;
+                const float* n = nrm + (size_t)i * 3;
+                const float n0 = __ldg(n), n1 = __ldg(n + 1), n2 = __ldg(n + 2);
+                const int pos = s_start[key[k]] + rank[k];
+                p.spts[(size_t)b * P + pos] = make_float4(__ldg(c), __ldg(c + 1), __ldg(c + 2), __int_as_float(i));  // .w: index in the caller's order
+                p.snrm[(size_t)b * P + pos] = make_float4(n0, n1, n2, 0.f);
+                amax = max(amax, __float_as_uint(fmaxf(fmaxf(fabsf(n0), fabsf(n1)), fabsf(n2))));
+            }
+        }
+        amax = __reduce_max_sync(0xffffffffu, amax);
+        if ((tid & 31) == 0 && amax) atomicMax(p.nmax + b, amax);
+    }
+    // The counts and the barrier word are cleared by the NEXT kernel of the forward (the splat pass, which starts when
+    // every block of this one is done): no exit round trip here, and a call still leaves the state it found.
+    (void)B;
+}
+// (the last block of each item owns no points: it builds the activity lists from the offsets meanwhile)
 __global__ void k_bin_scatter(const float* __restrict__ pts, const float* __restrict__ nrm, int P, int N, int NL,
                               int nbins, int* __restrict__ cursor, float4* __restrict__ spts,
-                              float4* __restrict__ snrm, unsigned* __restrict__ nmax) {
+                              float4* __restrict__ snrm, unsigned* __restrict__ nmax, const int* __restrict__ start, ActLists al) {
     pdl_wait();
     const int i = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y;
+    if (blockIdx.x == gridDim.x - 1) {
+        if (!al.zlist) return;
+        extern __shared__ int s_st[];   // [nbins + 1] copy of the offsets
+        __shared__ int wsum[32];
+        const int tid = threadIdx.x, nt = blockDim.x;
+        const int* st = start + (size_t)b * (nbins + 1);
+        for (int k = tid; k <= nbins; k += nt) s_st[k] = st[k];
+        __syncthreads();
+        build_act_lists(al, b, nbins, wsum, [&](int k) { return s_st[k]; });
+        return;
+    }
     unsigned amax = 0u;   // bit pattern of max_c |n_c| (non-negative floats order like their bits): scale of the fixed-point splat
     if (i < P) {
         const float* c = pts + ((size_t)b * P + i) * 3;
@@ -375,6 +600,9 @@ struct sap_dpsr {
     int* bin_cnt = nullptr;    // [B][nbins]   (zero between calls)
     int* bin_cursor = nullptr; // [B][nbins]
     int* bin_start = nullptr;  // [B][nbins+1]
+    unsigned* bsync = nullptr; // [3] barrier of k_bin_sort: arrivals, exits, time-out flag
+    int bin_gx_max = 0;        // co-resident blocks of k_bin_sort per batch item (0: three-kernel fall-back)
+    int coop_pdl = 1;          // cooperative launches also take the programmatic-serialization attribute (probed on first use)
     int nbins = 0;
     float2* S3 = nullptr;      // [B*3][N*N*H] 3-channel spectra
     float2* Q3 = nullptr;      // [B*3][N*N]
@@ -391,6 +619,13 @@ struct sap_dpsr {
     float* stats = nullptr;    // [B][4] {mu, a, s, -}
     float* bw = nullptr;       // [B][4] {s, beta/P, S1/a, beta/(P s)}
     unsigned* nmax = nullptr;  // [B] bit pattern of the largest |normal component| of the item (fixed-point scale of the splat)
+    // activity lists (ActLists, written by k_bin_scan): which planes / tiles a point can touch
+    int* plane_act = nullptr;  // [B][N]
+    int* zlist = nullptr;      // [B * nbins]
+    int* ylist = nullptr;      // [B * (N * KT + NYQT)] (N >= 256)
+    int* nact = nullptr;       // [4]
+    bool sparse = true;        // use the lists (SAP_DENSE=1 in the environment of sap_dpsr_create: every tile is processed)
+    bool lists_valid = false;  // the lists belong to the bins in the workspace (the latency path does not write them)
     // staging for the *_host entry points (allocated on first use)
     float *h_pts = nullptr, *h_nrm = nullptr, *h_chi = nullptr, *h_gchi = nullptr, *h_gp = nullptr, *h_gn = nullptr;
     int host_P = 0;
@@ -470,6 +705,28 @@ static void launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t s
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at; cfg.numAttrs = 1;
     cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+
+// cooperative launch (all blocks co-resident: the kernel has a grid barrier), with programmatic dependent launch on top
+// where the driver combines the two attributes
+template <class P>
+static cudaError_t launch_coop(sap_dpsr* h, void (*kernel)(P), dim3 grid, dim3 block, size_t smem, cudaStream_t st, const P& p) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[2];
+    at[0].id = cudaLaunchAttributeCooperative; at[0].val.cooperative = 1;
+    at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization; at[1].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = h->coop_pdl ? 2 : 1;
+    static const bool plain = getenv("SAP_BIN_COOP") && getenv("SAP_BIN_COOP")[0] == '0';   // experiment
+    if (plain) { at[0] = at[1]; cfg.numAttrs = 1; }
+    cudaError_t e = cudaLaunchKernelEx(&cfg, kernel, p);
+    if (e != cudaSuccess && h->coop_pdl) {
+        cudaGetLastError();
+        h->coop_pdl = 0;
+        cfg.numAttrs = 1;
+        e = cudaLaunchKernelEx(&cfg, kernel, p);
+    }
+    return e;
 }
 
 template <class K> static cudaError_t set_smem(K kernel, size_t bytes) {
@@ -573,6 +830,8 @@ template <int N> struct Runner {
         p.mapS = mS; p.mapQ = mQ; p.outS = outS; p.outQ = outQ; p.tw = h->tw; p.ftab = h->ftab;
         (void)axis;
         p.units = units; p.nyq_out_t = C::FUSED_ZY ? 0 : 1;
+        const bool listed = (MODE == MODE_FWD3 || MODE == MODE_INV3) && h->sparse && h->lists_valid;
+        p.ylist = listed ? h->ylist : nullptr; p.nact = h->nact;
         p.cs = (float)((2.0 / ((double)N * N * N)) / (-2.0 * 3.14159265358979323846));
         const long long total = (long long)units * (N * (H / RC::W) + N / RC::W);
         long long grid = (long long)RC::MINB * h->num_sms;
@@ -588,9 +847,11 @@ template <int N> struct Runner {
         if (grid > total) grid = total;
         launch_pdl(k_zl_gbar<N>, dim3((unsigned)grid), dim3(zl_threads<N, false>()), zl_smem_bytes<N, false>(), st, p);
     }
-    static void launch_zl_inv(sap_dpsr* h, cudaStream_t st, const float2* S, const float2* Q, float* out, int planes, int adj3 = 0) {
+    static void launch_zl_inv(sap_dpsr* h, cudaStream_t st, const float2* S, const float2* Q, float* out, int planes, int adj3 = 0,
+                              bool listed = false) {
         using ZC = ZlCfg<N, true>;
-        ZlInvParams p{S, Q, out, h->tw, planes, adj3, h->ftab};
+        ZlInvParams p{S, Q, out, h->tw, planes, adj3, h->ftab, nullptr, h->nact, h->nbins, C::FUSED_ZY ? 1 : N / 32};
+        if (listed && h->sparse && h->lists_valid) p.zlist = h->zlist;
         const long long total = (long long)planes * (N * N / ZC::NL);
         long long grid = (long long)ZC::MINB * h->num_sms;
         if (grid > total) grid = total;
@@ -650,23 +911,42 @@ template <int N> struct Runner {
                 SAP_LAUNCH_CHECK(h, "k_fused_fwd");
                 h->binned_P = P;
                 h->mse_valid = false;
+                h->lists_valid = false;   // the latency path bins the points itself and writes no activity lists
                 return SAP_OK;
             }
         }
         // F1a: bin the points (counting sort); the rasterisation itself happens inside k_zy_fwd
+        bool sorted_in_one = false;
         {
             const dim3 gp((P + 255) / 256, B);
-            launch_pdl(k_bin_count, dim3(gp), dim3(256), 0, st, pts, P, N, C::NL, h->nbins, h->bin_cnt);
-            SAP_LAUNCH_CHECK(h, "k_bin_count");
-            launch_pdl(k_bin_scan, dim3(B), dim3(1024), 0, st, h->bin_cnt, h->nbins, P, h->bin_start, h->bin_cursor, h->nmax);
-            SAP_LAUNCH_CHECK(h, "k_bin_scan");
-            launch_pdl(k_bin_scatter, dim3(gp), dim3(256), 0, st, pts, nrm, P, N, C::NL, h->nbins, h->bin_cursor, h->spts, h->snrm, h->nmax);
-            SAP_LAUNCH_CHECK(h, "k_bin_scatter");
+            constexpr int KT = C::FUSED_ZY ? 0 : H / RingCfg<N>::W, NYQT = C::FUSED_ZY ? 0 : N / RingCfg<N>::W;
+            static_assert(C::FUSED_ZY || RingCfg<N>::W == 16, "ylist is sized for 16-column y-pass tiles");
+            const ActLists al{h->plane_act, h->sparse ? h->zlist : nullptr, h->ylist, h->nact, N, N / C::NL, KT, NYQT};
+            // one launch when every point fits the registers of a co-resident grid (BIN_PPT per thread), else three
+            const int gx = (int)gp.x < h->bin_gx_max ? (int)gp.x : h->bin_gx_max;
+            // (above ~250,000 points the single launch loses: its counting atomics all return a value and arrive at once on
+            // counters that share 128-byte lines -- measured 160 us against 103 us for the three kernels at 10^6 points)
+            sorted_in_one = h->bin_gx_max >= 1 && (long long)gx * 256 * BIN_PPT >= P && (long long)B * P <= 262144;
+            if (sorted_in_one) {
+                const BinSortParams bp{pts, nrm, P, N, C::NL, h->nbins, h->bin_cnt, h->bin_start, h->spts, h->snrm, h->nmax, h->bsync, al};
+                if (!cuda_ok(h, launch_coop(h, k_bin_sort, dim3(gx + 1, B), dim3(256), (size_t)(h->nbins + 1) * sizeof(int), st, bp), "k_bin_sort")) return SAP_ERR_CUDA;
+                SAP_LAUNCH_CHECK(h, "k_bin_sort");
+            } else {
+                launch_pdl(k_bin_count, dim3(gp), dim3(256), 0, st, pts, P, N, C::NL, h->nbins, h->bin_cnt, h->nact);
+                SAP_LAUNCH_CHECK(h, "k_bin_count");
+                launch_pdl(k_bin_scan, dim3(B), dim3(1024), 0, st, h->bin_cnt, h->nbins, P, h->bin_start, h->bin_cursor, h->nmax);
+                SAP_LAUNCH_CHECK(h, "k_bin_scan");
+                launch_pdl(k_bin_scatter, dim3(gp.x + 1, B), dim3(256), (size_t)(h->nbins + 1) * sizeof(int), st, pts, nrm, P, N, C::NL, h->nbins, h->bin_cursor,
+                           h->spts, h->snrm, h->nmax, (const int*)h->bin_start, al);
+                SAP_LAUNCH_CHECK(h, "k_bin_scatter");
+            }
+            h->lists_valid = h->sparse;
             h->binned_P = P;
         }
         // F2 z (+y) forward, 3 channels
         {
-            ZyFwdParams p{h->spts, h->snrm, h->bin_start, P, nullptr, nullptr, h->S3, C::FUSED_ZY ? h->Q3 : h->QT3, h->tw, 3, h->nmax};
+            ZyFwdParams p{h->spts, h->snrm, h->bin_start, P, nullptr, nullptr, h->S3, C::FUSED_ZY ? h->Q3 : h->QT3, h->tw, 3, h->nmax,
+                          (!C::FUSED_ZY && h->sparse) ? h->plane_act : nullptr, sorted_in_one ? h->bin_cnt : nullptr, B * h->nbins, h->bsync};
             launch_pdl(k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_SPLAT, C::NT_ZY>, dim3(N * N / C::NL, B * 3), dim3(C::NT_ZY), zy_smem_bytes<N, C::NL>(), st, p);
             SAP_LAUNCH_CHECK(h, "k_zy_fwd");
         }
@@ -728,7 +1008,7 @@ template <int N> struct Runner {
         }
         // B2 + B3: Gbar' assembled on load, z (+y) forward
         {
-            ZyFwdParams p{h->spts, h->snrm, h->bin_start, P, gchi, h->bw, h->S1, C::FUSED_ZY ? h->Q1 : h->QT1, h->tw, 1, h->nmax};
+            ZyFwdParams p{h->spts, h->snrm, h->bin_start, P, gchi, h->bw, h->S1, C::FUSED_ZY ? h->Q1 : h->QT1, h->tw, 1, h->nmax, nullptr, nullptr, 0, nullptr};
             if constexpr (C::FUSED_ZY) launch_zl_gbar(h, st, p, B);
             else launch_pdl(k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_GBAR, C::NT_ZY>, dim3(N * N / C::NL, B), dim3(C::NT_ZY), zy_smem_bytes<N, C::NL>(), st, p);
             SAP_LAUNCH_CHECK(h, C::FUSED_ZY ? "k_zl_gbar" : "k_zy_fwd<GBAR>");
@@ -746,7 +1026,7 @@ template <int N> struct Runner {
         }
         // B5 (y +) z inverse -> vbar (into the v workspace)
         {
-            launch_zl_inv(h, st, h->S3, h->Q3, h->v, B * 3, C::FUSED_ZY ? 1 : 0);  // fused: planes (x, B, -) -> (x, y, z)
+            launch_zl_inv(h, st, h->S3, h->Q3, h->v, B * 3, C::FUSED_ZY ? 1 : 0, true);  // fused: planes (x, B, -) -> (x, y, z)
             SAP_LAUNCH_CHECK(h, "k_zl_inv");
         }
         // B6 gather
@@ -780,6 +1060,8 @@ static void free_all(sap_dpsr* h) {
     for (int i = 0; i < sap_dpsr::MAX_EV; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
     cudaFree(h->v); cudaFree(h->spts); cudaFree(h->snrm); cudaFree(h->bin_cnt); cudaFree(h->bin_cursor); cudaFree(h->bin_start); cudaFree(h->S3); cudaFree(h->Q3); cudaFree(h->S1); cudaFree(h->Q1); cudaFree(h->QT3); cudaFree(h->QT1); cudaFree(h->tw); cudaFree(h->ftab);
     cudaFree(h->fhist); cudaFree(h->facc); cudaFree(h->fsync); cudaFree(h->fstamps);
+    cudaFree(h->bsync);
+    cudaFree(h->plane_act); cudaFree(h->zlist); cudaFree(h->ylist); cudaFree(h->nact);
     cudaFree(h->gmse); cudaFree(h->acc_mse); cudaFree(h->acc); cudaFree(h->ticket); cudaFree(h->stats); cudaFree(h->bw); cudaFree(h->nmax);
     cudaFree(h->h_pts); cudaFree(h->h_nrm); cudaFree(h->h_chi); cudaFree(h->h_gchi); cudaFree(h->h_gp); cudaFree(h->h_gn);
 }
@@ -810,6 +1092,7 @@ extern "C" sap_status_t sap_dpsr_create(int N, float sigma, int batch, int max_p
     upd(dev_alloc(h, &h->bin_cnt, B * (size_t)h->nbins));
     upd(dev_alloc(h, &h->bin_cursor, B * (size_t)h->nbins));
     upd(dev_alloc(h, &h->bin_start, B * (size_t)(h->nbins + 1)));
+    upd(dev_alloc(h, &h->bsync, (size_t)4));
     upd(dev_alloc(h, &h->S3, B * 3 * SP));
     upd(dev_alloc(h, &h->Q3, B * 3 * QP));
     upd(dev_alloc(h, &h->S1, B * SP));
@@ -822,6 +1105,14 @@ extern "C" sap_status_t sap_dpsr_create(int N, float sigma, int batch, int max_p
     upd(dev_alloc(h, &h->stats, B * 4));
     upd(dev_alloc(h, &h->bw, B * 4));
     upd(dev_alloc(h, &h->nmax, B));
+    {
+        const char* dense = getenv("SAP_DENSE");
+        h->sparse = !(dense && dense[0] == '1');
+        upd(dev_alloc(h, &h->plane_act, B * (size_t)N));
+        upd(dev_alloc(h, &h->zlist, B * (size_t)h->nbins));
+        if (N >= 256) upd(dev_alloc(h, &h->ylist, B * ((size_t)N * (N / 2 / 16) + N / 16)));
+        upd(dev_alloc(h, &h->nact, (size_t)4));
+    }
     h->fused_ok = (N <= 128) && ((long long)batch * N <= h->num_sms) && batch <= (N == 32 ? 4 : N == 64 ? 2 : 1);
     if (h->fused_ok) {
         upd(dev_alloc(h, &h->fhist, B * (size_t)h->num_sms * N));
@@ -850,6 +1141,16 @@ extern "C" sap_status_t sap_dpsr_create(int N, float sigma, int batch, int max_p
     upd(cudaMemset(h->stats, 0, sizeof(float) * B * 4));
     upd(cudaMemset(h->bw, 0, sizeof(float) * B * 4));
     upd(cudaMemset(h->nmax, 0, sizeof(unsigned) * B));
+    upd(cudaMemset(h->nact, 0, sizeof(int) * 4));
+    upd(cudaMemset(h->bsync, 0, sizeof(unsigned) * 4));
+    {   // single-launch binning: all its blocks must be co-resident (grid barrier)
+        int occ = 0;
+        const size_t sm = (size_t)(h->nbins + 1) * sizeof(int);
+        upd(cudaFuncSetAttribute(k_bin_sort, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+        upd(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_bin_sort, 256, sm));
+        const char* b3 = getenv("SAP_BIN3");
+        h->bin_gx_max = (b3 && b3[0] == '1') ? 0 : (int)(((long long)occ * h->num_sms) / batch) - 1;   // + 1 publisher block per item
+    }
     if (h->fused_ok) {
         upd(cudaMemset(h->facc, 0, sizeof(double) * B * 2));
         upd(cudaMemset(h->fsync, 0, sizeof(unsigned) * 4));
@@ -1027,10 +1328,19 @@ extern "C" sap_status_t sap_dpsr_get_stats(sap_dpsr_t* h, float* stats_host, voi
     cudaStream_t s = (cudaStream_t)stream;
     float* tmp = new (std::nothrow) float[(size_t)h->batch * 4];
     if (!tmp) { h->err = "host allocation failed"; return SAP_ERR_OOM; }
-    unsigned flag = 0;
+    unsigned flag = 0, bflag = 0;
     bool ok = cuda_ok(h, cudaMemcpyAsync(tmp, h->stats, sizeof(float) * 4 * h->batch, cudaMemcpyDeviceToHost, s), "D2H stats") &&
               (!h->fsync || cuda_ok(h, cudaMemcpyAsync(&flag, h->fsync + 2, sizeof(unsigned), cudaMemcpyDeviceToHost, s), "D2H flag")) &&
+              cuda_ok(h, cudaMemcpyAsync(&bflag, h->bsync + 2, sizeof(unsigned), cudaMemcpyDeviceToHost, s), "D2H flag") &&
               cuda_ok(h, cudaStreamSynchronize(s), "cudaStreamSynchronize");
+    if (ok && bflag) {  // the barrier of k_bin_sort gave up waiting
+        h->err = "k_bin_sort: grid barrier timed out; results of that call are invalid";
+        cudaMemsetAsync(h->bsync, 0, sizeof(unsigned) * 4, s);
+        cudaMemsetAsync(h->bin_cnt, 0, sizeof(int) * (size_t)h->batch * h->nbins, s);
+        cudaStreamSynchronize(s);
+        delete[] tmp;
+        return SAP_ERR_CUDA;
+    }
     if (ok && flag) {  // a grid barrier of the fused path gave up waiting (the CTAs of the launch were not co-resident)
         h->err = "fused path: grid barrier timed out; results of that call are invalid";
         cudaMemsetAsync(h->fsync, 0, sizeof(unsigned) * 4, s);

@@ -37,7 +37,8 @@ template <int N, bool INV> constexpr int zl_threads() { return ZlCfg<N, INV>::NT
 template <int N, bool INV> constexpr int zl_buf_elems() { return ZlCfg<N, INV>::NL * (N / 2) + ZlCfg<N, INV>::NL; }  // float2 per buffer
 template <int N, bool INV> constexpr size_t zl_smem_bytes() {
     return (size_t)ZlCfg<N, INV>::NBUF * zl_buf_elems<N, INV>() * sizeof(float2) + (size_t)N * sizeof(float2) +
-           3 * ZlCfg<N, INV>::NBUF * sizeof(uint64_t) + (size_t)(N + N / 2 + 4) * sizeof(float) + 128;
+           3 * ZlCfg<N, INV>::NBUF * sizeof(uint64_t) + (size_t)(N + N / 2 + 4) * sizeof(float) + 128 +
+           (INV ? (size_t)zl_threads<N, INV>() * sizeof(int) : 0);   // tile ids of this CTA (listed mode of k_zl_inv)
 }
 
 static_assert(zl_smem_bytes<128, true>() <= SMEM_PER_CTA_MAX && zl_smem_bytes<256, true>() <= SMEM_PER_CTA_MAX &&
@@ -54,6 +55,11 @@ struct ZlInvParams {
     // planes are IFFT(plane 0), IFFT(h_y B), IFFT(h_z B): plane 2 is made from plane 1 (fetched again: an L2 hit)
     int adj3;
     const float4* ftab; // per-slot frequency table (spectral.cuh), used in adjoint mode
+    // listed mode (the three vbar planes of the backward; see ActLists in sap_dpsr.cu), nullptr = every tile: only the tiles
+    // a point can touch are transformed -- the gather (B6) reads nothing else
+    const int* zlist;   // ids item * nbins + bin of the active bin tiles (bin = x * NTY + ty, 32 lines for N >= 256, a plane below)
+    const int* nact;    // {|zlist|, -, -, -}
+    int nbins, nty;
 };
 
 // plain bulk copy global -> shared, completion on an mbarrier (bytes: multiple of 16, both addresses 16-aligned)
@@ -201,6 +207,27 @@ struct ZlRing {
     const float2* srcS;  // tile g: NL*H complex at srcS + g*NL*H
     const float2* srcQ;  // tile g: NL complex at srcQ + g*NL (nullptr: the tile has no Nyquist part, GBAR input)
     int adj3;            // fused adjoint planes: the tiles of plane 3i+2 are fetched from plane 3i+1
+    const int* tcache = nullptr;   // listed mode: tile ids of this CTA (shared memory, TCAP entries), else nullptr
+    const int* zlist = nullptr;
+    int nbins = 0, nty = 1;
+    static constexpr int TCAP = ZlCfg<N, INV>::NTC * ZlCfg<N, INV>::NG;
+    // listed mode: virtual tile v -> (active bin tile v / (3 SUB), channel, sub-tile) -> dense tile id
+    __device__ __forceinline__ long long expand(long long v) const {
+        constexpr int SUB = (N <= 128) ? 1 : 32 / NL, TPP = 2 * H * 2 * H / NL;
+        const long long e = v / (3 * SUB);
+        const int r = (int)(v - e * (3 * SUB)), ch = r / SUB, sub = r - ch * SUB;
+        const int id = zlist[e], item = id / nbins, bin = id - item * nbins;
+        const int x = bin / nty, ty = bin - x * nty;
+        const int tile = (N <= 128) ? x : (x * (2 * H) + ty * 32) / NL + sub;
+        return ((long long)item * 3 + ch) * TPP + tile;
+    }
+    // it-th tile of this CTA (dense tile id), -1 past the end
+    __device__ __forceinline__ long long tile_at(int it) const {
+        const long long v = (long long)blockIdx.x + (long long)it * gridDim.x;
+        if (v >= total) return -1;
+        if (zlist) return it < TCAP ? (long long)tcache[it] : expand(v);
+        return v;
+    }
     __device__ __forceinline__ void init() const {
         if (threadIdx.x == 0) {
             for (int s = 0; s < NBUF; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, NTC / 32); issued[s] = 0; }
@@ -208,8 +235,8 @@ struct ZlRing {
         }
     }
     __device__ __forceinline__ void issue_load(int it) const {
-        long long g = (long long)blockIdx.x + (long long)it * gridDim.x;
-        if (g >= total) return;
+        long long g = tile_at(it);
+        if (g < 0) return;
         if (adj3) {
             constexpr int TPP = 2 * H * 2 * H / NL;  // tiles per plane
             if ((g / TPP) % 3 == 2) g -= TPP;
@@ -262,6 +289,7 @@ __global__ void __launch_bounds__(zl_threads<N, true>(), ZlCfg<N, true>::MINB) k
     ring.adj3 = FUSED ? p.adj3 : 0;
     float* fy = reinterpret_cast<float*>(const_cast<int*>(ring.issued + NBUF));  // h_y per y slot, h_z per z slot (+ Nyquist)
     float* fz = fy + N;
+    int* tcache = reinterpret_cast<int*>(fz + H + 4);
     const int group = threadIdx.x / NTC, tid = threadIdx.x - group * NTC;
     for (int i = threadIdx.x; i < N; i += zl_threads<N, true>()) tw[i] = p.tw[i];
     if (FUSED && p.adj3) {
@@ -271,11 +299,22 @@ __global__ void __launch_bounds__(zl_threads<N, true>(), ZlCfg<N, true>::MINB) k
     ring.init();
     __syncthreads();
     pdl_wait();
+    if (p.zlist) {   // listed mode: the tiles of this CTA are entries blockIdx.x + it * gridDim.x of the expanded active list
+        constexpr int SUB = (N <= 128) ? 1 : 32 / NL;
+        ring.zlist = p.zlist; ring.nbins = p.nbins; ring.nty = p.nty;
+        ring.total = (long long)p.nact[0] * 3 * SUB;
+        const long long v = (long long)blockIdx.x + (long long)threadIdx.x * gridDim.x;
+        tcache[threadIdx.x] = v < ring.total ? (int)ring.expand(v) : -1;
+        ring.tcache = tcache;
+        __syncthreads();
+    }
     if (threadIdx.x == 0) {
 #pragma unroll 1
         for (int it = 0; it < NBUF; ++it) ring.issue_load(it);
     }
-    for (long long j = group, g = blockIdx.x + (long long)group * gridDim.x; g < ring.total; j += NG, g += (long long)NG * gridDim.x) {
+    for (long long j = group;; j += NG) {
+        const long long g = ring.tile_at((int)j);
+        if (g < 0) break;
         float2* s = ring.acquire((int)j);
         if constexpr (FUSED) {
             static_assert(!FUSED || Plan<N>::NS == 2, "fused planes use two-stage y plans");

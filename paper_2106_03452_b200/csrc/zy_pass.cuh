@@ -31,6 +31,11 @@ struct ZyFwdParams {
     const float2* tw;      // exp(-2 pi i t / N), t < N
     int nch;               // planes per batch item (3 for SPLAT, 1 for GBAR)
     const unsigned* nmax;  // SPLAT: [batch] bit pattern of max_i max_c |n_ic| (k_bin_scatter), for the fixed-point scale
+    const int* plane_act;  // SPLAT, N >= 256: [batch][N] activity of the x-planes (k_bin_scan), or nullptr.  The y pass
+                           // neither loads nor transforms an inactive plane: its tiles of channel 2 are not written
+    int* clear_cnt;        // SPLAT after k_bin_sort: the bin counts [clear_n] and the barrier word, cleared here for the next
+    int clear_n;           // forward (every block of k_bin_sort is done with them when this kernel starts), or nullptr
+    unsigned* clear_sync;
 };
 
 // Column swizzle of the main spectrum in HBM: the value of z slot pz of line (x, y) is stored in column
@@ -100,6 +105,10 @@ SAP_HD void zy_fwd_body(Ctx& ctx, const ZyFwdParams& p, float2* smem, int bx, in
     const size_t V = (size_t)N * N * N;
     const size_t line0 = (size_t)bx * NL;  // global line index = x*N + y
 
+    if (SRC == SRC_SPLAT && p.clear_cnt && bx == 0 && by == 0) {
+        for (int i = ctx.tid; i < p.clear_n; i += ctx.nthr) p.clear_cnt[i] = 0;
+        if (ctx.tid == 0) p.clear_sync[0] = 0u;
+    }
     float2* So = p.S + (size_t)by * ((size_t)N * N * H) + line0 * H;
     float2* Qo = p.Q + (size_t)by * ((size_t)N * N) + line0;
     // A0: which bins can touch lines [line0, line0 + NL): x-slabs {x, x-1} x y-tiles {ty, ty-1}
@@ -119,8 +128,12 @@ SAP_HD void zy_fwd_body(Ctx& ctx, const ZyFwdParams& p, float2* smem, int bx, in
         total += b_n[k];
     }
     if (SRC == SRC_SPLAT && total == 0) {  // nothing lands here: the spectrum of zeros is zeros (before any other work)
+        // inactive plane: the y pass (in place on channels 0 and 1) does not touch it and the x pass reads the zeros of
+        // channels 0 and 1 as the y pass's output; nobody reads channel 2
+        const bool skip_main = !DO_Y && ch == 2 && p.plane_act && p.plane_act[(size_t)item * N + x] == 0;
         float4* So4 = reinterpret_cast<float4*>(So);
-        for (int i = ctx.tid; i < NL * H / 2; i += ctx.nthr) So4[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (!skip_main)
+            for (int i = ctx.tid; i < NL * H / 2; i += ctx.nthr) So4[i] = make_float4(0.f, 0.f, 0.f, 0.f);
         if constexpr (DO_Y) {
             for (int l = ctx.tid; l < NL; l += ctx.nthr) Qo[l] = make_float2(0.f, 0.f);
         } else {
