@@ -39,6 +39,7 @@ KERNEL_BYTES_V = {
     # label: (compulsory V for N <= 128 (y fused with z), compulsory V for N >= 256)
     "F:k_bin_sort": (0.0, 0.0), "F:k_bin_count": (0.0, 0.0), "F:k_bin_scan": (0.0, 0.0), "F:k_bin_scatter": (0.0, 0.0),   # 72 B/point, no grid traffic
     "F:k_zy_fwd": (3.0, 3.0),            # writes 3 spectra; the splatted field never exists in HBM
+    "F:k_zw_fwd<SPLAT>": (3.0, 3.0),     # the same for N >= 256 (z pass only)
     "F:k_ring<FWD,y>": (0.0, 5.0),       # N >= 256 only: reads 3 spectra, writes 2 (x, u = h_y y + h_z z)
     "F:k_ring<SOLVE>": (4.0, 3.0),       # reads 3 (2) spectra, writes 1
     "F:k_ring<INV,y>": (0.0, 2.0),
@@ -48,7 +49,7 @@ KERNEL_BYTES_V = {
     "F:k_scale_shift_mse": (4.0, 4.0),
     "B:k_reduce_g": (2.0, 2.0),          # reads G and chi
     "B:k_zl_gbar": (2.0, 2.0),           # reads G, writes 1 spectrum (W is re-rasterised, not read)
-    "B:k_zy_fwd<GBAR>": (2.0, 2.0),
+    "B:k_zw_fwd<GBAR>": (2.0, 2.0),
     "B:k_ring<FWD,y>": (0.0, 2.0),
     "B:k_ring<ADJ>": (3.0, 3.0),         # reads 1 spectrum, writes 2 (x, B)
     "B:k_ring<INV,y>": (0.0, 5.0),       # reads 2 spectra, writes 3

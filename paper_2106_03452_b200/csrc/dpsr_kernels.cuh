@@ -9,12 +9,14 @@
 // "Stored order": slot p of an axis holds frequency pos2freq<len>(p) (fft_core.cuh); x and y are
 // length-N complex transforms, z is a real transform done as an H-point complex FFT + split.
 //
-//   zy_pass.cuh     splat + forward z (+ y) pass, one tile per CTA
+//   zy_pass.cuh     splat + forward z + y pass of the fused planes (N <= 128), one plane per CTA
+//   zwarp_pass.cuh  splat / Gbar' + forward z pass for N >= 256, one tile of 32 lines per CTA, a warp owns its lines
 //   zline_pass.cuh  persistent bulk-copy z (+ y) passes: inverse, fused Gbar'
 //   ring_pass.cuh   persistent TMA ring: x pass with the fused spectral solve / its adjoint, y pass (N >= 256)
 #pragma once
 #include "fft_core.cuh"
 #include "spectral.cuh"
 #include "zy_pass.cuh"
+#include "zwarp_pass.cuh"
 #include "ring_pass.cuh"
 #include "zline_pass.cuh"

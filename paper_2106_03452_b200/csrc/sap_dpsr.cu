@@ -788,9 +788,13 @@ template <int N> struct Runner {
         }
         auto upd = [&](cudaError_t x) { if (e == cudaSuccess) e = x; };
         upd(set_smem(k_zl_inv<N>, zl_smem_bytes<N, true>()));
-        upd(set_smem(k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_SPLAT, C::NT_ZY>, zy_smem_bytes<N, C::NL>()));
-        if constexpr (C::FUSED_ZY) upd(set_smem(k_zl_gbar<N>, zl_smem_bytes<N, false>()));
-        else upd(set_smem(k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_GBAR, C::NT_ZY>, zy_smem_bytes<N, C::NL>()));
+        if constexpr (C::FUSED_ZY) {
+            upd(set_smem(k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_SPLAT, C::NT_ZY>, zy_smem_bytes<N, C::NL>()));
+            upd(set_smem(k_zl_gbar<N>, zl_smem_bytes<N, false>()));
+        } else {
+            upd(set_smem(k_zw_fwd<N, SRC_SPLAT>, ZwCfg<N>::SMEM));
+            upd(set_smem(k_zw_fwd<N, SRC_GBAR>, ZwCfg<N>::SMEM));
+        }
         upd(set_smem(k_ring<N, MODE_SOLVE>, ring_smem_bytes<N, MODE_SOLVE>()));
         upd(set_smem(k_ring<N, MODE_ADJ>, ring_smem_bytes<N, MODE_ADJ>()));
         if constexpr (!C::FUSED_ZY) {
@@ -947,8 +951,11 @@ template <int N> struct Runner {
         {
             ZyFwdParams p{h->spts, h->snrm, h->bin_start, P, nullptr, nullptr, h->S3, C::FUSED_ZY ? h->Q3 : h->QT3, h->tw, 3, h->nmax,
                           (!C::FUSED_ZY && h->sparse) ? h->plane_act : nullptr, sorted_in_one ? h->bin_cnt : nullptr, B * h->nbins, h->bsync};
-            launch_pdl(k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_SPLAT, C::NT_ZY>, dim3(N * N / C::NL, B * 3), dim3(C::NT_ZY), zy_smem_bytes<N, C::NL>(), st, p);
-            SAP_LAUNCH_CHECK(h, "k_zy_fwd");
+            if constexpr (C::FUSED_ZY)
+                launch_pdl(k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_SPLAT, C::NT_ZY>, dim3(N * N / C::NL, B * 3), dim3(C::NT_ZY), zy_smem_bytes<N, C::NL>(), st, p);
+            else
+                launch_pdl(k_zw_fwd<N, SRC_SPLAT>, dim3(N * N / ZwCfg<N>::NL, B * 3), dim3(ZwCfg<N>::NT), ZwCfg<N>::SMEM, st, p);
+            SAP_LAUNCH_CHECK(h, C::FUSED_ZY ? "k_zy_fwd" : "k_zw_fwd<SPLAT>");
         }
         if constexpr (!C::FUSED_ZY) {
             launch_ring<MODE_FWD3>(h, st, B, h->mS3y, h->mQT3, h->S3, h->Q3, 1);  // planes (x, u, -) out of (x, y, z)
@@ -1010,8 +1017,8 @@ template <int N> struct Runner {
         {
             ZyFwdParams p{h->spts, h->snrm, h->bin_start, P, gchi, h->bw, h->S1, C::FUSED_ZY ? h->Q1 : h->QT1, h->tw, 1, h->nmax, nullptr, nullptr, 0, nullptr};
             if constexpr (C::FUSED_ZY) launch_zl_gbar(h, st, p, B);
-            else launch_pdl(k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_GBAR, C::NT_ZY>, dim3(N * N / C::NL, B), dim3(C::NT_ZY), zy_smem_bytes<N, C::NL>(), st, p);
-            SAP_LAUNCH_CHECK(h, C::FUSED_ZY ? "k_zl_gbar" : "k_zy_fwd<GBAR>");
+            else launch_pdl(k_zw_fwd<N, SRC_GBAR>, dim3(N * N / ZwCfg<N>::NL, B), dim3(ZwCfg<N>::NT), ZwCfg<N>::SMEM, st, p);
+            SAP_LAUNCH_CHECK(h, C::FUSED_ZY ? "k_zl_gbar" : "k_zw_fwd<GBAR>");
         }
         if constexpr (!C::FUSED_ZY) {
             launch_ring<MODE_FWD>(h, st, B, h->mS1y, h->mQT1, h->S1, h->Q1, 1);
