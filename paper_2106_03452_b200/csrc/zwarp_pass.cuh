@@ -97,7 +97,10 @@ __global__ void __launch_bounds__(ZwCfg<N>::NT, ZwCfg<N>::MINB) k_zw_fwd(const Z
     // tables, zero fill
     for (int i = tid; i < H; i += NT) { const float2 w = p.tw[(i >> 4) + R0 * (i & 15)]; tws[i] = make_float2(0.5f * w.x, 0.5f * w.y); }
     for (int i = tid; i < (R0 - 1) * 16; i += NT) tw0[i] = p.tw[2 * ((i >> 4) + 1) * (i & 15)];
-    {
+    // GBAR tile that no point can touch: W = 0 there, Gbar' = s G (- the delta term) straight from HBM: no zero fill, no
+    // rasterisation, one barrier less
+    const bool has_pts = total > 0;
+    if (has_pts) {
         float4* s4 = reinterpret_cast<float4*>(s);
         for (int i = tid; i < NL * LP / 2; i += NT) s4[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
@@ -105,8 +108,8 @@ __global__ void __launch_bounds__(ZwCfg<N>::NT, ZwCfg<N>::MINB) k_zw_fwd(const Z
     // component of the item) x 2^k < 2^30
     const float amax = (SRC == SRC_SPLAT) ? bits_u2f(p.nmax[item]) : 1.f;
     const FixScale fs = fix_scale((float)total * amax);
-    __syncthreads();
-    {
+    if (has_pts) __syncthreads();
+    if (has_pts) {
         int* si = reinterpret_cast<int*>(s);
         const float4* sp = p.spts + (size_t)item * p.P;
         const float4* sn = p.snrm + (size_t)item * p.P;
@@ -162,10 +165,15 @@ __global__ void __launch_bounds__(ZwCfg<N>::NT, ZwCfg<N>::MINB) k_zw_fwd(const Z
             if (SRC == SRC_GBAR) {
 #pragma unroll
                 for (int r = 0; r < R0; ++r) v[r] = g2[l * H + j + 16 * r];
+                if (has_pts) {
 #pragma unroll
-                for (int r = 0; r < R0; ++r) {
-                    const int2 iv = *reinterpret_cast<const int2*>(ls + BS * r);
-                    v[r] = __ffma2_rn(make_float2(cs_, cs_), v[r], __fmul2_rn(make_float2(cw, cw), make_float2((float)iv.x, (float)iv.y)));
+                    for (int r = 0; r < R0; ++r) {
+                        const int2 iv = *reinterpret_cast<const int2*>(ls + BS * r);
+                        v[r] = __ffma2_rn(make_float2(cs_, cs_), v[r], __fmul2_rn(make_float2(cw, cw), make_float2((float)iv.x, (float)iv.y)));
+                    }
+                } else {
+#pragma unroll
+                    for (int r = 0; r < R0; ++r) v[r] = cscale(cs_, v[r]);
                 }
                 if (line0 == 0 && l == 0 && j == 0) v[0].x -= c0;
             } else {
