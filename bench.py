@@ -58,6 +58,24 @@ KERNEL_BYTES_V = {
     # latency path: only chi (forward) / G and chi (backward) must cross HBM; the spectra live in L2 between the phases
     "F:k_fused_fwd": (1.0, 1.0), "B:k_fused_bwd": (2.0, 2.0),
 }
+# With the activity lists (sap_dpsr_get_activity: ft = active tiles / tiles, fp = active planes / planes) the listed kernels
+# only move what a point can touch: their compulsory bytes scale with the fraction they process.
+SPARSE_BYTES_V = {
+    "F:k_zw_fwd<SPLAT>": lambda N, ft, fp: 2.0 + fp,          # channels 0, 1 in full (zeros included), channel 2 on active planes
+    "F:k_ring<FWD,y>": lambda N, ft, fp: 5.0 * fp,             # 3 spectra in, 2 out, active planes only
+    "B:k_ring<INV,y>": lambda N, ft, fp: 5.0 * fp,             # 2 in, 3 out, active planes only
+    "B:k_zl_inv": lambda N, ft, fp: (5.0 if N <= 128 else 6.0) * ft,   # active tiles only
+}
+
+
+def compulsory_v(name, cfg, act):
+    """bytes (in V) kernel `name` must read once + write once on this workload; act = (ft, fp) or None (dense)"""
+    cv = KERNEL_BYTES_V.get(name, (0.0, 0.0))[0 if cfg.N <= 128 else 1]
+    if act is not None and name in SPARSE_BYTES_V and cv > 0:
+        cv = SPARSE_BYTES_V[name](cfg.N, act[0], act[1])
+    return cv
+
+
 TRAFFIC_JSON = os.path.join(ROOT, "profiles", "r02_traffic.json")
 
 
@@ -219,10 +237,18 @@ def time_config(cfg_id, steps, warmup, rank, torch, flush, with_e2e=True, with_p
         launches += h.last_launch_count
         b.record(stream)
     torch.cuda.synchronize()
+    act = None
+    if h.path == "throughput":
+        try:
+            at, nt_, ap_, np_ = h.activity(stream)
+            act = (at / max(nt_, 1), ap_ / max(np_, 1))
+        except Exception:   # lists switched off
+            act = None
     t_fwd = sum(a.elapsed_time(m) for a, m, b in ev)
     t_all = sum(a.elapsed_time(b) for a, m, b in ev)
     res = {"cfg": cfg, "ms_total": t_all, "ms_fwd": t_fwd / steps, "ms_bwd": (t_all - t_fwd) / steps,
-           "ms_step": t_all / steps, "launches": launches, "workspace_bytes": h.workspace_bytes, "path": h.path}
+           "ms_step": t_all / steps, "launches": launches, "workspace_bytes": h.workspace_bytes, "path": h.path,
+           "activity": act}
 
     if with_profile:   # second pass with per-kernel events (their gaps would perturb the headline timing)
         h.set_profiling(True)
@@ -474,7 +500,7 @@ def roofline_of(res, peak_gbs, traffic):
     V = 4.0 * cfg.N ** 3 * cfg.batch
     km = res["kernels_ms"]
     name = max(km, key=km.get)
-    comp_v = KERNEL_BYTES_V[name][0 if cfg.N <= 128 else 1]
+    comp_v = compulsory_v(name, cfg, res.get("activity"))
     ach = comp_v * V / (km[name] * 1e-3) / 1e9
     t = traffic.get(cfg.name, {}).get(name)
     return {"bound": "hbm", "kernel": name, "kernel_ms": km[name], "share_of_step": km[name] / sum(km.values()),
@@ -488,10 +514,19 @@ def kernel_fracs(res, peak_gbs):
     V = 4.0 * cfg.N ** 3 * cfg.batch
     out = {}
     for k, ms in res["kernels_ms"].items():
-        cv = KERNEL_BYTES_V.get(k, (0.0, 0.0))[0 if cfg.N <= 128 else 1]
+        cv = compulsory_v(k, cfg, res.get("activity"))
         if cv > 0:
             out[k] = round(cv * V / (ms * 1e-3) / 1e9 / peak_gbs, 3)
     return out
+
+
+def activity_of(res):
+    a = res.get("activity")
+    if a is None:
+        return None
+    return {"active_tile_fraction": round(a[0], 4), "active_plane_fraction": round(a[1], 4),
+            "what": "fraction of the 32-line tiles (planes for N <= 128) / x-planes a point can touch: the 3-channel y and z passes "
+                    "process only those (sap_dpsr_get_activity); their compulsory bytes are scaled accordingly"}
 
 
 def oracle_baseline(cfg_id, reps):
@@ -586,6 +621,7 @@ def main():
         "roofline": dict(roofline_of(res2, peak, traffic), peak_source=peak_src, traffic_source=traffic_src),
         "kernels_ms": res2["kernels_ms"],
         "kernel_frac_of_hbm_peak": kernel_fracs(res2, peak),
+        "activity": activity_of(res2),
         "paper_context": "PAPER.md Table 4: 12 ms forward only at 128^3, 140 ms at 256^3, on a GTX 1080 Ti (not the target)",
     }
     solo = rank == 0 and world == 1
@@ -607,7 +643,7 @@ def main():
                             "dram_bytes_per_fwd_bwd_in_V": (actual / (Vc * c.batch)) if actual else None,
                             "dram_GBps_actual": (actual / c.batch / (per_grid * 1e-3) / 1e9) if actual else None,
                             "roofline": roofline_of(r, peak, traffic), "kernels_ms": km,
-                            "kernel_frac_of_hbm_peak": kernel_fracs(r, peak)}
+                            "kernel_frac_of_hbm_peak": kernel_fracs(r, peak), "activity": activity_of(r)}
             if not args.no_cpu_baseline:
                 also[c.name]["cpu_baseline"] = oracle_baseline(cid, 1)
         # both implementations of the path where the latency path applies

@@ -166,6 +166,20 @@ int sap_dpsr_get_fused_phases(sap_dpsr_t* h, float* us, const char** names, int 
  * Synchronises `stream`. */
 sap_status_t sap_dpsr_get_stats(sap_dpsr_t* h, float* stats_host, void* stream);
 
+/*
+ * Activity lists (on by default).  The binning of a forward also records which 32-line tiles (whole x-planes for
+ * N <= 128) and which x-planes a point can touch at all (Eq.10-11: a point reaches the 8 grid nodes
+ * around it).  The splatted field is identically zero elsewhere and the gather of the backward reads nothing there, so
+ * the y and z passes of the three-channel spectra (forward y pass and inverse y pass for N >= 256, inverse z pass of
+ * the backward for every N) only load, transform and store what is active; results are unchanged.
+ * sap_dpsr_set_sparse(h, 0) makes every pass process every tile (for measurements); takes effect at the next forward.
+ * sap_dpsr_get_activity copies the counts of the last throughput-path forward to host, summed over the batch:
+ * out_host[4] = {active tiles, tiles, active planes, planes}; synchronises `stream`.  SAP_ERR_INVALID_ARG when the
+ * lists are off or the last forward took the latency path (which keeps no lists).
+ */
+sap_status_t sap_dpsr_set_sparse(sap_dpsr_t* h, int on);
+sap_status_t sap_dpsr_get_activity(sap_dpsr_t* h, int* out_host, void* stream);
+
 /* Frees the workspace and the handle.  NULL is allowed. */
 void sap_dpsr_destroy(sap_dpsr_t* h);
 

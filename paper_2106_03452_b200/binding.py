@@ -17,7 +17,7 @@ EXPORTS = [
     "sap_dpsr_backward_host", "sap_dpsr_get_stats", "sap_dpsr_destroy", "sap_dpsr_last_error",
     "sap_dpsr_workspace_bytes", "sap_dpsr_last_launch_count", "sap_dpsr_set_profiling", "sap_dpsr_get_profile",
     "sap_dpsr_epoch", "sap_dpsr_check_epoch", "sap_dpsr_reserve", "sap_dpsr_set_path", "sap_dpsr_get_path",
-    "sap_dpsr_get_fused_phases",
+    "sap_dpsr_get_fused_phases", "sap_dpsr_set_sparse", "sap_dpsr_get_activity",
 ]
 SAP_PATH_AUTO, SAP_PATH_THROUGHPUT, SAP_PATH_LATENCY = 0, 1, 2
 PATHS = {"auto": 0, "throughput": 1, "latency": 2}
@@ -65,6 +65,10 @@ def lib():
     L.sap_dpsr_last_error.restype = ctypes.c_char_p
     L.sap_dpsr_workspace_bytes.argtypes = [vp]
     L.sap_dpsr_workspace_bytes.restype = ctypes.c_size_t
+    L.sap_dpsr_set_sparse.argtypes = [vp, ci]
+    L.sap_dpsr_set_sparse.restype = ci
+    L.sap_dpsr_get_activity.argtypes = [vp, vp, vp]
+    L.sap_dpsr_get_activity.restype = ci
     L.sap_dpsr_last_launch_count.argtypes = [vp]
     L.sap_dpsr_last_launch_count.restype = ci
     L.sap_dpsr_set_profiling.argtypes = [vp, ci]
@@ -205,6 +209,17 @@ class Dpsr:
         out = np.empty((self.batch, 3), np.float32)
         self._check(lib().sap_dpsr_get_stats(self._h, out.ctypes.data_as(ctypes.c_void_p), _stream_ptr(stream)))
         return out
+
+    def set_sparse(self, on=True):
+        """Activity lists on / off (sap_dpsr_set_sparse); takes effect at the next forward."""
+        self._check(lib().sap_dpsr_set_sparse(self._h, 1 if on else 0))
+
+    def activity(self, stream=None):
+        """(active tiles, tiles, active planes, planes) of the last throughput-path forward, summed over the batch."""
+        import numpy as np
+        out = np.zeros(4, np.int32)
+        self._check(lib().sap_dpsr_get_activity(self._h, out.ctypes.data_as(ctypes.c_void_p), _stream_ptr(stream)))
+        return tuple(int(v) for v in out)
 
     @property
     def epoch(self):

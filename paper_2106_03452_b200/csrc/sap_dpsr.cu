@@ -1361,6 +1361,26 @@ extern "C" sap_status_t sap_dpsr_get_stats(sap_dpsr_t* h, float* stats_host, voi
     return ok ? SAP_OK : SAP_ERR_CUDA;
 }
 
+extern "C" sap_status_t sap_dpsr_set_sparse(sap_dpsr_t* h, int on) {
+    if (!h) return SAP_ERR_INVALID_ARG;
+    h->err.clear();
+    h->sparse = on != 0;
+    h->lists_valid = false;   // the next forward rebuilds (or drops) the lists
+    return SAP_OK;
+}
+extern "C" sap_status_t sap_dpsr_get_activity(sap_dpsr_t* h, int* out_host, void* stream) {
+    if (!h) return SAP_ERR_INVALID_ARG;
+    h->err.clear();
+    if (!out_host) { h->err = "null pointer argument"; return SAP_ERR_INVALID_ARG; }
+    if (!h->sparse || !h->lists_valid) { h->err = "no activity lists (switched off, or the last forward took the latency path)"; return SAP_ERR_INVALID_ARG; }
+    int n[4] = {0, 0, 0, 0};
+    cudaStream_t s = (cudaStream_t)stream;
+    if (!cuda_ok(h, cudaMemcpyAsync(n, h->nact, sizeof n, cudaMemcpyDeviceToHost, s), "D2H activity") ||
+        !cuda_ok(h, cudaStreamSynchronize(s), "cudaStreamSynchronize")) return SAP_ERR_CUDA;
+    out_host[0] = n[0]; out_host[1] = h->batch * h->nbins; out_host[2] = n[2]; out_host[3] = h->batch * h->N;
+    return SAP_OK;
+}
+
 extern "C" void sap_dpsr_destroy(sap_dpsr_t* h) {
     if (!h) return;
     free_all(h);

@@ -439,3 +439,117 @@ def test_autograd_function():
     assert np.linalg.norm(tp.grad.cpu().numpy()[0] - b["grad_points"]) <= GRAD_TOL * np.linalg.norm(b["grad_points"])
     assert np.linalg.norm(tn.grad.cpu().numpy()[0] - b["grad_normals"]) <= GRAD_TOL * np.linalg.norm(b["grad_normals"])
     h.close()
+
+
+# ---- activity lists ("nobody computes what nobody reads", sap_dpsr_set_sparse / sap_dpsr_get_activity) -----------------------
+def _blob(P, centre, radius, seed):
+    """points on a small sphere (a few active planes / tiles), periodic wrap when it sticks out of the cube"""
+    rng = np.random.default_rng(seed)
+    d = rng.normal(size=(P, 3))
+    d /= np.linalg.norm(d, axis=1, keepdims=True)
+    pts = (np.asarray(centre)[None] + radius * d) % 1.0
+    return pts.astype(np.float32), d.astype(np.float32)
+
+
+def _active_counts(N, pts):
+    """numpy restatement of the activity rule: tile (x, ty) is active when a point lies in bin (x | x-1, ty | ty-1)"""
+    NL = N if N <= 128 else 32
+    NTY = N // NL
+    j = np.floor(pts.astype(np.float32) * np.float32(N)).astype(np.int64) % N
+    cnt = np.zeros((N, NTY), np.int64)
+    np.add.at(cnt, (j[:, 0], j[:, 1] // NL), 1)
+    act = cnt + np.roll(cnt, 1, 0)
+    if NTY > 1:
+        act = act + np.roll(cnt, 1, 1) + np.roll(np.roll(cnt, 1, 0), 1, 1)
+    ta = act > 0
+    return int(ta.sum()), int(ta.any(1).sum())
+
+
+def _run_sparse_dense(N, sigma, pts, nrm, G):
+    import torch
+    from paper_2106_03452_b200.binding import Dpsr
+    B, P = pts.shape[0], pts.shape[1]
+    out = {}
+    for mode in ("sparse", "dense"):
+        h = Dpsr(N, sigma, B, P)
+        h.set_path("throughput")
+        h.set_sparse(mode == "sparse")
+        tp, tn = torch.from_numpy(pts).cuda(), torch.from_numpy(nrm).cuda()
+        chi = h.forward(tp, tn)
+        act = h.activity() if mode == "sparse" else None
+        gp, gn = h.backward(tp, tn, chi, torch.from_numpy(G).cuda())
+        torch.cuda.synchronize()
+        out[mode] = dict(chi=chi.cpu().numpy(), gp=gp.cpu().numpy(), gn=gn.cpu().numpy(), act=act, stats=h.stats())
+        if mode == "dense":
+            with pytest.raises(Exception):
+                h.activity()
+        h.close()
+    return out
+
+
+@pytest.mark.parametrize("N,B,P", [(64, 2, 2500), (128, 3, 4000), (256, 1, 12000)])
+def test_activity_lists_leave_results_unchanged(N, B, P):
+    # items with very different activity: a small blob wrapping around the cube corner, a blob in the middle, a full-size shape
+    pts = np.empty((B, P, 3), np.float32)
+    nrm = np.empty((B, P, 3), np.float32)
+    specs = [((0.02, 0.97, 0.5), 0.06), ((0.5, 0.52, 0.47), 0.11), None]
+    for b in range(B):
+        if specs[b % 3] is None:
+            pts[b], nrm[b] = inputs.make_cloud("ellipsoids3", P, seed=40 + b)
+        else:
+            pts[b], nrm[b] = _blob(P, specs[b % 3][0], specs[b % 3][1], seed=40 + b)
+    G = inputs.upstream_grad(N, B, seed=11)
+    r = _run_sparse_dense(N, 2.0, pts, nrm, G)
+    s, d = r["sparse"], r["dense"]
+    # the skipped tiles hold zeros (forward) or values nobody reads (backward): same arithmetic on everything else (the
+    # order of the points inside a bin, hence of the float sums of the point mean and the gather, varies from run to run)
+    assert np.abs(s["chi"] - d["chi"]).max() <= 2e-6 * np.abs(d["chi"]).max()
+    assert np.linalg.norm(s["gp"] - d["gp"]) <= 1e-5 * np.linalg.norm(d["gp"])
+    assert np.linalg.norm(s["gn"] - d["gn"]) <= 1e-5 * np.linalg.norm(d["gn"])
+    want_t = sum(_active_counts(N, pts[b])[0] for b in range(B))
+    want_p = sum(_active_counts(N, pts[b])[1] for b in range(B))
+    NTY = 1 if N <= 128 else N // 32
+    assert s["act"] == (want_t, B * N * NTY, want_p, B * N)
+    assert want_p < B * N    # the case does exercise skipped planes
+    for b in range(B):
+        _check_item(N, 2.0, pts[b], nrm[b], G[b], s["chi"][b], s["stats"][b], s["gp"][b], s["gn"][b])
+
+
+def test_single_launch_binning_matches_the_three_kernel_fallback(monkeypatch):
+    # k_bin_sort (one cooperative launch) against k_bin_count / k_bin_scan / k_bin_scatter: same bins; the order of the
+    # points inside a bin differs, which only reorders float sums in the point mean and nothing in the fixed-point splat
+    N, P = 128, 7001
+    pts, nrm = inputs.make_cloud("torus", P, seed=5)
+    G = inputs.upstream_grad(N, 1, seed=12)
+    a = _gpu_run(N, 2.0, pts[None], nrm[None], G, path="throughput")
+    monkeypatch.setenv("SAP_BIN3", "1")
+    b = _gpu_run(N, 2.0, pts[None], nrm[None], G, path="throughput")
+    monkeypatch.delenv("SAP_BIN3")
+    assert a["fwd_launches"] + 2 == b["fwd_launches"]
+    assert np.abs(a["chi"] - b["chi"]).max() <= 2e-6 * np.abs(b["chi"]).max()
+    assert np.linalg.norm(a["gp"] - b["gp"]) <= 1e-5 * np.linalg.norm(b["gp"])
+    assert np.linalg.norm(a["gn"] - b["gn"]) <= 1e-5 * np.linalg.norm(b["gn"])
+    _check_item(N, 2.0, pts, nrm, G[0], a["chi"][0], a["stats"][0], a["gp"][0], a["gn"][0])
+
+
+def test_forward_on_one_path_backward_on_the_other_with_lists():
+    # the latency path writes no activity lists: a throughput backward after it must fall back to every tile
+    import torch
+    from paper_2106_03452_b200.binding import Dpsr
+    N, P = 64, 3000
+    pts, nrm = _blob(P, (0.3, 0.3, 0.6), 0.12, seed=3)
+    G = inputs.upstream_grad(N, 1, seed=13)
+    h = Dpsr(N, 2.0, 1, P)
+    tp, tn, tG = torch.from_numpy(pts[None]).cuda(), torch.from_numpy(nrm[None]).cuda(), torch.from_numpy(G).cuda()
+    h.set_path("throughput")
+    chi = h.forward(tp, tn)
+    assert h.activity()[2] < N
+    h.set_path("latency")
+    chi = h.forward(tp, tn)
+    with pytest.raises(Exception):
+        h.activity()
+    h.set_path("throughput")
+    gp, gn = h.backward(tp, tn, chi, tG)
+    torch.cuda.synchronize()
+    _check_item(N, 2.0, pts, nrm, G[0], chi.cpu().numpy()[0], h.stats()[0], gp.cpu().numpy()[0], gn.cpu().numpy()[0])
+    h.close()
