@@ -276,6 +276,9 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
     int* tcache = const_cast<int*>(reinterpret_cast<volatile int*>(issued + NSTAGE + (NSTAGE & 1)));  // listed mode: this CTA's tile ids
     constexpr int TCAP = ring_threads<N, MODE>();
     constexpr bool CAN_LIST = (MODE == MODE_FWD3 || MODE == MODE_INV3);
+    // The forward y passes read what the z pass before them wrote plane by plane in ascending x: they walk the planes in
+    // DESCENDING x, so that the planes written last -- still in the 126 MB L2 -- are read first.
+    constexpr bool REVERSED = (MODE == MODE_FWD3 || MODE == MODE_FWD);
     const int group = threadIdx.x / NTC, tid = threadIdx.x - group * NTC;
 
     for (int i = threadIdx.x; i < TWE; i += ring_threads<N, MODE>()) {
@@ -297,13 +300,14 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
     const long long total = listed ? (long long)p.nact[1] : (long long)p.units * tiles_per_unit;
     if (CAN_LIST && listed) {
         const long long idx = (long long)blockIdx.x + (long long)threadIdx.x * gridDim.x;
-        tcache[threadIdx.x] = idx < total ? p.ylist[idx] : -1;
+        tcache[threadIdx.x] = idx < total ? p.ylist[REVERSED ? total - 1 - idx : idx] : -1;
         __syncthreads();
     }
     // j-th tile of this CTA (global tile id), -1 past the end
     auto tile_at = [&](int j) -> long long {
-        const long long idx = (long long)blockIdx.x + (long long)j * gridDim.x;
+        long long idx = (long long)blockIdx.x + (long long)j * gridDim.x;
         if (idx >= total) return -1;
+        if (REVERSED) idx = total - 1 - idx;
         if (CAN_LIST && listed) return j < TCAP ? (long long)tcache[j] : (long long)p.ylist[idx];
         return idx;
     };

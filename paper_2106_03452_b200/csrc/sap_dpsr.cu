@@ -504,10 +504,12 @@ __global__ void k_reduce_g(const float4* __restrict__ G, const float4* __restric
     float s0 = 0.f, s1 = 0.f;
     const size_t stride = (size_t)gridDim.x * blockDim.x;
     size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    // (walks the grids from the END: chi was written front to back by the normalisation pass, its tail is still in L2)
+    const size_t last = n4_per_item - 1;
     for (; i + 3 * stride < n4_per_item; i += 4 * stride) {  // 8 independent 16-byte loads in flight per thread
         float4 a[4], x[4];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) { a[u] = __ldcs(g + i + u * stride); x[u] = __ldcs(c + i + u * stride); }
+        for (int u = 0; u < 4; ++u) { a[u] = __ldcs(g + (last - (i + u * stride))); x[u] = __ldcs(c + (last - (i + u * stride))); }
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
             s0 += (a[u].x + a[u].y) + (a[u].z + a[u].w);
@@ -515,7 +517,7 @@ __global__ void k_reduce_g(const float4* __restrict__ G, const float4* __restric
         }
     }
     for (; i < n4_per_item; i += stride) {
-        const float4 a = g[i], x = c[i];
+        const float4 a = g[last - i], x = c[last - i];
         s0 += (a.x + a.y) + (a.z + a.w);
         s1 += (a.x * x.x + a.y * x.y) + (a.z * x.z + a.w * x.w);
     }

@@ -223,9 +223,12 @@ struct ZlRing {
     }
     // it-th tile of this CTA (dense tile id), -1 past the end
     __device__ __forceinline__ long long tile_at(int it) const {
-        const long long v = (long long)blockIdx.x + (long long)it * gridDim.x;
+        long long v = (long long)blockIdx.x + (long long)it * gridDim.x;
         if (v >= total) return -1;
-        if (zlist) return it < TCAP ? (long long)tcache[it] : expand(v);
+        // N = 256, inverse (at 512^3 a spectrum is four times the L2: measured no gain): the y pass before this kernel wrote the planes in ascending x; walk them in descending x so
+        // that the planes still in L2 are read first
+        if (INV && N == 256) v = total - 1 - v;
+        if (zlist) return it < TCAP ? (long long)tcache[it] : expand(v);   // (v already reversed above)
         return v;
     }
     __device__ __forceinline__ void init() const {
@@ -304,7 +307,7 @@ __global__ void __launch_bounds__(zl_threads<N, true>(), ZlCfg<N, true>::MINB) k
         ring.zlist = p.zlist; ring.nbins = p.nbins; ring.nty = p.nty;
         ring.total = (long long)p.nact[0] * 3 * SUB;
         const long long v = (long long)blockIdx.x + (long long)threadIdx.x * gridDim.x;
-        tcache[threadIdx.x] = v < ring.total ? (int)ring.expand(v) : -1;
+        tcache[threadIdx.x] = v < ring.total ? (int)ring.expand(N == 256 ? ring.total - 1 - v : v) : -1;
         ring.tcache = tcache;
         __syncthreads();
     }
