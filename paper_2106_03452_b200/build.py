@@ -10,7 +10,7 @@ PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libsap_dpsr.so"
 SOURCES = [CSRC / "sap_dpsr.cu", CSRC / "sap_mesh.cu"]
-HEADERS = [CSRC / "fft_core.cuh", CSRC / "zwarp_pass.cuh", CSRC / "fused_small.cuh", CSRC / "dpsr_kernels.cuh", CSRC / "zy_pass.cuh", CSRC / "spectral.cuh", CSRC / "ring_pass.cuh", CSRC / "zline_pass.cuh", PKG.parent / "include" / "sap_dpsr.h", PKG.parent / "include" / "sap_mesh.h"]
+HEADERS = [CSRC / "fft_core.cuh", CSRC / "zwarp_pass.cuh", CSRC / "zwarp_inv.cuh", CSRC / "fused_small.cuh", CSRC / "dpsr_kernels.cuh", CSRC / "zy_pass.cuh", CSRC / "spectral.cuh", CSRC / "ring_pass.cuh", CSRC / "zline_pass.cuh", PKG.parent / "include" / "sap_dpsr.h", PKG.parent / "include" / "sap_mesh.h"]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

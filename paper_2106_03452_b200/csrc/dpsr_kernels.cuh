@@ -11,6 +11,7 @@
 //
 //   zy_pass.cuh     splat + forward z + y pass of the fused planes (N <= 128), one plane per CTA
 //   zwarp_pass.cuh  splat / Gbar' + forward z pass for N >= 256, one tile of 32 lines per CTA, a warp owns its lines
+//   zwarp_inv.cuh   inverse z pass for N >= 256, the mirror of zwarp_pass.cuh
 //   zline_pass.cuh  persistent bulk-copy z (+ y) passes: inverse, fused Gbar'
 //   ring_pass.cuh   persistent TMA ring: x pass with the fused spectral solve / its adjoint, y pass (N >= 256)
 #pragma once
@@ -20,3 +21,4 @@
 #include "zwarp_pass.cuh"
 #include "ring_pass.cuh"
 #include "zline_pass.cuh"
+#include "zwarp_inv.cuh"

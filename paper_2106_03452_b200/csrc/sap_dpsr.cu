@@ -796,6 +796,7 @@ template <int N> struct Runner {
         } else {
             upd(set_smem(k_zw_fwd<N, SRC_SPLAT>, ZwCfg<N>::SMEM));
             upd(set_smem(k_zw_fwd<N, SRC_GBAR>, ZwCfg<N>::SMEM));
+            upd(set_smem(k_zw_inv<N>, ZwCfg<N>::SMEM));
         }
         upd(set_smem(k_ring<N, MODE_SOLVE>, ring_smem_bytes<N, MODE_SOLVE>()));
         upd(set_smem(k_ring<N, MODE_ADJ>, ring_smem_bytes<N, MODE_ADJ>()));
@@ -858,6 +859,16 @@ template <int N> struct Runner {
         using ZC = ZlCfg<N, true>;
         ZlInvParams p{S, Q, out, h->tw, planes, adj3, h->ftab, nullptr, h->nact, h->nbins, C::FUSED_ZY ? 1 : N / 32};
         if (listed && h->sparse && h->lists_valid) p.zlist = h->zlist;
+        if constexpr (!C::FUSED_ZY) {
+            static const bool ring = getenv("SAP_ZL_RING") && getenv("SAP_ZL_RING")[0] == '1';   // experiment: the ring kernel
+            if (!ring) {
+                const long long total = (long long)planes * (N * N / ZwCfg<N>::NL);
+                long long grid = (long long)ZwCfg<N>::MINB * h->num_sms;
+                if (grid > total) grid = total;
+                launch_pdl(k_zw_inv<N>, dim3((unsigned)grid), dim3(ZwCfg<N>::NT), ZwCfg<N>::SMEM, st, p);
+                return;
+            }
+        }
         const long long total = (long long)planes * (N * N / ZC::NL);
         long long grid = (long long)ZC::MINB * h->num_sms;
         if (grid > total) grid = total;

@@ -82,6 +82,9 @@ def bench_label(name: str, backward: bool) -> str:
     m = re.match(r"k_zy_fwd<(\d+), ?(\d+), ?(\w+), ?(\d+)", n)
     if m:
         return pre + ("k_zy_fwd<GBAR>" if m.group(4) == "1" else "k_zy_fwd")
+    m = re.match(r"k_zw_fwd<(\d+), ?(\d+)>", n)
+    if m:
+        return pre + ("k_zw_fwd<GBAR>" if m.group(2) == "1" else "k_zw_fwd<SPLAT>")
     return pre + re.sub(r"<.*", "", n)
 
 
@@ -126,7 +129,7 @@ def summarise_full(rep: str, cfg: str, cmd: str):
              "Command (under gpurun, directly after the same command exited 0 without ncu):", "", f"    {cmd}", "",
              "Launches in capture order.  Times are under the profiler (replayed, cold): use them for ratios and counters, not as",
              "bench values.  `k_ring<N, MODE>`: MODE 0 = FWD(y), 1 = INV(y), 2 = SOLVE, 3 = ADJ, 4 = FWD3, 5 = INV3; `k_zy_fwd<N, NL, FUSED_Y,",
-             "SRC, NT>`: SRC 0 = SPLAT, 1 = GBAR.  `dram % of ncu peak` is of ncu's own peak (about 8.2 TB/s); the measured copy bandwidth",
+             "SRC, NT>` and `k_zw_fwd<N, SRC>`: SRC 0 = SPLAT, 1 = GBAR.  `dram % of ncu peak` is of ncu's own peak (about 8.2 TB/s); the measured copy bandwidth",
              "(MEASURED_PEAKS.json, 6.54 TB/s) is 80 % of it.  `dram read` + `dram write` per launch is `roofline.traffic` in bench.py.", "",
              "| metric | " + " | ".join(f"`{n}`" for n in names) + " |", "|---|" + "---|" * len(names),
              "| grid | " + " | ".join(r[col["Grid Size"]] for r in data) + " |"]
