@@ -44,6 +44,7 @@ KERNEL_BYTES_V = {
     "F:k_ring<SOLVE>": (4.0, 3.0),       # reads 3 (2) spectra, writes 1
     "F:k_ring<INV,y>": (0.0, 2.0),
     "F:k_zl_inv": (2.0, 2.0),            # reads 1 spectrum, writes chi'
+    "F:k_zw_inv": (2.0, 2.0),            # the same for N >= 256 (z pass only)
     "F:k_sample_mean": (0.0, 0.0),       # gathers 8 values per point
     "F:k_scale_shift": (2.0, 2.0),
     "F:k_scale_shift_mse": (4.0, 4.0),
@@ -53,6 +54,7 @@ KERNEL_BYTES_V = {
     "B:k_ring<FWD,y>": (0.0, 2.0),
     "B:k_ring<ADJ>": (3.0, 3.0),         # reads 1 spectrum, writes 2 (x, B)
     "B:k_ring<INV,y>": (0.0, 5.0),       # reads 2 spectra, writes 3
+    "B:k_zw_inv": (6.0, 6.0),            # N >= 256: reads 3 spectra, writes 3 grids
     "B:k_zl_inv": (5.0, 6.0),            # N <= 128: reads 2 spectra (B twice, the second time from L2), writes 3 grids
     "B:k_gather_grads": (0.0, 0.0),      # gathers 32 values per point
     # latency path: only chi (forward) / G and chi (backward) must cross HBM; the spectra live in L2 between the phases
@@ -65,6 +67,7 @@ SPARSE_BYTES_V = {
     "F:k_ring<FWD,y>": lambda N, ft, fp: 5.0 * fp,             # 3 spectra in, 2 out, active planes only
     "B:k_ring<INV,y>": lambda N, ft, fp: 5.0 * fp,             # 2 in, 3 out, active planes only
     "B:k_zl_inv": lambda N, ft, fp: (5.0 if N <= 128 else 6.0) * ft,   # active tiles only
+    "B:k_zw_inv": lambda N, ft, fp: 6.0 * ft,
 }
 
 

@@ -226,13 +226,14 @@ __global__ void k_bin_scan(int* __restrict__ cnt, int nbins, int P, int* __restr
 struct BinSortParams {
     const float* pts; const float* nrm;
     int P, N, NL, nbins;
-    int* cnt;        // [B][nbins] zero on entry and on exit
+    int* cnt;        // [B][nbins][BIN_CS] (entry 0 of each group of BIN_CS) zero on entry; cleared by the splat pass
     int* start;      // [B][nbins + 1]
     float4* spts; float4* snrm;
     unsigned* nmax;  // [B]
     unsigned* bsync; // [3] arrivals, -, time-out flag
     ActLists al;
 };
+constexpr int BIN_CS = 8;    // k_bin_sort keeps one counter per 32-byte sector (atomics to one 128-byte line serialise in L2)
 constexpr int BIN_PPT = 8;   // points per thread of k_bin_sort; bin and rank stay in registers across the barrier
 __global__ void __launch_bounds__(256, 6) k_bin_sort(const BinSortParams p) {
     extern __shared__ int s_start[];   // [nbins + 1]
@@ -244,7 +245,7 @@ __global__ void __launch_bounds__(256, 6) k_bin_sort(const BinSortParams p) {
     const bool publisher = (int)blockIdx.x == gx;
     const unsigned nblk = gridDim.x * gridDim.y;
     const int nbins = p.nbins, P = p.P;
-    int* cnt = p.cnt + (size_t)b * nbins;
+    int* cnt = p.cnt + (size_t)b * nbins * BIN_CS;
     const float* pts = p.pts + (size_t)b * P * 3;
     const float* nrm = p.nrm + (size_t)b * P * 3;
     int key[BIN_PPT], rank[BIN_PPT];
@@ -269,7 +270,7 @@ __global__ void __launch_bounds__(256, 6) k_bin_sort(const BinSortParams p) {
         for (int k = 0; k < BIN_PPT; ++k) {
             const int i = (k * gx + blockIdx.x) * 256 + tid;
             rank[k] = 0;
-            if (i < P) rank[k] = atomicAdd(cnt + key[k], 1);
+            if (i < P) rank[k] = atomicAdd(cnt + key[k] * BIN_CS, 1);
         }
     }
     // barrier over all blocks of the launch (co-resident: cooperative launch); bounded spin, sticky time-out flag
@@ -292,7 +293,7 @@ __global__ void __launch_bounds__(256, 6) k_bin_sort(const BinSortParams p) {
     }
     __syncthreads();
     // phase 2: exclusive scan of the item's counts into shared memory (every block)
-    for (int i = tid; i < nbins; i += 256) s_start[i] = __ldcg(cnt + i);   // independent, coalesced loads (L2: written by atomics)
+    for (int i = tid; i < nbins; i += 256) s_start[i] = __ldcg(cnt + i * BIN_CS);   // independent loads (L2: written by atomics)
     __syncthreads();
     const int per = (nbins + 255) / 256;
     const int lo = min(tid * per, nbins), hi = min(lo + per, nbins);
@@ -941,9 +942,10 @@ template <int N> struct Runner {
             const ActLists al{h->plane_act, h->sparse ? h->zlist : nullptr, h->ylist, h->nact, N, N / C::NL, KT, NYQT};
             // one launch when every point fits the registers of a co-resident grid (BIN_PPT per thread), else three
             const int gx = (int)gp.x < h->bin_gx_max ? (int)gp.x : h->bin_gx_max;
-            // (above ~250,000 points the single launch loses: its counting atomics all return a value and arrive at once on
-            // counters that share 128-byte lines -- measured 160 us against 103 us for the three kernels at 10^6 points)
-            sorted_in_one = h->bin_gx_max >= 1 && (long long)gx * 256 * BIN_PPT >= P && (long long)B * P <= 262144;
+            // (measured with one counter per 32-byte sector: 480,000 points 31 us against 48 us for the three kernels, 10^6 points
+            // 131 us against 98 us -- every counting atomic returns a value and they all arrive at once)
+            constexpr long long bin1_max = 524288;
+            sorted_in_one = h->bin_gx_max >= 1 && (long long)gx * 256 * BIN_PPT >= P && (long long)B * P <= bin1_max;
             if (sorted_in_one) {
                 const BinSortParams bp{pts, nrm, P, N, C::NL, h->nbins, h->bin_cnt, h->bin_start, h->spts, h->snrm, h->nmax, h->bsync, al};
                 if (!cuda_ok(h, launch_coop(h, k_bin_sort, dim3(gx + 1, B), dim3(256), (size_t)(h->nbins + 1) * sizeof(int), st, bp), "k_bin_sort")) return SAP_ERR_CUDA;
@@ -963,7 +965,7 @@ template <int N> struct Runner {
         // F2 z (+y) forward, 3 channels
         {
             ZyFwdParams p{h->spts, h->snrm, h->bin_start, P, nullptr, nullptr, h->S3, C::FUSED_ZY ? h->Q3 : h->QT3, h->tw, 3, h->nmax,
-                          (!C::FUSED_ZY && h->sparse) ? h->plane_act : nullptr, sorted_in_one ? h->bin_cnt : nullptr, B * h->nbins, h->bsync};
+                          (!C::FUSED_ZY && h->sparse) ? h->plane_act : nullptr, sorted_in_one ? h->bin_cnt : nullptr, B * h->nbins * BIN_CS, h->bsync};
             if constexpr (C::FUSED_ZY)
                 launch_pdl(k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_SPLAT, C::NT_ZY>, dim3(N * N / C::NL, B * 3), dim3(C::NT_ZY), zy_smem_bytes<N, C::NL>(), st, p);
             else
@@ -984,7 +986,7 @@ template <int N> struct Runner {
         // F4 (y +) z inverse -> chi'
         {
             launch_zl_inv(h, st, h->S1, h->Q1, chi, B);
-            SAP_LAUNCH_CHECK(h, "k_zl_inv");
+            SAP_LAUNCH_CHECK(h, C::FUSED_ZY ? "k_zl_inv" : "k_zw_inv");
         }
         // F5 normalise
         {
@@ -1047,7 +1049,7 @@ template <int N> struct Runner {
         // B5 (y +) z inverse -> vbar (into the v workspace)
         {
             launch_zl_inv(h, st, h->S3, h->Q3, h->v, B * 3, C::FUSED_ZY ? 1 : 0, true);  // fused: planes (x, B, -) -> (x, y, z)
-            SAP_LAUNCH_CHECK(h, "k_zl_inv");
+            SAP_LAUNCH_CHECK(h, C::FUSED_ZY ? "k_zl_inv" : "k_zw_inv");
         }
         // B6 gather
         launch_pdl(k_gather_grads, dim3(dim3((P + 127) / 128, B)), dim3(128), 0, st, (const float4*)h->spts, (const float4*)h->snrm, P, N, (const float*)h->v, chi, (const float*)h->bw, gp, gn);
@@ -1109,7 +1111,7 @@ extern "C" sap_status_t sap_dpsr_create(int N, float sigma, int batch, int max_p
     upd(dev_alloc(h, &h->v, B * 3 * V));
     upd(dev_alloc(h, &h->spts, B * (size_t)max_points));
     upd(dev_alloc(h, &h->snrm, B * (size_t)max_points));
-    upd(dev_alloc(h, &h->bin_cnt, B * (size_t)h->nbins));
+    upd(dev_alloc(h, &h->bin_cnt, B * (size_t)h->nbins * BIN_CS));
     upd(dev_alloc(h, &h->bin_cursor, B * (size_t)h->nbins));
     upd(dev_alloc(h, &h->bin_start, B * (size_t)(h->nbins + 1)));
     upd(dev_alloc(h, &h->bsync, (size_t)4));
@@ -1155,7 +1157,7 @@ extern "C" sap_status_t sap_dpsr_create(int N, float sigma, int batch, int max_p
     }
     upd(cudaMemcpy(h->tw, tw, sizeof(float2) * N, cudaMemcpyHostToDevice));
     delete[] tw;
-    upd(cudaMemset(h->bin_cnt, 0, sizeof(int) * B * h->nbins));
+    upd(cudaMemset(h->bin_cnt, 0, sizeof(int) * B * h->nbins * BIN_CS));
     upd(cudaMemset(h->acc, 0, sizeof(double) * B * 3));
     upd(cudaMemset(h->ticket, 0, sizeof(unsigned) * B * 2));
     upd(cudaMemset(h->stats, 0, sizeof(float) * B * 4));
@@ -1356,7 +1358,7 @@ extern "C" sap_status_t sap_dpsr_get_stats(sap_dpsr_t* h, float* stats_host, voi
     if (ok && bflag) {  // the barrier of k_bin_sort gave up waiting
         h->err = "k_bin_sort: grid barrier timed out; results of that call are invalid";
         cudaMemsetAsync(h->bsync, 0, sizeof(unsigned) * 4, s);
-        cudaMemsetAsync(h->bin_cnt, 0, sizeof(int) * (size_t)h->batch * h->nbins, s);
+        cudaMemsetAsync(h->bin_cnt, 0, sizeof(int) * (size_t)h->batch * h->nbins * BIN_CS, s);
         cudaStreamSynchronize(s);
         delete[] tmp;
         return SAP_ERR_CUDA;
