@@ -63,9 +63,9 @@ KERNEL_BYTES_V = {
 # With the activity lists (sap_dpsr_get_activity: ft = active tiles / tiles, fp = active planes / planes) the listed kernels
 # only move what a point can touch: their compulsory bytes scale with the fraction they process.
 SPARSE_BYTES_V = {
-    "F:k_zw_fwd<SPLAT>": lambda N, ft, fp: 2.0 + fp,          # channels 0, 1 in full (zeros included), channel 2 on active planes
+    "F:k_zw_fwd<SPLAT>": lambda N, ft, fp: 3.0 * ft + 2.0 * (1.0 - fp),   # active tiles x 3 channels + the zeros of channels 0, 1 on inactive planes
     "F:k_ring<FWD,y>": lambda N, ft, fp: 5.0 * fp,             # 3 spectra in, 2 out, active planes only
-    "B:k_ring<INV,y>": lambda N, ft, fp: 5.0 * fp,             # 2 in, 3 out, active planes only
+    "B:k_ring<INV,y>": lambda N, ft, fp: 2.0 * fp + 3.0 * ft,  # 2 in on active planes, 3 out on active tiles
     "B:k_zl_inv": lambda N, ft, fp: (5.0 if N <= 128 else 6.0) * ft,   # active tiles only
     "B:k_zw_inv": lambda N, ft, fp: 6.0 * ft,
 }

@@ -44,7 +44,8 @@ template <int N, int MODE> constexpr size_t ring_smem_bytes() {
     using C = RingCfgM<N, MODE>;
     return (size_t)C::NSTAGE * N * C::W * sizeof(float2) + 2 * (size_t)ring_tw_entries<N>() * sizeof(float4) +
            (size_t)N * sizeof(float4) + 3 * C::NSTAGE * sizeof(uint64_t) + 128 +
-           (size_t)ring_threads<N, MODE>() * sizeof(int);   // tile ids of this CTA (listed mode)
+           (size_t)ring_threads<N, MODE>() * sizeof(int) +  // tile ids of this CTA (listed mode)
+           (N >= 256 && (MODE == MODE_FWD3 || MODE == MODE_INV3) ? 256 * sizeof(unsigned) : 0);   // activity bits of the z-pass tiles
 }
 constexpr size_t SMEM_PER_CTA_MAX = 227 * 1024;  // sm_100a opt-in limit per CTA
 static_assert(ring_smem_bytes<32, MODE_SOLVE>() * 4 <= SMEM_PER_CTA_MAX + 4096 && ring_smem_bytes<64, MODE_SOLVE>() * 3 <= SMEM_PER_CTA_MAX &&
@@ -67,6 +68,11 @@ struct RingParams {
                          // MODE_FWD3 runs in place: the rows of an inactive plane in the output planes 0 and 1 are the zeros
                          // the splat pass wrote there; MODE_INV3's output there is never read
     const int* nact;     // {-, |ylist|, -, -}
+    // ... and inside an active plane the rows of the INACTIVE z-pass tiles (32 lines each) are neither written by the splat pass
+    // (MODE_FWD3 fetches whatever is there with the tile and its stage 0 reads those rows as zeros; fetching only the active
+    // rows with one 32-row box each was measured slower: 4 KB boxes, 8-16 per tile) nor stored by MODE_INV3 (the inverse z pass
+    // does not read them)
+    const unsigned* tile_bits;   // [units][N * (N / 32) / 32] activity bits of the z-pass tiles, bit x * (N / 32) + ty
 };
 
 // ---- PTX wrappers ---------------------------------------------------------------------------------------
@@ -115,8 +121,12 @@ namespace sap {
 // ---- in-place stages on a dense [N][W] tile; lanes run over the W columns -------------------------------
 // Stage S (S = 0 or the middle stage of a 3-stage plan).  tab = this stage's twiddle table for this direction.
 // swz = 15 for a y-pass tile of the main spectrum (row n holds z slot c in column c ^ (n & 15), see kz_swz), else 0.
+// 32-row group of tile row q + r ST (q < ST): rowmask bit of the z-pass tile (32 lines) the row belongs to
+template <int ST> __device__ __forceinline__ int ring_row_group(int q, int r) { return ((r * ST) >> 5) + (ST >= 32 ? (q >> 5) : 0); }
+// rowmask (y-pass tiles, listed mode): bit g set = rows [32 g, 32 g + 32) of the tile belong to an active z-pass tile; the
+// rows of the other groups are zeros that nobody wrote: stage 0 reads them as 0 whatever the buffer holds
 template <int N, int S, int W, int NTC, bool INV>
-__device__ __forceinline__ void ring_stage(float2* s, const float4* tab, int tid, int swz = 0) {
+__device__ __forceinline__ void ring_stage(float2* s, const float4* tab, int tid, int swz = 0, unsigned rowmask = 0xffffffffu) {
     constexpr int R = StageInfo<N, S>::R, ST = StageInfo<N, S>::ST;
     constexpr int NT = (N / R) * W;  // butterflies of the tile
 #pragma unroll
@@ -129,7 +139,10 @@ __device__ __forceinline__ void ring_stage(float2* s, const float4* tab, int tid
         const float4* tr = tab + j * R;
         float2 v[R];
 #pragma unroll
-        for (int r = 0; r < R; ++r) v[r] = s[(row0 + r * ST) * W + (c ^ ((row0 + r * ST) & swz))];
+        for (int r = 0; r < R; ++r) {
+            v[r] = s[(row0 + r * ST) * W + (c ^ ((row0 + r * ST) & swz))];
+            if (S == 0 && !INV && !((rowmask >> ring_row_group<ST>(j, r)) & 1u)) v[r] = make_float2(0.f, 0.f);
+        }
         if (!INV) {
             dft_fwd<R>(v);
             if constexpr (ST > 1) {
@@ -149,7 +162,8 @@ __device__ __forceinline__ void ring_stage(float2* s, const float4* tab, int tid
 }
 // inverse stage 0: smem -> registers -> HBM.  out + off(row n, column c) = out[n * sn + c * sc]
 template <int N, int W, int NTC>
-__device__ __forceinline__ void ring_stage0_inv_store(const float2* s, const float4* tab, int tid, float2* out, unsigned sn, unsigned sc, int swz = 0) {
+__device__ __forceinline__ void ring_stage0_inv_store(const float2* s, const float4* tab, int tid, float2* out, unsigned sn, unsigned sc, int swz = 0,
+                                                      unsigned rowmask = 0xffffffffu) {
     constexpr int R = StageInfo<N, 0>::R, ST = StageInfo<N, 0>::ST;
     constexpr int NT = ST * W;
 #pragma unroll
@@ -165,7 +179,8 @@ __device__ __forceinline__ void ring_stage0_inv_store(const float2* s, const flo
         for (int r = 1; r < R; ++r) v[r] = cmul4(v[r], tr[r]);
         dft_inv<R>(v);
 #pragma unroll
-        for (int r = 0; r < R; ++r) out[(unsigned)(q + r * ST) * sn + (unsigned)(c ^ ((q + r * ST) & swz)) * sc] = v[r];
+        for (int r = 0; r < R; ++r)
+            if ((rowmask >> ring_row_group<ST>(q, r)) & 1u) out[(unsigned)(q + r * ST) * sn + (unsigned)(c ^ ((q + r * ST) & swz)) * sc] = v[r];
     }
 }
 
@@ -199,7 +214,7 @@ __device__ __forceinline__ void ring_stage0_fwd2(float2* s1, const float2* s2, c
 // inverse stage 0 of a y-pass tile with a per-column output factor scale(c), c = z slot inside the tile
 template <int N, int W, int NTC, class F>
 __device__ __forceinline__ void ring_stage0_inv_store_scaled(const float2* s, const float4* tab, int tid, float2* out, unsigned sn,
-                                                             unsigned sc, int swz, F scale) {
+                                                             unsigned sc, int swz, F scale, unsigned rowmask = 0xffffffffu) {
     constexpr int R = StageInfo<N, 0>::R, ST = StageInfo<N, 0>::ST;
     constexpr int NT = ST * W;
 #pragma unroll
@@ -216,12 +231,13 @@ __device__ __forceinline__ void ring_stage0_inv_store_scaled(const float2* s, co
         for (int r = 1; r < R; ++r) v[r] = cmul4(v[r], tr[r]);
         dft_inv<R>(v);
 #pragma unroll
-        for (int r = 0; r < R; ++r) out[(unsigned)(q + r * ST) * sn + (unsigned)(c ^ ((q + r * ST) & swz)) * sc] = cscale(w, v[r]);
+        for (int r = 0; r < R; ++r)
+            if ((rowmask >> ring_row_group<ST>(q, r)) & 1u) out[(unsigned)(q + r * ST) * sn + (unsigned)(c ^ ((q + r * ST) & swz)) * sc] = cscale(w, v[r]);
     }
 }
 // forward stage 0 of a y-pass tile with a per-column input factor scale(c)
 template <int N, int W, int NTC, class F>
-__device__ __forceinline__ void ring_stage0_fwd_scaled(float2* s, const float4* tab, int tid, int swz, F scale) {
+__device__ __forceinline__ void ring_stage0_fwd_scaled(float2* s, const float4* tab, int tid, int swz, F scale, unsigned rowmask = 0xffffffffu) {
     constexpr int R = StageInfo<N, 0>::R, ST = StageInfo<N, 0>::ST;
     constexpr int NT = ST * W;
 #pragma unroll
@@ -233,7 +249,10 @@ __device__ __forceinline__ void ring_stage0_fwd_scaled(float2* s, const float4* 
         const float w = scale(c);
         float2 v[R];
 #pragma unroll
-        for (int r = 0; r < R; ++r) v[r] = cscale(w, s[(q + r * ST) * W + (c ^ ((q + r * ST) & swz))]);
+        for (int r = 0; r < R; ++r) {
+            v[r] = cscale(w, s[(q + r * ST) * W + (c ^ ((q + r * ST) & swz))]);
+            if (!((rowmask >> ring_row_group<ST>(q, r)) & 1u)) v[r] = make_float2(0.f, 0.f);
+        }
         dft_fwd<R>(v);
 #pragma unroll
         for (int r = 1; r < R; ++r) v[r] = cmul4(v[r], tr[r]);
@@ -298,6 +317,19 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
     pdl_wait();  // the tables above are constants of the handle; the spectra below are the predecessor's output
     const bool listed = CAN_LIST && p.ylist != nullptr;
     const long long total = listed ? (long long)p.nact[1] : (long long)p.units * tiles_per_unit;
+    // activity bits of the z-pass tiles (listed mode, N >= 256): cached when they fit, else read from global memory
+    constexpr int BITW = N * (N / 32) / 32;   // words per unit
+    unsigned* bits_s = reinterpret_cast<unsigned*>(tcache + TCAP);
+    const bool bits_cached = CAN_LIST && listed && (long long)p.units * BITW <= 256;
+    if (bits_cached)
+        for (int i = threadIdx.x; i < p.units * BITW; i += TCAP) bits_s[i] = p.tile_bits[i];
+    // rowmask of the y-pass tile of plane o: bit ty = z-pass tile (o, ty) is active
+    auto rowmask_of = [&](int unit, int o) -> unsigned {
+        constexpr int NTY = N / 32;
+        const int bit0 = o * NTY, w = unit * BITW + (bit0 >> 5);
+        const unsigned word = bits_cached ? bits_s[w] : p.tile_bits[w];
+        return (word >> (bit0 & 31)) & ((NTY >= 32) ? 0xffffffffu : ((1u << NTY) - 1u));
+    };
     if (CAN_LIST && listed) {
         const long long idx = (long long)blockIdx.x + (long long)threadIdx.x * gridDim.x;
         tcache[threadIdx.x] = idx < total ? p.ylist[REVERSED ? total - 1 - idx : idx] : -1;
@@ -321,10 +353,10 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
         if (g < 0) return;
         const int unit = (int)(g / tiles_per_unit), T = (int)(g - (long long)unit * tiles_per_unit);
         const int s = it % NSTAGE;
-        mbar_expect_tx(full + s, TILE_BYTES);
-        issued[s] = it / NSTAGE + 1;
         const int plane = unit * IN_STRIDE + ((MODE == MODE_INV3 && ch == 2) ? 1 : ch);  // INV3 fetches plane 1 twice
         const uint32_t dst = smem_u32(bufs + (size_t)s * TILE_ELEMS);
+        mbar_expect_tx(full + s, TILE_BYTES);
+        issued[s] = it / NSTAGE + 1;
         if (T < TILES_MAIN) {
             const int o = T / KT, kt = T - o * KT;
 #pragma unroll
@@ -375,6 +407,8 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
         const unsigned sn = (unsigned)d.sn, sc = (unsigned)d.sc;
         const int swz = (AXIS == 1 && !d.nyq) ? 15 : 0;  // y-pass tiles of the main spectrum: column swizzle per row
         const int xswz = (AXIS == 0 && !d.nyq) ? (d.other & 15) : 0;  // x-pass tile at y = d.other: one XOR for the tile
+        // listed 3-channel y passes: which 32-row groups of this tile exist (d.other = the plane x of a main tile)
+        const unsigned rowmask = (CAN_LIST && N >= 256 && listed && !d.nyq) ? rowmask_of(unit, d.other) : 0xffffffffu;
         auto out_tile = [&](int c) {  // first element of this tile in output channel c
             const size_t plane = (size_t)unit * OUT_CH + c;
             return (d.nyq ? p.outQ + plane * QPLANE : p.outS + plane * SPLANE) + d.base;
@@ -423,8 +457,8 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
 #pragma unroll
             for (int ch = 0; ch < 3; ++ch) {
                 float2* buf = acquire(it + ch);
-                if (ch == 2) ring_stage0_fwd_scaled<N, W, NTC>(buf, tabF, tid, swz, hz_of);
-                else ring_stage<N, 0, W, NTC, false>(buf, tabF, tid, swz);
+                if (ch == 2) ring_stage0_fwd_scaled<N, W, NTC>(buf, tabF, tid, swz, hz_of, rowmask);
+                else ring_stage<N, 0, W, NTC, false>(buf, tabF, tid, swz, rowmask);
                 consumer_sync<NTC>(group);
                 if constexpr (NS == 3) {
                     ring_stage<N, 1, W, NTC, false>(buf, tabF + N, tid, swz);
@@ -481,8 +515,8 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
                 // LANDED before plane 1 of this tile is overwritten (an issued bulk load is not ordered against later
                 // generic stores), so wait for the ch = 2 buffer's full barrier first.  It is a separate buffer: no cost.
                 if (ch == 1) acquire(it + 2);
-                if (ch < 2) ring_stage0_inv_store<N, W, NTC>(buf, tabI, tid, out_tile(ch), sn, sc, swz);
-                else ring_stage0_inv_store_scaled<N, W, NTC>(buf, tabI, tid, out_tile(2), sn, sc, swz, hz_of);
+                if (ch < 2) ring_stage0_inv_store<N, W, NTC>(buf, tabI, tid, out_tile(ch), sn, sc, swz, rowmask);
+                else ring_stage0_inv_store_scaled<N, W, NTC>(buf, tabI, tid, out_tile(2), sn, sc, swz, hz_of, rowmask);
                 release(it + ch);
             }
         } else if constexpr (MODE == MODE_SOLVE) {

@@ -92,6 +92,7 @@ struct ActLists {
     int* zlist;       // [B * nbins]
     int* ylist;       // [B * (N * KT + NYQT)]  (N >= 256)
     int* nact;        // [4]
+    unsigned* tile_bits;  // [B][nbins / 32] activity bits of the tiles, bit = bin index
     int N, NTY, KT, NYQT;  // KT = y-pass tiles per plane (0: no y pass), NYQT = Nyquist tiles per item
 };
 __device__ __forceinline__ int block_excl_scan_1024(int v, int* wsum, int& total) {
@@ -140,6 +141,7 @@ __device__ __forceinline__ void build_act_lists(const ActLists& al, int b, int n
     // active tiles: word w -> its set bits
     const int nwords = nbins >> 5;
     const unsigned myw = tid < nwords ? s_bits[tid] : 0u;
+    if (tid < nwords) al.tile_bits[(size_t)b * nwords + tid] = myw;
     int ztot;
     int zoff = block_excl_scan_1024(__popc(myw), wsum, ztot);
     if (tid == 0) s_base[0] = atomicAdd(al.nact + 0, ztot);
@@ -627,6 +629,7 @@ struct sap_dpsr {
     int* zlist = nullptr;      // [B * nbins]
     int* ylist = nullptr;      // [B * (N * KT + NYQT)] (N >= 256)
     int* nact = nullptr;       // [4]
+    unsigned* tile_bits = nullptr;  // [B][nbins / 32]
     bool sparse = true;        // use the lists (SAP_DENSE=1 in the environment of sap_dpsr_create: every tile is processed)
     bool lists_valid = false;  // the lists belong to the bins in the workspace (the latency path does not write them)
     // staging for the *_host entry points (allocated on first use)
@@ -840,6 +843,7 @@ template <int N> struct Runner {
         p.units = units; p.nyq_out_t = C::FUSED_ZY ? 0 : 1;
         const bool listed = (MODE == MODE_FWD3 || MODE == MODE_INV3) && h->sparse && h->lists_valid;
         p.ylist = listed ? h->ylist : nullptr; p.nact = h->nact;
+        p.tile_bits = h->tile_bits;
         p.cs = (float)((2.0 / ((double)N * N * N)) / (-2.0 * 3.14159265358979323846));
         const long long total = (long long)units * (N * (H / RC::W) + N / RC::W);
         long long grid = (long long)RC::MINB * h->num_sms;
@@ -939,7 +943,7 @@ template <int N> struct Runner {
             const dim3 gp((P + 255) / 256, B);
             constexpr int KT = C::FUSED_ZY ? 0 : H / RingCfg<N>::W, NYQT = C::FUSED_ZY ? 0 : N / RingCfg<N>::W;
             static_assert(C::FUSED_ZY || RingCfg<N>::W == 16, "ylist is sized for 16-column y-pass tiles");
-            const ActLists al{h->plane_act, h->sparse ? h->zlist : nullptr, h->ylist, h->nact, N, N / C::NL, KT, NYQT};
+            const ActLists al{h->plane_act, h->sparse ? h->zlist : nullptr, h->ylist, h->nact, h->tile_bits, N, N / C::NL, KT, NYQT};
             // one launch when every point fits the registers of a co-resident grid (BIN_PPT per thread), else three
             const int gx = (int)gp.x < h->bin_gx_max ? (int)gp.x : h->bin_gx_max;
             // (measured with one counter per 32-byte sector: 480,000 points 31 us against 48 us for the three kernels, 10^6 points
@@ -1083,7 +1087,7 @@ static void free_all(sap_dpsr* h) {
     cudaFree(h->v); cudaFree(h->spts); cudaFree(h->snrm); cudaFree(h->bin_cnt); cudaFree(h->bin_cursor); cudaFree(h->bin_start); cudaFree(h->S3); cudaFree(h->Q3); cudaFree(h->S1); cudaFree(h->Q1); cudaFree(h->QT3); cudaFree(h->QT1); cudaFree(h->tw); cudaFree(h->ftab);
     cudaFree(h->fhist); cudaFree(h->facc); cudaFree(h->fsync); cudaFree(h->fstamps);
     cudaFree(h->bsync);
-    cudaFree(h->plane_act); cudaFree(h->zlist); cudaFree(h->ylist); cudaFree(h->nact);
+    cudaFree(h->tile_bits); cudaFree(h->plane_act); cudaFree(h->zlist); cudaFree(h->ylist); cudaFree(h->nact);
     cudaFree(h->gmse); cudaFree(h->acc_mse); cudaFree(h->acc); cudaFree(h->ticket); cudaFree(h->stats); cudaFree(h->bw); cudaFree(h->nmax);
     cudaFree(h->h_pts); cudaFree(h->h_nrm); cudaFree(h->h_chi); cudaFree(h->h_gchi); cudaFree(h->h_gp); cudaFree(h->h_gn);
 }
@@ -1134,6 +1138,7 @@ extern "C" sap_status_t sap_dpsr_create(int N, float sigma, int batch, int max_p
         upd(dev_alloc(h, &h->zlist, B * (size_t)h->nbins));
         if (N >= 256) upd(dev_alloc(h, &h->ylist, B * ((size_t)N * (N / 2 / 16) + N / 16)));
         upd(dev_alloc(h, &h->nact, (size_t)4));
+        upd(dev_alloc(h, &h->tile_bits, B * (size_t)(h->nbins / 32)));
     }
     h->fused_ok = (N <= 128) && ((long long)batch * N <= h->num_sms) && batch <= (N == 32 ? 4 : N == 64 ? 2 : 1);
     if (h->fused_ok) {

@@ -85,9 +85,10 @@ __global__ void __launch_bounds__(ZwCfg<N>::NT, ZwCfg<N>::MINB) k_zw_fwd(const Z
         total += b_n[k];
     }
     if (SRC == SRC_SPLAT && total == 0) {  // nothing lands here: the spectrum of zeros is zeros
-        // inactive plane: the y pass (in place on channels 0 and 1) does not touch it and the x pass reads the zeros of
-        // channels 0 and 1 as the y pass's output; nobody reads channel 2
-        const bool skip_main = ch == 2 && p.plane_act && p.plane_act[(size_t)item * N + x] == 0;
+        // With the activity lists: in an ACTIVE plane the y pass fetches only the rows of the active tiles (it reads this one as
+        // zeros without anybody writing them); an INACTIVE plane is not touched by the y pass (in place on channels 0 and 1) and
+        // the x pass reads the zeros of channels 0 and 1 as the y pass's output -- nobody reads channel 2
+        const bool skip_main = p.plane_act && (p.plane_act[(size_t)item * N + x] != 0 || ch == 2);
         float4* So4 = reinterpret_cast<float4*>(So);
         if (!skip_main)
             for (int i = tid; i < NL * H / 2; i += NT) So4[i] = make_float4(0.f, 0.f, 0.f, 0.f);
