@@ -85,9 +85,9 @@ __global__ void __launch_bounds__(ZwCfg<N>::NT, ZwCfg<N>::MINB) k_zw_fwd(const Z
         total += b_n[k];
     }
     if (SRC == SRC_SPLAT && total == 0) {  // nothing lands here: the spectrum of zeros is zeros
-        // With the activity lists: in an ACTIVE plane the y pass fetches only the rows of the active tiles (it reads this one as
-        // zeros without anybody writing them); an INACTIVE plane is not touched by the y pass (in place on channels 0 and 1) and
-        // the x pass reads the zeros of channels 0 and 1 as the y pass's output -- nobody reads channel 2
+        // With the activity lists: in an ACTIVE plane the first stage of the y pass reads the rows of an inactive tile as zeros
+        // whatever the spectrum holds there (nobody has to write them); an INACTIVE plane is not touched by the y pass (in place
+        // on channels 0 and 1) and the x pass reads the zeros of channels 0 and 1 as the y pass's output -- nobody reads channel 2
         const bool skip_main = p.plane_act && (p.plane_act[(size_t)item * N + x] != 0 || ch == 2);
         float4* So4 = reinterpret_cast<float4*>(So);
         if (!skip_main)
