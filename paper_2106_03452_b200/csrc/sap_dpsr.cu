@@ -973,7 +973,7 @@ template <int N> struct Runner {
             if constexpr (C::FUSED_ZY)
                 launch_pdl(k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_SPLAT, C::NT_ZY>, dim3(N * N / C::NL, B * 3), dim3(C::NT_ZY), zy_smem_bytes<N, C::NL>(), st, p);
             else
-                launch_pdl(k_zw_fwd<N, SRC_SPLAT>, dim3(N * N / ZwCfg<N>::NL, B * 3), dim3(ZwCfg<N>::NT), ZwCfg<N>::SMEM, st, p);
+                launch_pdl(k_zw_fwd<N, SRC_SPLAT>, dim3(N * N / ZwCfg<N>::NL, B), dim3(ZwCfg<N>::NT), ZwCfg<N>::SMEM, st, p);
             SAP_LAUNCH_CHECK(h, C::FUSED_ZY ? "k_zy_fwd" : "k_zw_fwd<SPLAT>");
         }
         if constexpr (!C::FUSED_ZY) {

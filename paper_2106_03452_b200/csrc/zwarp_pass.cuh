@@ -56,17 +56,14 @@ __global__ void __launch_bounds__(ZwCfg<N>::NT, ZwCfg<N>::MINB) k_zw_fwd(const Z
     float2* tws = s + (size_t)NL * LP;   // [H]  split twiddles, halved: tws[k0 * 16 + j] = w_N^(k0 + R0 j) / 2
     float2* tw0 = tws + H;               // [(R0-1) * 16] stage-0 twiddles: tw0[(r-1) * 16 + q] = w_H^(r q)
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int bx = blockIdx.x, by = blockIdx.y;
+    const int bx = blockIdx.x, item = blockIdx.y;   // a CTA takes the p.nch channels of its tile one after the other
     pdl_wait();
-    if (SRC == SRC_SPLAT && p.clear_cnt && bx == 0 && by == 0) {
+    if (SRC == SRC_SPLAT && p.clear_cnt && bx == 0 && item == 0) {
         for (int i = tid; i < p.clear_n; i += NT) p.clear_cnt[i] = 0;
         if (tid == 0) p.clear_sync[0] = 0u;
     }
     const size_t V = (size_t)N * N * N;
     const size_t line0 = (size_t)bx * NL;  // global line index = x*N + y
-    float2* So = p.S + (size_t)by * ((size_t)N * N * H) + line0 * H;
-    float2* Qt = p.Q + (size_t)by * ((size_t)N * N);   // transposed Nyquist plane [y][x]
-    const int item = by / p.nch, ch = by - item * p.nch;
     const int x = (int)(line0 / N), y0 = (int)(line0 % N), ty = y0 / NL;
     if (SRC == SRC_GBAR) {   // pull the tile of G (32 KB, contiguous) towards L2 while the points are rasterised
         const char* g = reinterpret_cast<const char*>(p.G + (size_t)item * V + line0 * N);
@@ -84,6 +81,19 @@ __global__ void __launch_bounds__(ZwCfg<N>::NT, ZwCfg<N>::MINB) k_zw_fwd(const Z
         b_n[k] = bs[bin + 1] - b_lo[k];
         total += b_n[k];
     }
+    // the bins, the tables and the fixed-point scale are the same for every channel of the tile (the points come from L1
+    // the second and third time)
+    if (total > 0 || SRC == SRC_GBAR) {
+        for (int i = tid; i < H; i += NT) { const float2 w = p.tw[(i >> 4) + R0 * (i & 15)]; tws[i] = make_float2(0.5f * w.x, 0.5f * w.y); }
+        for (int i = tid; i < (R0 - 1) * 16; i += NT) tw0[i] = p.tw[2 * ((i >> 4) + 1) * (i & 15)];
+    }
+    const int lw = warp * LPW;
+    const int hw = lane >> 4, j = lane & 15;
+#pragma unroll 1
+    for (int ch = 0; ch < p.nch; ++ch) {
+    const int by = item * p.nch + ch;
+    float2* So = p.S + (size_t)by * ((size_t)N * N * H) + line0 * H;
+    float2* Qt = p.Q + (size_t)by * ((size_t)N * N);   // transposed Nyquist plane [y][x]
     if (SRC == SRC_SPLAT && total == 0) {  // nothing lands here: the spectrum of zeros is zeros
         // With the activity lists: in an ACTIVE plane the first stage of the y pass reads the rows of an inactive tile as zeros
         // whatever the spectrum holds there (nobody has to write them); an INACTIVE plane is not touched by the y pass (in place
@@ -93,11 +103,9 @@ __global__ void __launch_bounds__(ZwCfg<N>::NT, ZwCfg<N>::MINB) k_zw_fwd(const Z
         if (!skip_main)
             for (int i = tid; i < NL * H / 2; i += NT) So4[i] = make_float4(0.f, 0.f, 0.f, 0.f);
         for (int l = tid; l < NL; l += NT) Qt[(size_t)(y0 + l) * N + x] = make_float2(0.f, 0.f);
-        return;
+        continue;
     }
-    // tables, zero fill
-    for (int i = tid; i < H; i += NT) { const float2 w = p.tw[(i >> 4) + R0 * (i & 15)]; tws[i] = make_float2(0.5f * w.x, 0.5f * w.y); }
-    for (int i = tid; i < (R0 - 1) * 16; i += NT) tw0[i] = p.tw[2 * ((i >> 4) + 1) * (i & 15)];
+    if (ch > 0) __syncthreads();   // every warp is done with the previous channel's tile
     // GBAR tile that no point can touch: W = 0 there, Gbar' = s G (- the delta term) straight from HBM: no zero fill, no
     // rasterisation, one barrier less
     const bool has_pts = total > 0;
@@ -148,8 +156,6 @@ __global__ void __launch_bounds__(ZwCfg<N>::NT, ZwCfg<N>::MINB) k_zw_fwd(const Z
     }
     __syncthreads();
     // ---- from here on a warp works on its own LPW lines ----
-    const int lw = warp * LPW;
-    const int hw = lane >> 4, j = lane & 15;
     // stage 0 (radix R0, stride 16): task = (line, q), q = lane & 15; fixed point -> float (GBAR: combined with G) on the way in
     {
         float cs_ = 0.f, cw = 0.f, c0 = 0.f;
@@ -266,6 +272,7 @@ __global__ void __launch_bounds__(ZwCfg<N>::NT, ZwCfg<N>::MINB) k_zw_fwd(const Z
             }
         }
     }
+    }   // channels
 }
 
 }  // namespace sap
