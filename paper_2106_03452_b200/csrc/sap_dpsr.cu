@@ -69,13 +69,14 @@ __device__ __forceinline__ int bin_key(const float* __restrict__ c, int N, int N
     const int jx = (int)floorf(c[0] * (float)N) & M, jy = (int)floorf(c[1] * (float)N) & M;
     return jx * (N / NL) + jy / NL;
 }
+constexpr int BIN_CS = 8;    // one bin counter / cursor per 32-byte sector (atomics to one 128-byte line serialise in L2)
 __global__ void k_bin_count(const float* __restrict__ pts, int P, int N, int NL, int nbins, int* __restrict__ cnt,
                             int* __restrict__ nact) {
     pdl_wait();
     const int i = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y;
     if (i == 0 && b == 0) { nact[0] = 0; nact[1] = 0; nact[2] = 0; nact[3] = 0; }  // lengths of the active-tile lists (k_bin_scan appends)
     if (i >= P) return;
-    atomicAdd(cnt + (size_t)b * nbins + bin_key(pts + ((size_t)b * P + i) * 3, N, NL), 1);
+    atomicAdd(cnt + ((size_t)b * nbins + bin_key(pts + ((size_t)b * P + i) * 3, N, NL)) * BIN_CS, 1);
 }
 // one block per item: exclusive scan of the counts -> start[nbins+1]; cursor = start; counts reset to 0
 // Activity lists ("nobody computes what nobody reads").  A tile (x, ty) = the NL z-lines y in [ty NL, (ty+1) NL) of plane x is
@@ -184,13 +185,16 @@ __global__ void k_bin_scan(int* __restrict__ cnt, int nbins, int P, int* __restr
     if (threadIdx.x == 0) nmax[blockIdx.x] = 0u;   // k_bin_scatter (the next launch) takes the max of |n| into it
     __shared__ int wsum[32];
     const int b = blockIdx.x, tid = threadIdx.x, nt = blockDim.x;
-    int* c = cnt + (size_t)b * nbins;
+    int* c = cnt + (size_t)b * nbins * BIN_CS;
     int* st = start + (size_t)b * (nbins + 1);
-    int* cu = cursor + (size_t)b * nbins;
+    int* cu = cursor + (size_t)b * nbins * BIN_CS;
+    extern __shared__ int s_cnt[];   // [nbins] the counts, fetched with independent loads (one sector each) and cleared
+    for (int i = tid; i < nbins; i += nt) { s_cnt[i] = c[i * BIN_CS]; c[i * BIN_CS] = 0; }
+    __syncthreads();
     const int per = (nbins + nt - 1) / nt;
     const int lo = tid * per, hi = min(lo + per, nbins);
     int local = 0;
-    for (int i = lo; i < hi; ++i) local += c[i];
+    for (int i = lo; i < hi; ++i) local += s_cnt[i];
     int incl = local;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
@@ -211,10 +215,9 @@ __global__ void k_bin_scan(int* __restrict__ cnt, int nbins, int P, int* __restr
     __syncthreads();
     int run = incl - local + ((tid >> 5) ? wsum[(tid >> 5) - 1] : 0);
     for (int i = lo; i < hi; ++i) {
-        const int n = c[i];
+        const int n = s_cnt[i];
         st[i] = run;
-        cu[i] = run;
-        c[i] = 0;
+        cu[i * BIN_CS] = run;
         run += n;
     }
     if (tid == 0) st[nbins] = P;
@@ -235,7 +238,6 @@ struct BinSortParams {
     unsigned* bsync; // [3] arrivals, -, time-out flag
     ActLists al;
 };
-constexpr int BIN_CS = 8;    // k_bin_sort keeps one counter per 32-byte sector (atomics to one 128-byte line serialise in L2)
 constexpr int BIN_PPT = 8;   // points per thread of k_bin_sort; bin and rank stay in registers across the barrier
 __global__ void __launch_bounds__(256, 6) k_bin_sort(const BinSortParams p) {
     extern __shared__ int s_start[];   // [nbins + 1]
@@ -354,7 +356,7 @@ __global__ void k_bin_scatter(const float* __restrict__ pts, const float* __rest
     if (i < P) {
         const float* c = pts + ((size_t)b * P + i) * 3;
         const float* n = nrm + ((size_t)b * P + i) * 3;
-        const int pos = atomicAdd(cursor + (size_t)b * nbins + bin_key(c, N, NL), 1);
+        const int pos = atomicAdd(cursor + ((size_t)b * nbins + bin_key(c, N, NL)) * BIN_CS, 1);
         spts[(size_t)b * P + pos] = make_float4(c[0], c[1], c[2], __int_as_float(i));  // .w: index in the caller's order
         snrm[(size_t)b * P + pos] = make_float4(n[0], n[1], n[2], 0.f);
         amax = __float_as_uint(fmaxf(fmaxf(fabsf(n[0]), fabsf(n[1])), fabsf(n[2])));
@@ -957,7 +959,7 @@ template <int N> struct Runner {
             } else {
                 launch_pdl(k_bin_count, dim3(gp), dim3(256), 0, st, pts, P, N, C::NL, h->nbins, h->bin_cnt, h->nact);
                 SAP_LAUNCH_CHECK(h, "k_bin_count");
-                launch_pdl(k_bin_scan, dim3(B), dim3(1024), 0, st, h->bin_cnt, h->nbins, P, h->bin_start, h->bin_cursor, h->nmax);
+                launch_pdl(k_bin_scan, dim3(B), dim3(1024), (size_t)h->nbins * sizeof(int), st, h->bin_cnt, h->nbins, P, h->bin_start, h->bin_cursor, h->nmax);
                 SAP_LAUNCH_CHECK(h, "k_bin_scan");
                 launch_pdl(k_bin_scatter, dim3(gp.x + 1, B), dim3(256), (size_t)(h->nbins + 1) * sizeof(int), st, pts, nrm, P, N, C::NL, h->nbins, h->bin_cursor,
                            h->spts, h->snrm, h->nmax, (const int*)h->bin_start, al);
@@ -1116,7 +1118,7 @@ extern "C" sap_status_t sap_dpsr_create(int N, float sigma, int batch, int max_p
     upd(dev_alloc(h, &h->spts, B * (size_t)max_points));
     upd(dev_alloc(h, &h->snrm, B * (size_t)max_points));
     upd(dev_alloc(h, &h->bin_cnt, B * (size_t)h->nbins * BIN_CS));
-    upd(dev_alloc(h, &h->bin_cursor, B * (size_t)h->nbins));
+    upd(dev_alloc(h, &h->bin_cursor, B * (size_t)h->nbins * BIN_CS));
     upd(dev_alloc(h, &h->bin_start, B * (size_t)(h->nbins + 1)));
     upd(dev_alloc(h, &h->bsync, (size_t)4));
     upd(dev_alloc(h, &h->S3, B * 3 * SP));
