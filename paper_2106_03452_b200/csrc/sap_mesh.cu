@@ -418,6 +418,48 @@ __global__ void __launch_bounds__(256) k_nn_brute(const float* __restrict__ q, i
     if (live) { nn[i] = bi; d2out[i] = (bi >= 0) ? best : 0.f; }
 }
 
+// The same search with the TARGETS split into gridDim.y chunks as well (few queries against many targets -- 20,000 input
+// points against 100,000 mesh vertices -- would leave most SMs idle with one block per 256 queries).  A block keeps the
+// best of its chunk per query and merges it with atomicMin on the 64-bit key (distance bits << 32 | index): distances are
+// non-negative floats, so the keys order like (distance, index) and the lowest index still wins an exact tie.  keys must
+// be all ones on entry; k_nn_finish unpacks them.
+__global__ void __launch_bounds__(256) k_nn_brute_chunks(const float* __restrict__ q, int nq, const int* nq_dev, const float* __restrict__ t, int nt,
+                                                         const int* nt_dev, unsigned long long* __restrict__ keys) {
+    __shared__ float4 tile[BF_TILE];
+    const int n_q = count_of(nq, nq_dev), n_t = count_of(nt, nt_dev);
+    if ((int)(blockIdx.x * blockDim.x) >= n_q) return;
+    const int ntiles = (n_t + BF_TILE - 1) / BF_TILE, per = (ntiles + (int)gridDim.y - 1) / (int)gridDim.y;
+    const int t_lo = (int)blockIdx.y * per * BF_TILE, t_hi = min(n_t, t_lo + per * BF_TILE);
+    if (t_lo >= t_hi) return;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const bool live = i < n_q;
+    const float px = live ? q[3 * i] : 0.f, py = live ? q[3 * i + 1] : 0.f, pz = live ? q[3 * i + 2] : 0.f;
+    float best = INFINITY;
+    int bi = -1;
+    for (int t0 = t_lo; t0 < t_hi; t0 += BF_TILE) {
+        const int m = min(BF_TILE, t_hi - t0);
+        __syncthreads();
+        for (int k = threadIdx.x; k < m; k += blockDim.x) tile[k] = make_float4(t[3 * (t0 + k)], t[3 * (t0 + k) + 1], t[3 * (t0 + k) + 2], 0.f);
+        __syncthreads();
+#pragma unroll 8
+        for (int k = 0; k < m; ++k) {
+            const float4 c = tile[k];
+            const float dx = px - c.x, dy = py - c.y, dz = pz - c.z;
+            const float d = dx * dx + dy * dy + dz * dz;
+            if (d < best) { best = d; bi = t0 + k; }
+        }
+    }
+    if (live && bi >= 0) atomicMin(keys + i, ((unsigned long long)__float_as_uint(best) << 32) | (unsigned)bi);
+}
+__global__ void k_nn_finish(const unsigned long long* __restrict__ keys, int nq, const int* nq_dev, int* __restrict__ nn, float* __restrict__ d2out) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= count_of(nq, nq_dev)) return;
+    const unsigned long long k = keys[i];
+    const bool found = k != ~0ull;
+    nn[i] = found ? (int)(unsigned)(k & 0xffffffffull) : -1;
+    d2out[i] = found ? __uint_as_float((unsigned)(k >> 32)) : 0.f;
+}
+
 __device__ __forceinline__ float block_sum_f(float x, float* sh) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
@@ -495,6 +537,8 @@ struct sap_mesh {
     float* d2_a = nullptr;               // [max_p]
     float* d2_b = nullptr;               // [max_p]
     double* lacc = nullptr;              // [1]
+    unsigned long long* nn_keys = nullptr;  // [max_p] (distance, index) keys of the chunked exhaustive search
+    int num_sms = 148;
     bool extracted = false;
     size_t ws_bytes = 0;
     std::string err;
@@ -517,7 +561,7 @@ template <class T> static cudaError_t alloc(sap_mesh* h, T** p, size_t n) {
 static void free_all(sap_mesh* h) {
     cudaFree(h->code); cudaFree(h->cfg); cudaFree(h->blocksum); cudaFree(h->vprefix); cudaFree(h->tprefix); cudaFree(h->vt);
     cudaFree(h->counts_dev); cudaFree(h->cell_cnt); cudaFree(h->cell_start); cudaFree(h->cell_cursor); cudaFree(h->sorted);
-    cudaFree(h->nn_tmp_a); cudaFree(h->nn_tmp_b); cudaFree(h->d2_a); cudaFree(h->d2_b); cudaFree(h->lacc);
+    cudaFree(h->nn_tmp_a); cudaFree(h->nn_tmp_b); cudaFree(h->d2_a); cudaFree(h->d2_b); cudaFree(h->lacc); cudaFree(h->nn_keys);
 }
 static sap_status_t check(sap_mesh* h) {
     if (!h) return SAP_ERR_INVALID_ARG;
@@ -571,6 +615,8 @@ extern "C" sap_status_t sap_mesh_create(int N, int max_vertices, int max_triangl
     upd(alloc(h, &h->nn_tmp_a, (size_t)max_points)); upd(alloc(h, &h->nn_tmp_b, (size_t)max_points));
     upd(alloc(h, &h->d2_a, (size_t)max_points)); upd(alloc(h, &h->d2_b, (size_t)max_points));
     upd(alloc(h, &h->lacc, (size_t)1));
+    upd(alloc(h, &h->nn_keys, (size_t)max_points));
+    h->num_sms = prop.multiProcessorCount;
     if (e == cudaSuccess) upd(cudaMemset(h->lacc, 0, sizeof(double)));
     if (e == cudaSuccess) upd(cudaMemset(h->cell_cnt, 0, sizeof(int) * C));
     if (e == cudaSuccess) upd(cudaMemset(h->counts_dev, 0, 2 * sizeof(int)));
@@ -637,11 +683,26 @@ extern "C" sap_status_t sap_chamfer(sap_mesh_t* h, const float* a, int na, const
     // exhaustive search while the number of pairs is moderate (na is the capacity when the count lives on the device)
     const bool brute = h->nn_mode == SAP_NN_BRUTE || (h->nn_mode == SAP_NN_AUTO && (double)na * (double)nb <= 2.0e10);
     if (brute) {
-        k_nn_brute<<<ga, 256, 0, s>>>(a, na, na_dev, b, nb, nullptr, nna, h->d2_a);
+        // one block per 256 queries; when that leaves SMs idle the targets are split over gridDim.y chunks as well
+        auto nn_brute = [&](const float* q, int nq, const int* nq_dev, int gq, const float* t, int nt, const int* nt_dev, int* nn, float* d2) -> bool {
+            const int ntiles = (nt + BF_TILE - 1) / BF_TILE;
+            int chunks = (6 * h->num_sms + gq - 1) / gq;
+            if (chunks > ntiles) chunks = ntiles;
+            if (chunks <= 1) {
+                k_nn_brute<<<gq, 256, 0, s>>>(q, nq, nq_dev, t, nt, nt_dev, nn, d2);
+                return cudaGetLastError() == cudaSuccess;
+            }
+            if (cudaMemsetAsync(h->nn_keys, 0xff, sizeof(unsigned long long) * (size_t)nq, s) != cudaSuccess) return false;
+            k_nn_brute_chunks<<<dim3(gq, chunks), 256, 0, s>>>(q, nq, nq_dev, t, nt, nt_dev, h->nn_keys);
+            k_nn_finish<<<gq, 256, 0, s>>>(h->nn_keys, nq, nq_dev, nn, d2);
+            h->launches += 1;
+            return cudaGetLastError() == cudaSuccess;
+        };
+        if (!nn_brute(a, na, na_dev, ga, b, nb, nullptr, nna, h->d2_a)) { ok(h, cudaGetLastError(), "k_nn_brute"); h->err = "k_nn_brute launch failed"; return SAP_ERR_CUDA; }
         MESH_LAUNCH_CHECK(h, "k_nn_brute");
         k_chamfer_a<<<ga, 256, 0, s>>>(a, na, na_dev, b, nna, h->d2_a, grad_a, h->lacc);
         MESH_LAUNCH_CHECK(h, "k_chamfer_a");
-        k_nn_brute<<<gb, 256, 0, s>>>(b, nb, nullptr, a, na, na_dev, nnb, h->d2_b);
+        if (!nn_brute(b, nb, nullptr, gb, a, na, na_dev, nnb, h->d2_b)) { h->err = "k_nn_brute launch failed"; return SAP_ERR_CUDA; }
         MESH_LAUNCH_CHECK(h, "k_nn_brute");
         k_chamfer_b<<<gb, 256, 0, s>>>(a, na, na_dev, b, nb, nnb, h->d2_b, grad_a, h->lacc);
         MESH_LAUNCH_CHECK(h, "k_chamfer_b");
