@@ -392,9 +392,37 @@ __global__ void k_nn_query(const float* __restrict__ q, int nq, const int* nq_de
 // still far from the cloud (the ring search then walks thousands of empty cells per query).  Targets are visited in
 // index order and a candidate must be strictly closer, so the lowest index wins an exact tie.
 constexpr int BF_TILE = 1024;
+// A tile holds the targets two by two: tile[3 k2 .. 3 k2 + 2] = (x, x'), (y, y'), (z, z') of targets 2 k2 and 2 k2 + 1, so that the
+// three differences, the square and the two fused multiply-adds of a PAIR of targets are six packed FP32x2 instructions; the
+// two candidates are then examined in index order (strictly closer wins: the lowest index keeps an exact tie).  The sum is
+// formed as fma(dz, dz, fma(dy, dy, dx dx)), what the scalar expression dx dx + dy dy + dz dz contracts to.
+__device__ __forceinline__ void bf_fill_tile(float2* tile, const float* __restrict__ t, int t0, int m) {
+    for (int k2 = threadIdx.x; 2 * k2 < m; k2 += blockDim.x) {
+        const int k = 2 * k2;
+        const bool two = k + 1 < m;   // an odd tail gets a far-away partner that can never win
+        const float* a = t + 3 * (size_t)(t0 + k);
+        tile[3 * k2 + 0] = make_float2(a[0], two ? a[3] : 3.0e18f);
+        tile[3 * k2 + 1] = make_float2(a[1], two ? a[4] : 3.0e18f);
+        tile[3 * k2 + 2] = make_float2(a[2], two ? a[5] : 3.0e18f);
+    }
+}
+__device__ __forceinline__ void bf_scan_tile(const float2* tile, int m, int t0, float px, float py, float pz, float& best, int& bi) {
+    const float2 px2 = make_float2(px, px), py2 = make_float2(py, py), pz2 = make_float2(pz, pz);
+    const int m2 = (m + 1) >> 1;
+#pragma unroll 4
+    for (int k2 = 0; k2 < m2; ++k2) {
+        const float2 cx = tile[3 * k2], cy = tile[3 * k2 + 1], cz = tile[3 * k2 + 2];
+        const float2 dx = __fadd2_rn(px2, make_float2(-cx.x, -cx.y));
+        const float2 dy = __fadd2_rn(py2, make_float2(-cy.x, -cy.y));
+        const float2 dz = __fadd2_rn(pz2, make_float2(-cz.x, -cz.y));
+        const float2 d = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
+        if (d.x < best) { best = d.x; bi = t0 + 2 * k2; }
+        if (d.y < best) { best = d.y; bi = t0 + 2 * k2 + 1; }
+    }
+}
 __global__ void __launch_bounds__(256) k_nn_brute(const float* __restrict__ q, int nq, const int* nq_dev, const float* __restrict__ t, int nt,
                                                   const int* nt_dev, int* __restrict__ nn, float* __restrict__ d2out) {
-    __shared__ float4 tile[BF_TILE];
+    __shared__ float2 tile[3 * BF_TILE / 2];
     const int n_q = count_of(nq, nq_dev), n_t = count_of(nt, nt_dev);
     if ((int)(blockIdx.x * blockDim.x) >= n_q) return;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -405,15 +433,9 @@ __global__ void __launch_bounds__(256) k_nn_brute(const float* __restrict__ q, i
     for (int t0 = 0; t0 < n_t; t0 += BF_TILE) {
         const int m = min(BF_TILE, n_t - t0);
         __syncthreads();
-        for (int k = threadIdx.x; k < m; k += blockDim.x) tile[k] = make_float4(t[3 * (t0 + k)], t[3 * (t0 + k) + 1], t[3 * (t0 + k) + 2], 0.f);
+        bf_fill_tile(tile, t, t0, m);
         __syncthreads();
-#pragma unroll 8
-        for (int k = 0; k < m; ++k) {
-            const float4 c = tile[k];
-            const float dx = px - c.x, dy = py - c.y, dz = pz - c.z;
-            const float d = dx * dx + dy * dy + dz * dz;
-            if (d < best) { best = d; bi = t0 + k; }
-        }
+        bf_scan_tile(tile, m, t0, px, py, pz, best, bi);
     }
     if (live) { nn[i] = bi; d2out[i] = (bi >= 0) ? best : 0.f; }
 }
@@ -425,7 +447,7 @@ __global__ void __launch_bounds__(256) k_nn_brute(const float* __restrict__ q, i
 // be all ones on entry; k_nn_finish unpacks them.
 __global__ void __launch_bounds__(256) k_nn_brute_chunks(const float* __restrict__ q, int nq, const int* nq_dev, const float* __restrict__ t, int nt,
                                                          const int* nt_dev, unsigned long long* __restrict__ keys) {
-    __shared__ float4 tile[BF_TILE];
+    __shared__ float2 tile[3 * BF_TILE / 2];
     const int n_q = count_of(nq, nq_dev), n_t = count_of(nt, nt_dev);
     if ((int)(blockIdx.x * blockDim.x) >= n_q) return;
     const int ntiles = (n_t + BF_TILE - 1) / BF_TILE, per = (ntiles + (int)gridDim.y - 1) / (int)gridDim.y;
@@ -439,15 +461,9 @@ __global__ void __launch_bounds__(256) k_nn_brute_chunks(const float* __restrict
     for (int t0 = t_lo; t0 < t_hi; t0 += BF_TILE) {
         const int m = min(BF_TILE, t_hi - t0);
         __syncthreads();
-        for (int k = threadIdx.x; k < m; k += blockDim.x) tile[k] = make_float4(t[3 * (t0 + k)], t[3 * (t0 + k) + 1], t[3 * (t0 + k) + 2], 0.f);
+        bf_fill_tile(tile, t, t0, m);
         __syncthreads();
-#pragma unroll 8
-        for (int k = 0; k < m; ++k) {
-            const float4 c = tile[k];
-            const float dx = px - c.x, dy = py - c.y, dz = pz - c.z;
-            const float d = dx * dx + dy * dy + dz * dz;
-            if (d < best) { best = d; bi = t0 + k; }
-        }
+        bf_scan_tile(tile, m, t0, px, py, pz, best, bi);
     }
     if (live && bi >= 0) atomicMin(keys + i, ((unsigned long long)__float_as_uint(best) << 32) | (unsigned)bi);
 }
