@@ -487,7 +487,7 @@ def _run_sparse_dense(N, sigma, pts, nrm, G):
     return out
 
 
-@pytest.mark.parametrize("N,B,P", [(64, 2, 2500), (128, 3, 4000), (256, 1, 12000)])
+@pytest.mark.parametrize("N,B,P", [(64, 2, 2500), (128, 3, 4000), (256, 1, 12000), (256, 2, 6000)])
 def test_activity_lists_leave_results_unchanged(N, B, P):
     # items with very different activity: a small blob wrapping around the cube corner, a blob in the middle, a full-size shape
     pts = np.empty((B, P, 3), np.float32)
