@@ -73,6 +73,9 @@ struct RingParams {
     // rows with one 32-row box each was measured slower: 4 KB boxes, 8-16 per tile) nor stored by MODE_INV3 (the inverse z pass
     // does not read them)
     const unsigned* tile_bits;   // [units][N * (N / 32) / 32] activity bits of the z-pass tiles, bit x * (N / 32) + ty
+    // MODE_SOLVE of the fused planes (N <= 128) in the throughput regime (sap_dpsr.cu decides), else nullptr: the splat pass
+    // has not written the zeros of the inactive planes, the solve reads those rows as zeros (xrow_masks)
+    const unsigned* plane_bits;  // [units][N / 32] activity bits of the x-planes
 };
 
 // ---- PTX wrappers ---------------------------------------------------------------------------------------
@@ -125,8 +128,28 @@ namespace sap {
 template <int ST> __device__ __forceinline__ int ring_row_group(int q, int r) { return ((r * ST) >> 5) + (ST >= 32 ? (q >> 5) : 0); }
 // rowmask (y-pass tiles, listed mode): bit g set = rows [32 g, 32 g + 32) of the tile belong to an active z-pass tile; the
 // rows of the other groups are zeros that nobody wrote: stage 0 reads them as 0 whatever the buffer holds
+// x-pass tiles of the solve (rows = x-planes) with the plane masks on: bit r of xm[i] says whether row q + r ST of the thread's
+// i-th stage-0 task lies in an ACTIVE plane.  The rows of inactive planes are zeros that the splat pass did not write: stage 0
+// reads them as 0 whatever the tile holds.  pw = the unit's N/32 plane-activity words.
+template <int N, int W, int NTC>
+__device__ __forceinline__ void xrow_masks(const unsigned* __restrict__ pw, int tid, unsigned (&xm)[2]) {
+    constexpr int R = StageInfo<N, 0>::R, ST = StageInfo<N, 0>::ST, NT = ST * W;
+    static_assert((NT + NTC - 1) / NTC <= 2, "at most two stage-0 tasks per thread");
+#pragma unroll
+    for (int i = 0; i < (NT + NTC - 1) / NTC; ++i) {
+        const int q = (tid + i * NTC) / W;
+        unsigned m = 0u;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int x = (q + r * ST) & (N - 1);
+            m |= ((__ldg(pw + (x >> 5)) >> (x & 31)) & 1u) << r;
+        }
+        xm[i] = m;
+    }
+}
 template <int N, int S, int W, int NTC, bool INV>
-__device__ __forceinline__ void ring_stage(float2* s, const float4* tab, int tid, int swz = 0, unsigned rowmask = 0xffffffffu) {
+__device__ __forceinline__ void ring_stage(float2* s, const float4* tab, int tid, int swz = 0, unsigned rowmask = 0xffffffffu,
+                                           const unsigned* xm = nullptr) {
     constexpr int R = StageInfo<N, S>::R, ST = StageInfo<N, S>::ST;
     constexpr int NT = (N / R) * W;  // butterflies of the tile
 #pragma unroll
@@ -142,6 +165,7 @@ __device__ __forceinline__ void ring_stage(float2* s, const float4* tab, int tid
         for (int r = 0; r < R; ++r) {
             v[r] = s[(row0 + r * ST) * W + (c ^ ((row0 + r * ST) & swz))];
             if (S == 0 && !INV && !((rowmask >> ring_row_group<ST>(j, r)) & 1u)) v[r] = make_float2(0.f, 0.f);
+            if (S == 0 && !INV && xm && !((xm[i] >> r) & 1u)) v[r] = make_float2(0.f, 0.f);
         }
         if (!INV) {
             dft_fwd<R>(v);
@@ -192,7 +216,8 @@ namespace sap {
 // factors of the divergence (and of the adjoint) do not depend on x, so they commute with the transform along x:
 // sum_c h_c v~_c needs two forward x transforms, not three (and the adjoint two inverse ones).
 template <int N, int W, int NTC>
-__device__ __forceinline__ void ring_stage0_fwd2(float2* s1, const float2* s2, const float4* tab, int tid, float wy, float wz) {
+__device__ __forceinline__ void ring_stage0_fwd2(float2* s1, const float2* s2, const float4* tab, int tid, float wy, float wz,
+                                                 const unsigned* xm = nullptr) {
     constexpr int R = StageInfo<N, 0>::R, ST = StageInfo<N, 0>::ST;
     constexpr int NT = ST * W;
 #pragma unroll
@@ -203,7 +228,10 @@ __device__ __forceinline__ void ring_stage0_fwd2(float2* s1, const float2* s2, c
         const float4* tr = tab + q * R;
         float2 v[R];
 #pragma unroll
-        for (int r = 0; r < R; ++r) v[r] = caxpy(wz, s2[(q + r * ST) * W + c], cscale(wy, s1[(q + r * ST) * W + c]));
+        for (int r = 0; r < R; ++r) {
+            v[r] = caxpy(wz, s2[(q + r * ST) * W + c], cscale(wy, s1[(q + r * ST) * W + c]));
+            if (xm && !((xm[i] >> r) & 1u)) v[r] = make_float2(0.f, 0.f);
+        }
         dft_fwd<R>(v);
 #pragma unroll
         for (int r = 1; r < R; ++r) v[r] = cmul4(v[r], tr[r]);
@@ -409,6 +437,10 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
         const int xswz = (AXIS == 0 && !d.nyq) ? (d.other & 15) : 0;  // x-pass tile at y = d.other: one XOR for the tile
         // listed 3-channel y passes: which 32-row groups of this tile exist (d.other = the plane x of a main tile)
         const unsigned rowmask = (CAN_LIST && N >= 256 && listed && !d.nyq) ? rowmask_of(unit, d.other) : 0xffffffffu;
+        unsigned xmv[2] = {0xffffffffu, 0xffffffffu};
+        const bool xmasked = MODE == MODE_SOLVE && N <= 128 && p.plane_bits != nullptr && !d.nyq;
+        if (MODE == MODE_SOLVE && N <= 128 && xmasked) xrow_masks<N, W, NTC>(p.plane_bits + (size_t)unit * (N / 32), tid, xmv);
+        const unsigned* xm = xmasked ? xmv : nullptr;
         auto out_tile = [&](int c) {  // first element of this tile in output channel c
             const size_t plane = (size_t)unit * OUT_CH + c;
             return (d.nyq ? p.outQ + plane * QPLANE : p.outS + plane * SPLANE) + d.base;
@@ -530,7 +562,7 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
             (void)acc;
             constexpr bool SIDE = NSTAGE >= 2 * 3;  // the ring can hold whole tiles and still prefetch
             float2* b0 = acquire(it);
-            ring_stage<N, 0, W, NTC, false>(b0, tabF, tid);
+            ring_stage<N, 0, W, NTC, false>(b0, tabF, tid, 0, 0xffffffffu, xm);
             if constexpr (!SIDE) {  // N = 512: finish the x channel and hand its buffer back first
                 consumer_sync<NTC>(group);
                 if constexpr (NS == 3) {
@@ -555,7 +587,7 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
                 consumer_sync<NTC>(group);
             } else {
                 float2* b2 = acquire(it + 2);
-                ring_stage0_fwd2<N, W, NTC>(b1, b2, tabF, tid, ey.x, ez.x);
+                ring_stage0_fwd2<N, W, NTC>(b1, b2, tabF, tid, ey.x, ez.x, xm);
                 consumer_sync<NTC>(group);
                 release(it + 2);  // the z channel has been folded into b1
             }

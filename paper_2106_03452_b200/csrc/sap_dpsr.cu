@@ -94,6 +94,7 @@ struct ActLists {
     int* ylist;       // [B * (N * KT + NYQT)]  (N >= 256)
     int* nact;        // [4]
     unsigned* tile_bits;  // [B][nbins / 32] activity bits of the tiles, bit = bin index
+    unsigned* plane_bits; // [B][N / 32] activity bits of the planes
     int N, NTY, KT, NYQT;  // KT = y-pass tiles per plane (0: no y pass), NYQT = Nyquist tiles per item
 };
 __device__ __forceinline__ int block_excl_scan_1024(int v, int* wsum, int& total) {
@@ -155,6 +156,10 @@ __device__ __forceinline__ void build_act_lists(const ActLists& al, int b, int n
             const int bit0 = x << lg;
             pact = ((s_bits[bit0 >> 5] >> (bit0 & 31)) & ((NTY >= 32) ? 0xffffffffu : ((1u << NTY) - 1u))) ? 1 : 0;
             al.plane_act[(size_t)b * N + x] = pact;
+        }
+        if (x0 + (tid & ~31) < N) {   // whole warps: N is a multiple of 32
+            const unsigned pw = __ballot_sync(0xffffffffu, pact != 0);
+            if ((tid & 31) == 0) al.plane_bits[(size_t)b * (N >> 5) + (x >> 5)] = pw;
         }
         int tot;
         const int poff = ptot + block_excl_scan_1024(pact, wsum, tot);
@@ -632,6 +637,8 @@ struct sap_dpsr {
     int* ylist = nullptr;      // [B * (N * KT + NYQT)] (N >= 256)
     int* nact = nullptr;       // [4]
     unsigned* tile_bits = nullptr;  // [B][nbins / 32]
+    unsigned* plane_bits = nullptr; // [B][N / 32]
+    bool mask_solve = false;   // fused planes in the throughput regime: the splat pass writes no zeros for inactive planes, the solve masks them
     bool sparse = true;        // use the lists (SAP_DENSE=1 in the environment of sap_dpsr_create: every tile is processed)
     bool lists_valid = false;  // the lists belong to the bins in the workspace (the latency path does not write them)
     // staging for the *_host entry points (allocated on first use)
@@ -846,6 +853,7 @@ template <int N> struct Runner {
         const bool listed = (MODE == MODE_FWD3 || MODE == MODE_INV3) && h->sparse && h->lists_valid;
         p.ylist = listed ? h->ylist : nullptr; p.nact = h->nact;
         p.tile_bits = h->tile_bits;
+        p.plane_bits = (MODE == MODE_SOLVE && h->sparse && h->mask_solve) ? h->plane_bits : nullptr;
         p.cs = (float)((2.0 / ((double)N * N * N)) / (-2.0 * 3.14159265358979323846));
         const long long total = (long long)units * (N * (H / RC::W) + N / RC::W);
         long long grid = (long long)RC::MINB * h->num_sms;
@@ -945,7 +953,7 @@ template <int N> struct Runner {
             const dim3 gp((P + 255) / 256, B);
             constexpr int KT = C::FUSED_ZY ? 0 : H / RingCfg<N>::W, NYQT = C::FUSED_ZY ? 0 : N / RingCfg<N>::W;
             static_assert(C::FUSED_ZY || RingCfg<N>::W == 16, "ylist is sized for 16-column y-pass tiles");
-            const ActLists al{h->plane_act, h->sparse ? h->zlist : nullptr, h->ylist, h->nact, h->tile_bits, N, N / C::NL, KT, NYQT};
+            const ActLists al{h->plane_act, h->sparse ? h->zlist : nullptr, h->ylist, h->nact, h->tile_bits, h->plane_bits, N, N / C::NL, KT, NYQT};
             // one launch when every point fits the registers of a co-resident grid (BIN_PPT per thread), else three
             const int gx = (int)gp.x < h->bin_gx_max ? (int)gp.x : h->bin_gx_max;
             // (measured with one counter per 32-byte sector: 480,000 points 31 us against 48 us for the three kernels, 10^6 points
@@ -971,7 +979,7 @@ template <int N> struct Runner {
         // F2 z (+y) forward, 3 channels
         {
             ZyFwdParams p{h->spts, h->snrm, h->bin_start, P, nullptr, nullptr, h->S3, C::FUSED_ZY ? h->Q3 : h->QT3, h->tw, 3, h->nmax,
-                          (!C::FUSED_ZY && h->sparse) ? h->plane_act : nullptr, sorted_in_one ? h->bin_cnt : nullptr, B * h->nbins * BIN_CS, h->bsync};
+                          (h->sparse && (!C::FUSED_ZY || h->mask_solve)) ? h->plane_act : nullptr, sorted_in_one ? h->bin_cnt : nullptr, B * h->nbins * BIN_CS, h->bsync};
             if constexpr (C::FUSED_ZY)
                 launch_pdl(k_zy_fwd<N, C::NL, C::FUSED_ZY, SRC_SPLAT, C::NT_ZY>, dim3(N * N / C::NL, B * 3), dim3(C::NT_ZY), zy_smem_bytes<N, C::NL>(), st, p);
             else
@@ -1089,7 +1097,7 @@ static void free_all(sap_dpsr* h) {
     cudaFree(h->v); cudaFree(h->spts); cudaFree(h->snrm); cudaFree(h->bin_cnt); cudaFree(h->bin_cursor); cudaFree(h->bin_start); cudaFree(h->S3); cudaFree(h->Q3); cudaFree(h->S1); cudaFree(h->Q1); cudaFree(h->QT3); cudaFree(h->QT1); cudaFree(h->tw); cudaFree(h->ftab);
     cudaFree(h->fhist); cudaFree(h->facc); cudaFree(h->fsync); cudaFree(h->fstamps);
     cudaFree(h->bsync);
-    cudaFree(h->tile_bits); cudaFree(h->plane_act); cudaFree(h->zlist); cudaFree(h->ylist); cudaFree(h->nact);
+    cudaFree(h->tile_bits); cudaFree(h->plane_bits); cudaFree(h->plane_act); cudaFree(h->zlist); cudaFree(h->ylist); cudaFree(h->nact);
     cudaFree(h->gmse); cudaFree(h->acc_mse); cudaFree(h->acc); cudaFree(h->ticket); cudaFree(h->stats); cudaFree(h->bw); cudaFree(h->nmax);
     cudaFree(h->h_pts); cudaFree(h->h_nrm); cudaFree(h->h_chi); cudaFree(h->h_gchi); cudaFree(h->h_gp); cudaFree(h->h_gn);
 }
@@ -1141,6 +1149,11 @@ extern "C" sap_status_t sap_dpsr_create(int N, float sigma, int batch, int max_p
         if (N >= 256) upd(dev_alloc(h, &h->ylist, B * ((size_t)N * (N / 2 / 16) + N / 16)));
         upd(dev_alloc(h, &h->nact, (size_t)4));
         upd(dev_alloc(h, &h->tile_bits, B * (size_t)(h->nbins / 32)));
+        upd(dev_alloc(h, &h->plane_bits, B * (size_t)(N / 32)));
+        // Measured: at 128^3 x 32 the splat pass drops from 224 to 192 us when it need not write the zeros of the inactive planes and
+        // the (memory-bound) solve is not slower for masking them; with one grid in flight the masks cost the solve 1.7 us and
+        // buy nothing, and for N >= 256 they cost the instruction-bound solve more than the z pass gains
+        h->mask_solve = N <= 128 && (long long)batch * N >= 4LL * h->num_sms;
     }
     h->fused_ok = (N <= 128) && ((long long)batch * N <= h->num_sms) && batch <= (N == 32 ? 4 : N == 64 ? 2 : 1);
     if (h->fused_ok) {

@@ -128,9 +128,9 @@ SAP_HD void zy_fwd_body(Ctx& ctx, const ZyFwdParams& p, float2* smem, int bx, in
         total += b_n[k];
     }
     if (SRC == SRC_SPLAT && total == 0) {  // nothing lands here: the spectrum of zeros is zeros (before any other work)
-        // inactive plane: the y pass (in place on channels 0 and 1) does not touch it and the x pass reads the zeros of
-        // channels 0 and 1 as the y pass's output; nobody reads channel 2
-        const bool skip_main = !DO_Y && ch == 2 && p.plane_act && p.plane_act[(size_t)item * N + x] == 0;
+        // fused planes with the solve's plane masks on (plane_act set): the solve reads the rows of an inactive plane as zeros
+        // whatever the spectrum holds there, nobody has to write them
+        const bool skip_main = p.plane_act != nullptr;
         float4* So4 = reinterpret_cast<float4*>(So);
         if (!skip_main)
             for (int i = ctx.tid; i < NL * H / 2; i += ctx.nthr) So4[i] = make_float4(0.f, 0.f, 0.f, 0.f);

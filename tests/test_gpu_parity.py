@@ -487,9 +487,10 @@ def _run_sparse_dense(N, sigma, pts, nrm, G):
     return out
 
 
-@pytest.mark.parametrize("N,B,P", [(64, 2, 2500), (128, 3, 4000), (256, 1, 12000), (256, 2, 6000)])
+@pytest.mark.parametrize("N,B,P", [(64, 2, 2500), (64, 10, 1500), (128, 3, 4000), (256, 1, 12000), (256, 2, 6000)])
 def test_activity_lists_leave_results_unchanged(N, B, P):
     # items with very different activity: a small blob wrapping around the cube corner, a blob in the middle, a full-size shape
+    # (batch 10 at 64^3: the throughput regime in which the solve masks the inactive planes instead of reading written zeros)
     pts = np.empty((B, P, 3), np.float32)
     nrm = np.empty((B, P, 3), np.float32)
     specs = [((0.02, 0.97, 0.5), 0.06), ((0.5, 0.52, 0.47), 0.11), None]
