@@ -142,7 +142,8 @@ sap_status_t sap_dpsr_reserve(sap_dpsr_t* h, int what);
 
 /*
  * Two implementations of the same path live in the library:
- *   SAP_PATH_THROUGHPUT  one kernel per pass (13 launches per forward+backward), persistent TMA rings: every size, any batch;
+ *   SAP_PATH_THROUGHPUT  one kernel per pass (11 launches per forward+backward for N <= 128, 15 for N >= 256), persistent TMA rings:
+ *                        every size, any batch;
  *   SAP_PATH_LATENCY     the whole forward and the whole backward as ONE cooperative kernel each, phases separated by grid
  *                        barriers, planes kept in shared memory across them (N <= 128 and batch * N <= number of SMs:
  *                        the 32^3 / 64^3 / 128^3 levels of the coarse-to-fine schedule, at batch 1).
