@@ -82,6 +82,31 @@ enum { SAP_NN_AUTO = 0, SAP_NN_BRUTE = 1, SAP_NN_GRID = 2 };
 sap_status_t sap_chamfer_set_search(sap_mesh_t* h, int mode);
 
 /*
+ * The exhaustive nearest-neighbour search of sap_chamfer (M6: nn[i] = argmin_k |q_i - t_k|^2, the lowest index wins an
+ * exact tie) for callers that cannot allocate: code under CUDA graph capture, serving loops and harnesses that forbid
+ * cudaMalloc.  NO HANDLE AND NO ALLOCATION: the only scratch of the search -- one 64-bit (distance, index) key per query,
+ * merged with atomicMin by the blocks that scan different chunks of the targets -- lives in a file-scope device array of
+ * the library, SAP_NN_STATIC_MAX_QUERIES keys = 2 MiB, which every GPU that loads the library holds until the process
+ * exits.  The call makes no cudaMalloc / cudaFree and calls no allocating routine; it enqueues three kernels on `stream`
+ * (reset the keys of this call, scan, unpack) and does not synchronise.  The first call on a device also resolves the
+ * array's device address (cudaGetSymbolAddress, once per device, with that device current): make one call before a
+ * stream capture begins.
+ *   queries, nq   dev [nq][3] float, 0 <= nq <= SAP_NN_STATIC_MAX_QUERIES (nq == 0: nothing is enqueued)
+ *   targets, nt   dev [nt][3] float, nt >= 1
+ *   nn            dev [nq] int    index of the nearest target, overwritten
+ *   d2            dev [nq] float  its squared distance, overwritten
+ * Returns SAP_ERR_INVALID_ARG for null pointers, nt < 1, nq < 0 and for nq > SAP_NN_STATIC_MAX_QUERIES (the message of
+ * sap_mesh_last_error(NULL) names the limit; larger sets go through sap_chamfer and a handle), SAP_ERR_UNSUPPORTED when the
+ * device is not sm_100, SAP_ERR_CUDA for a failed launch.
+ * The array is SHARED by every call of the process on that GPU and keeps the keys of the last call: a call first resets
+ * the nq keys it uses, so consecutive calls on one stream (or otherwise ordered) are independent of one another, but two
+ * calls that OVERLAP on the GPU (different streams without an event between them, two host threads) race on it and give
+ * wrong neighbours.  Results are bit-identical to the nn_a / nn_b of sap_chamfer in SAP_NN_BRUTE mode.
+ */
+#define SAP_NN_STATIC_MAX_QUERIES 262144
+sap_status_t sap_chamfer_nn_static(const float* queries, int nq, const float* targets, int nt, int* nn, float* d2, void* stream);
+
+/*
  * The plain point update of BASELINE.json configs[3] ("iterations with a point update between them") and of the
  * fixed-gradient mode of the coarse-to-fine driver, as two small kernels instead of a dozen framework ops:
  *   eta = move / (N max |grad_points|);  points <- clip(points - eta grad_points, 0, 1 - 1e-6);  normals <- normals - eta grad_normals

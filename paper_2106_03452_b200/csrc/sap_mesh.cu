@@ -12,6 +12,8 @@
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdio.h>
+#include <atomic>
+#include <mutex>
 #include <new>
 #include <string>
 
@@ -793,6 +795,93 @@ extern "C" sap_status_t sap_chamfer_set_search(sap_mesh_t* h, int mode) {
     h->err.clear();
     if (mode != SAP_NN_AUTO && mode != SAP_NN_BRUTE && mode != SAP_NN_GRID) { h->err = "unknown search mode"; return SAP_ERR_INVALID_ARG; }
     h->nn_mode = mode;
+    return SAP_OK;
+}
+
+// ---- nearest-neighbour search without a handle and without an allocation (sap_chamfer_nn_static, sap_mesh.h) ---------------
+// The scratch of the chunked exhaustive search (k_nn_brute_chunks: one (distance, index) key per query) as a file-scope
+// device array: part of the module image, so every GPU that loads the library holds these 2 MiB until the process exits
+// and nobody calls cudaMalloc for them.  In HOST code the name below is a host-side stand-in, not a device address: the
+// entry point resolves the address once per device with cudaGetSymbolAddress (that device current) and hands the pointer
+// to the kernels.  Every call on a GPU shares the array; it keeps the keys of the last call, so a call resets the keys
+// it uses first, and calls that overlap on the GPU race on it.
+namespace sapm {
+static __device__ __align__(256) unsigned long long g_nn_static_keys[SAP_NN_STATIC_MAX_QUERIES];
+constexpr int NN_STATIC_MAX_DEVICES = 64;
+struct NnStaticDevice {
+    std::atomic<int> ready{0};             // 0: not set up, 1: set up, -1: not an sm_100 device
+    unsigned long long* keys = nullptr;    // device address of g_nn_static_keys on this device
+    int num_sms = 0;
+};
+static NnStaticDevice g_nn_static[NN_STATIC_MAX_DEVICES];
+static std::mutex g_nn_static_mu;
+// keys of this call <- all ones (= "no candidate yet", larger than every (distance, index) key)
+__global__ void k_nn_static_reset(unsigned long long* __restrict__ keys, int nq) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < nq) keys[i] = ~0ull;
+}
+// set-up of the current device: once per device, no allocation (attribute queries + the symbol's address)
+static sap_status_t nn_static_device(NnStaticDevice** out) {
+    int dev = -1;
+    if (!ok(nullptr, cudaGetDevice(&dev), "cudaGetDevice")) return SAP_ERR_CUDA;
+    if (dev < 0 || dev >= NN_STATIC_MAX_DEVICES) { g_err = "sap_chamfer_nn_static: device ordinal beyond the per-device table (64)"; return SAP_ERR_UNSUPPORTED; }
+    NnStaticDevice& d = g_nn_static[dev];
+    int st = d.ready.load(std::memory_order_acquire);
+    if (st == 0) {
+        std::lock_guard<std::mutex> lock(g_nn_static_mu);
+        st = d.ready.load(std::memory_order_acquire);
+        if (st == 0) {
+            int major = 0, sms = 0;
+            if (!ok(nullptr, cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev), "cudaDeviceGetAttribute")) return SAP_ERR_CUDA;
+            if (!ok(nullptr, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev), "cudaDeviceGetAttribute")) return SAP_ERR_CUDA;
+            if (major != 10) {
+                d.ready.store(-1, std::memory_order_release);
+                st = -1;
+            } else {
+                unsigned long long* ptr = nullptr;
+                if (!ok(nullptr, cudaGetSymbolAddress((void**)&ptr, g_nn_static_keys), "cudaGetSymbolAddress(g_nn_static_keys)")) return SAP_ERR_CUDA;
+                if (!ptr) { g_err = "cudaGetSymbolAddress returned a null address for g_nn_static_keys"; return SAP_ERR_CUDA; }
+                d.keys = ptr;
+                d.num_sms = sms > 0 ? sms : 148;
+                d.ready.store(1, std::memory_order_release);
+                st = 1;
+            }
+        }
+    }
+    if (st < 0) { g_err = "device is not sm_100 (Blackwell B200); this library has no other code path"; return SAP_ERR_UNSUPPORTED; }
+    *out = &d;
+    return SAP_OK;
+}
+}  // namespace sapm
+
+extern "C" sap_status_t sap_chamfer_nn_static(const float* queries, int nq, const float* targets, int nt, int* nn, float* d2, void* stream) {
+    g_err.clear();
+    if (!queries || !targets || !nn || !d2) { g_err = "null pointer argument"; return SAP_ERR_INVALID_ARG; }
+    if (nq < 0 || nt < 1) { g_err = "point counts out of range (nq >= 0, nt >= 1)"; return SAP_ERR_INVALID_ARG; }
+    if (nq > SAP_NN_STATIC_MAX_QUERIES) {
+        char buf[256];
+        snprintf(buf, sizeof buf, "nq = %d exceeds SAP_NN_STATIC_MAX_QUERIES = %d, the size of the library's static scratch array "
+                 "(use sap_chamfer with a handle for larger sets)", nq, SAP_NN_STATIC_MAX_QUERIES);
+        g_err = buf;
+        return SAP_ERR_INVALID_ARG;
+    }
+    if (nq == 0) return SAP_OK;
+    NnStaticDevice* d = nullptr;
+    const sap_status_t st = nn_static_device(&d);
+    if (st != SAP_OK) return st;
+    cudaStream_t s = (cudaStream_t)stream;
+    // the launch shape of sap_chamfer's exhaustive search: one block per 256 queries, the targets split over gridDim.y
+    // chunks while that leaves SMs idle; here always through the keys (a single chunk included)
+    const int gq = (nq + 255) / 256, ntiles = (nt + BF_TILE - 1) / BF_TILE;
+    int chunks = (6 * d->num_sms + gq - 1) / gq;
+    if (chunks > ntiles) chunks = ntiles;
+    if (chunks < 1) chunks = 1;
+    k_nn_static_reset<<<gq, 256, 0, s>>>(d->keys, nq);
+    if (!ok(nullptr, cudaGetLastError(), "k_nn_static_reset")) return SAP_ERR_CUDA;
+    k_nn_brute_chunks<<<dim3(gq, chunks), 256, 0, s>>>(queries, nq, nullptr, targets, nt, nullptr, d->keys);
+    if (!ok(nullptr, cudaGetLastError(), "k_nn_brute_chunks")) return SAP_ERR_CUDA;
+    k_nn_finish<<<gq, 256, 0, s>>>(d->keys, nq, nullptr, nn, d2);
+    if (!ok(nullptr, cudaGetLastError(), "k_nn_finish")) return SAP_ERR_CUDA;
     return SAP_OK;
 }
 

@@ -8,8 +8,10 @@ import ctypes
 from .binding import SAP_OK, SapError, _stream_ptr, lib as _dpsr_lib
 
 EXPORTS = ["sap_mesh_create", "sap_mc_extract", "sap_mc_backward", "sap_chamfer", "sap_mc_table", "sap_mesh_destroy",
-           "sap_mesh_last_error", "sap_mesh_workspace_bytes", "sap_mesh_last_launch_count", "sap_points_sgd_step", "sap_chamfer_set_search"]
+           "sap_mesh_last_error", "sap_mesh_workspace_bytes", "sap_mesh_last_launch_count", "sap_points_sgd_step", "sap_chamfer_set_search",
+           "sap_chamfer_nn_static"]
 MC_MAX_TRI = 12
+NN_STATIC_MAX_QUERIES = 262144   # SAP_NN_STATIC_MAX_QUERIES of include/sap_mesh.h
 _ready = False
 
 
@@ -32,6 +34,8 @@ def lib():
         L.sap_points_sgd_step.restype = ci
         L.sap_chamfer_set_search.argtypes = [vp, ci]
         L.sap_chamfer_set_search.restype = ci
+        L.sap_chamfer_nn_static.argtypes = [vp, ci, vp, ci, vp, vp, vp]
+        L.sap_chamfer_nn_static.restype = ci
         L.sap_mesh_destroy.argtypes = [vp]
         L.sap_mesh_destroy.restype = None
         L.sap_mesh_last_error.argtypes = [vp]
@@ -60,6 +64,23 @@ def sgd_step(points, normals, grad_points, grad_normals, N, move, scratch, strea
                                    int(points.numel()), int(N), float(move), ctypes.c_void_p(scratch.data_ptr()), _stream_ptr(stream))
     if st != SAP_OK:
         raise SapError(st, "sap_points_sgd_step")
+
+
+def nn_static(queries, targets, nn, d2, stream=None):
+    """sap_chamfer_nn_static: exact nearest target of every query (CUDA float32 [nq,3] / [nt,3], contiguous) into the
+    caller's nn (int32 [nq]) and d2 (float32 [nq]).  No handle, no allocation on either side of the ABI: the scratch is the
+    library's static device array (at most NN_STATIC_MAX_QUERIES queries; calls that overlap on the GPU race on it)."""
+    import torch
+    nq, nt = int(queries.shape[0]), int(targets.shape[0])
+    for t, dt, shape, name in ((queries, torch.float32, (nq, 3), "queries"), (targets, torch.float32, (nt, 3), "targets"),
+                               (nn, torch.int32, (nq,), "nn"), (d2, torch.float32, (nq,), "d2")):
+        if not (t.is_cuda and t.dtype == dt and tuple(t.shape) == shape and t.is_contiguous()):
+            raise ValueError(f"{name}: expected a contiguous CUDA {dt} tensor of shape {shape}")
+    L = lib()
+    st = L.sap_chamfer_nn_static(ctypes.c_void_p(queries.data_ptr()), nq, ctypes.c_void_p(targets.data_ptr()), nt,
+                                 ctypes.c_void_p(nn.data_ptr()), ctypes.c_void_p(d2.data_ptr()), _stream_ptr(stream))
+    if st != SAP_OK:
+        raise SapError(st, (L.sap_mesh_last_error(None) or b"sap_chamfer_nn_static").decode())
 
 
 class Mesh:
