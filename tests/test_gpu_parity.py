@@ -516,6 +516,50 @@ def test_activity_lists_leave_results_unchanged(N, B, P):
         _check_item(N, 2.0, pts[b], nrm[b], G[b], s["chi"][b], s["stats"][b], s["gp"][b], s["gn"][b])
 
 
+@pytest.mark.parametrize("N,path", [(64, "latency"), (64, "throughput"), (128, "throughput"), (256, "throughput")])
+def test_all_points_in_one_cell_and_a_volume_filling_cloud(N, path):
+    # the two ends of the activity range, one item each in one batch:
+    #  - 3000 points inside ONE cell with nearly parallel normals: every contribution lands on the same 8 nodes (the
+    #    worst case of the shared-memory atomics and of the fixed-point scale, which is set from count x largest
+    #    component), one or two active planes, every other plane / tile skipped by the listed kernels;
+    #  - points uniform in the whole cube with random normals: every bin non-empty, every tile active (lists = dense)
+    P, sigma = 3000, 2.0
+    rng = np.random.default_rng(N)
+    pts = np.empty((2, P, 3), np.float32)
+    nrm = np.empty((2, P, 3), np.float32)
+    cell = np.array([N // 2 + 3, N - 1, 17 % N], np.float64)        # the y index is the last cell: its +1 corner wraps
+    pts[0] = ((cell[None] + rng.uniform(0.05, 0.95, (P, 3))) / N).astype(np.float32)
+    d = np.array([0.3, -0.5, 0.81]) + 0.05 * rng.normal(size=(P, 3))
+    nrm[0] = (d / np.linalg.norm(d, axis=1, keepdims=True)).astype(np.float32)
+    pts[1] = rng.uniform(0.0, 1.0, (P, 3)).astype(np.float32).clip(0.0, np.float32(1.0 - 6e-8))
+    d = rng.normal(size=(P, 3))
+    nrm[1] = (d / np.linalg.norm(d, axis=1, keepdims=True)).astype(np.float32)
+    G = inputs.upstream_grad(N, 2, seed=21)
+    r = _gpu_run(N, sigma, pts, nrm, G, path)
+    _check_item(N, sigma, pts[1], nrm[1], G[1], r["chi"][1], r["stats"][1], r["gp"][1], r["gn"][1])
+    t0, p0 = _active_counts(N, pts[0])
+    assert p0 == 2 and t0 <= 4                                       # one cell touches planes x and x + 1 only
+    # Item 0 is the degenerate case of Eq.4 itself (reading R5 of DESIGN.md): a cloud inside one cell is a dipole, chi' is
+    # antisymmetric about it, so its mean over the points m and chi'[0] are both ~1e-4 of max|chi'| and the scale
+    # s = 0.5 / |chi'[0] - m| divides by their difference a.  An ABSOLUTE error eps max|chi'| of the float32 field (all
+    # samples read the same 8 nodes: it does not average out) becomes a RELATIVE error eps kappa of s, kappa = max|chi'| / |a|,
+    # in chi and in every gradient.  So: chi' and the statistics to the float32 bar, chi and the gradients to the bar times kappa.
+    f = orc.forward(N, sigma, pts[0], nrm[0])
+    chip_o = f["chi"] / f["s"] + f["mu"]
+    M = np.abs(chip_o).max()
+    kappa, eps = M / abs(f["a"]), 1e-6
+    assert kappa > 500                                               # the case is what it claims to be (776 at 64^3, 4900 at 256^3)
+    mu, a, sc = r["stats"][0][0], r["stats"][0][1], r["stats"][0][2]
+    chip = r["chi"][0].astype(np.float64) / sc + mu
+    assert np.abs(chip - chip_o).max() <= eps * M
+    assert abs(mu - f["mu"]) <= eps * M and abs(a - f["a"]) <= eps * M
+    bar = 2 * eps * kappa
+    assert np.abs(r["chi"][0] - f["chi"]).max() <= max(CHI_TOL, bar) * np.abs(f["chi"]).max()
+    bo = orc.backward(N, sigma, pts[0], nrm[0], f, G[0])
+    for got, want in ((r["gp"][0], bo["grad_points"]), (r["gn"][0], bo["grad_normals"])):
+        assert np.linalg.norm(got - want) <= max(GRAD_TOL, bar) * np.linalg.norm(want)
+
+
 def test_single_launch_binning_matches_the_three_kernel_fallback(monkeypatch):
     # k_bin_sort (one cooperative launch) against k_bin_count / k_bin_scan / k_bin_scatter: same bins; the order of the
     # points inside a bin differs, which only reorders float sums in the point mean and nothing in the fixed-point splat
