@@ -153,14 +153,34 @@ template <int R, bool INV> SAP_HD void dft_dir(float2 (&v)[R]) {
         for (int i = 0; i < R / 2; ++i) { e[i] = v[2 * i]; o[i] = v[2 * i + 1]; }
         dft_dir<R / 2, INV>(e);
         dft_dir<R / 2, INV>(o);
+        // v[k] = e + t, v[k + R/2] = e - t with t = o w^k (forward) or o conj(w^k) (inverse).  The roots are compile-time
+        // constants: written so that each enters as a SCALAR immediate of a packed instruction and the rotations +-i o as
+        // operand modifiers (half swap + per-half negate).  A constant PAIR (wr, wi) would have to sit in two registers, and
+        // at the register budget of these kernels the compiler rebuilt such pairs with two MOVs per use (10-12 % of all
+        // executed instructions).  t = wr o + wi (i o) [forward; -i o inverse]:
+        //   general root:            e +- t = fma(+-wi, rot, fma(+-wr, o, e))                     4 packed instructions
+        //   w = c (+-1 - i) (k = R/8, 3R/8):  t = c s, s = rot' +- o,  e +- t = fma(+-c, s, e)    3 instead of 4
 #pragma unroll
         for (int k = 0; k < R / 2; ++k) {
-            float2 t;
-            if (k == 0) t = o[k];
-            else if (k == R / 4) t = INV ? mul_pi(o[k]) : mul_mi(o[k]);
-            else t = INV ? cmulc(o[k], unit_root<R>(k)) : cmul(o[k], unit_root<R>(k));
-            v[k] = cadd(e[k], t);
-            v[k + R / 2] = csub(e[k], t);
+            if (k == 0) {
+                v[k] = cadd(e[k], o[k]);
+                v[k + R / 2] = csub(e[k], o[k]);
+            } else if (k == R / 4) {
+                const float2 t = INV ? mul_pi(o[k]) : mul_mi(o[k]);
+                v[k] = cadd(e[k], t);
+                v[k + R / 2] = csub(e[k], t);
+            } else if (R >= 8 && (8 * k == R || 8 * k == 3 * R)) {
+                constexpr float c = 0.70710678118654752f;
+                const float2 r = INV ? mul_pi(o[k]) : mul_mi(o[k]);
+                const float2 sm = (8 * k == R) ? cadd(r, o[k]) : csub(r, o[k]);
+                v[k] = caxpy(c, sm, e[k]);
+                v[k + R / 2] = caxpy(-c, sm, e[k]);
+            } else {
+                const float2 w = unit_root<R>(k);   // (wr, wi), folded to immediates (k is an unrolled constant)
+                const float2 rot = INV ? mul_mi(o[k]) : mul_pi(o[k]);
+                v[k] = caxpy(w.y, rot, caxpy(w.x, o[k], e[k]));
+                v[k + R / 2] = caxpy(-w.y, rot, caxpy(-w.x, o[k], e[k]));
+            }
         }
     }
 }
