@@ -216,6 +216,29 @@ SAP_HD void bfly_inv(float2 (&v)[StageInfo<N, S>::R], int j, const float2* tw) {
 
 // r2c / c2r pair formulas on single values (see r2c_split / c2r_split below for the derivation).
 // w = exp(-2 pi i k / N).  In: a = Z[k], b = Z[H-k].  Out: a = X[k], b = X[H-k].
+// Device path: packed (7 instructions instead of 12; bit-identical: the halvings are exact): t = a + conj b = 2 E,
+// u = a - conj b = 2 D, g = (u / 2) w, X[k] = t / 2 - i g, X[H-k] = conj(t / 2 + i g).
+#ifdef __CUDA_ARCH__
+SAP_HD void r2c_pair(float2& a, float2& b, float2 w) {
+    const float2 half = make_float2(0.5f, 0.5f);
+    const float2 t = __fadd2_rn(a, make_float2(b.x, -b.y));
+    const float2 u = __fadd2_rn(a, make_float2(-b.x, b.y));
+    const float2 g = cmul(__fmul2_rn(u, half), w);
+    a = __ffma2_rn(t, half, make_float2(g.y, -g.x));
+    const float2 q = __ffma2_rn(t, half, make_float2(-g.y, g.x));
+    b = make_float2(q.x, -q.y);
+}
+// t = a + conj b = 2 E, u = a - conj b = 2 D, o = (u / 2) conj w, Z[k] = t / 2 + i o, Z[H-k] = conj(t / 2 - i o)
+SAP_HD void c2r_pair(float2& a, float2& b, float2 w) {
+    const float2 half = make_float2(0.5f, 0.5f);
+    const float2 t = __fadd2_rn(a, make_float2(b.x, -b.y));
+    const float2 u = __fadd2_rn(a, make_float2(-b.x, b.y));
+    const float2 o = cmulc(__fmul2_rn(u, half), w);
+    a = __ffma2_rn(t, half, make_float2(-o.y, o.x));
+    const float2 q = __ffma2_rn(t, half, make_float2(o.y, -o.x));
+    b = make_float2(q.x, -q.y);
+}
+#else
 SAP_HD void r2c_pair(float2& a, float2& b, float2 w) {
     float2 e = make_float2(0.5f * (a.x + b.x), 0.5f * (a.y - b.y));
     float2 d = make_float2(0.5f * (a.x - b.x), 0.5f * (a.y + b.y));
@@ -235,6 +258,7 @@ SAP_HD void c2r_pair(float2& a, float2& b, float2 w) {
     float2 g = csub(e, io);
     b = make_float2(g.x, -g.y);
 }
+#endif
 
 // ---- one radix stage over a set of lines in shared memory --------------------------------------
 // Element n of line l lives at s[l * LS + n * ES].  tw is the table exp(-2 pi i t / TWN), t < TWN,
