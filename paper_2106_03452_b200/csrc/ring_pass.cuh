@@ -656,7 +656,7 @@ __global__ void __launch_bounds__(ring_threads<N, MODE>(), RingCfgM<N, MODE>::MI
 #pragma unroll
                 for (int r = 0; r < RL; ++r) {
                     const float f = mult_fc(fx[blk * RL + r], mc);
-                    acc[i][r] = make_float2(f * v[r].y, -f * v[r].x);
+                    acc[i][r] = cscale(f, mul_mi(v[r]));   // -i f v: one packed multiply (half swap + negate are operand modifiers)
                 }
             }
 #pragma unroll

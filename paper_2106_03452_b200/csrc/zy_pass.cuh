@@ -205,11 +205,11 @@ SAP_HD void zy_fwd_body(Ctx& ctx, const ZyFwdParams& p, float2* smem, int bx, in
 #pragma unroll
             for (int r = 0; r < R0; ++r) {
                 const int2 iv = reinterpret_cast<const int2*>(s)[(q + ST0 * r) * PITCH + l];   // fixed-point sums
-                float2 xv = make_float2(fs.invS * (float)iv.x, fs.invS * (float)iv.y);
+                float2 xv = cscale(fs.invS, make_float2((float)iv.x, (float)iv.y));
                 if (SRC == SRC_GBAR) {
                     const int e = l * H + q + ST0 * r;
                     const float2 g = g2[e];
-                    xv = make_float2(cs_ * g.x + cw * xv.x, cs_ * g.y + cw * xv.y);
+                    xv = caxpy(cs_, g, cscale(cw, xv));
                     if (line0 == 0 && e == 0) xv.x -= c0;
                 }
                 v[r] = xv;
