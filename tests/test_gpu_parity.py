@@ -577,6 +577,27 @@ def test_single_launch_binning_matches_the_three_kernel_fallback(monkeypatch):
     _check_item(N, 2.0, pts, nrm, G[0], a["chi"][0], a["stats"][0], a["gp"][0], a["gn"][0])
 
 
+def test_binning_with_several_points_per_thread_and_a_batch(monkeypatch):
+    # from 65,536 points per item on k_bin_sort gives every thread four points (fewer blocks scan the counts and meet at the
+    # grid barrier): two items of 70,000 points at 64^3, against the three-kernel binning and against the oracle
+    N, P, B = 64, 70000, 2
+    pts = np.empty((B, P, 3), np.float32)
+    nrm = np.empty((B, P, 3), np.float32)
+    pts[0], nrm[0] = inputs.make_cloud("torus", P, seed=61)
+    pts[1], nrm[1] = inputs.make_cloud("ellipsoids3", P, seed=62)
+    G = inputs.upstream_grad(N, B, seed=13)
+    a = _gpu_run(N, 2.0, pts, nrm, G, path="throughput")
+    monkeypatch.setenv("SAP_BIN3", "1")
+    b = _gpu_run(N, 2.0, pts, nrm, G, path="throughput")
+    monkeypatch.delenv("SAP_BIN3")
+    assert a["fwd_launches"] + 2 == b["fwd_launches"]
+    assert np.abs(a["chi"] - b["chi"]).max() <= 2e-6 * np.abs(b["chi"]).max()
+    assert np.linalg.norm(a["gp"] - b["gp"]) <= 1e-5 * np.linalg.norm(b["gp"])
+    assert np.linalg.norm(a["gn"] - b["gn"]) <= 1e-5 * np.linalg.norm(b["gn"])
+    for i in range(B):
+        _check_item(N, 2.0, pts[i], nrm[i], G[i], a["chi"][i], a["stats"][i], a["gp"][i], a["gn"][i])
+
+
 def test_forward_on_one_path_backward_on_the_other_with_lists():
     # the latency path writes no activity lists: a throughput backward after it must fall back to every tile
     import torch
